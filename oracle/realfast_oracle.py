@@ -1,0 +1,211 @@
+"""Plain float64 CPU oracle of the realfast search loop.  TEST INFRASTRUCTURE.
+
+Slow, unblocked, unfused: each function is the definition written out, in the
+order the paper gives it (PAPER.md = /root/reference/PAPER.md; readings A1-A20
+are DESIGN.md "Readings", taken from SURVEY.md section 8(c)).
+
+    O1  delay table            PAPER.md:45 (footnote 1: tau = 4.15 ms DM / nu^2)
+    O2  uv cell table          PAPER.md:72, 84 (FFT imaging, no gridding kernel)
+    O3  dedisperse + resample  PAPER.md:63, 104 (loops over DM and sampling time), 118
+    O4  gridding
+    O5  2-D FFT Stokes-I image PAPER.md:88, 118
+    O6  peak and robust sigma  PAPER.md:86-88 ("thresholding each image")
+    O7  threshold              PAPER.md:88 ("S/N greater than a threshold")
+
+Pins (tests/test_oracle_pins.py): every function below is pinned to something
+other than itself -- closed forms, exact rational arithmetic, a direct DFT,
+Parseval, the analytic noise variance, an injected source, brute force.  The
+one free choice the paper does not fix is the sigma ESTIMATOR (reading A9:
+1.4826 x MAD over all pixels): "parity unpinned" by the paper for that choice;
+it is pinned only statistically (MAD-sigma ~ rms ~ analytic value on noise).
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / reference
+legs may import this module.  It imports nothing from the CUDA package.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass
+from typing import Iterable, List, Optional, Sequence, Tuple
+
+import numpy as np
+
+K_DM = 4.148808e-3      # s GHz^2 cm^3/pc; reading A1 (paper prints 4.15 ms)
+C_LIGHT = 299792458.0   # m/s
+MAD_TO_SIGMA = 1.4826   # reading A9
+
+
+@dataclass(frozen=True)
+class Candidate:
+    dm_idx: int
+    dt_idx: int
+    t_idx: int      # index j in the dt-resampled series
+    l_pix: int      # signed x offset in [-npix/2, npix/2)
+    m_pix: int      # signed y offset
+    peak: float
+    sigma: float
+    snr: float
+
+    @property
+    def key(self) -> Tuple[int, int, int]:
+        return (self.dm_idx, self.dt_idx, self.t_idx)
+
+
+# --------------------------------------------------------------------------- O1
+def delay_table(freqs_hz: np.ndarray, dm_list: np.ndarray, inttime_s: float) -> np.ndarray:
+    """int32 [ndm][nchan]: dispersion delay in whole integrations relative to the
+    highest channel (readings A1, A3, A4: round half up)."""
+    f = np.asarray(freqs_hz, dtype=np.float64) / 1e9
+    fmax = f.max()
+    dm = np.asarray(dm_list, dtype=np.float64)[:, None]
+    # elementwise IEEE float64, evaluated left to right exactly as written (A4)
+    x = K_DM * dm * (1.0 / (f * f) - 1.0 / (fmax * fmax))[None, :] / inttime_s
+    return np.floor(x + 0.5).astype(np.int32)
+
+
+# --------------------------------------------------------------------------- O2
+def cell_table(uvw_m: np.ndarray, freqs_hz: np.ndarray, npix: int, cell_rad: float,
+               chan_weights: Optional[np.ndarray] = None):
+    """(iu, iv, keep): int32 [nbl][nchan] signed cell indices and the kept mask.
+
+    u_lambda = u_m f / c; cell size du = 1/(npix*cell); nearest cell, round half
+    up; kept iff inside [-npix/2, npix/2) on both axes and channel weight != 0
+    (readings A8, A17).  w is ignored (A8)."""
+    uvw = np.asarray(uvw_m, dtype=np.float64)
+    f = np.asarray(freqs_hz, dtype=np.float64)
+    du = 1.0 / (npix * cell_rad)
+    half = npix // 2
+    ul = uvw[:, 0:1] * f[None, :] / C_LIGHT          # [nbl][nchan], (u*f)/c in this order
+    vl = uvw[:, 1:2] * f[None, :] / C_LIGHT
+    iu = np.floor(ul / du + 0.5).astype(np.int32)
+    iv = np.floor(vl / du + 0.5).astype(np.int32)
+    keep = (iu >= -half) & (iu < half) & (iv >= -half) & (iv < half)
+    if chan_weights is not None:
+        keep &= (np.asarray(chan_weights) != 0)[None, :]
+    return iu, iv, keep
+
+
+# --------------------------------------------------------------------------- O3
+def n_images(nint: int, max_delay: int, dt: int, span: int = 0) -> int:
+    """Number of output indices j of one (dm, dt): all j with (j+1)*dt <= n_search.
+
+    n_search = nint - max_ch delay[dm] for a single segment (reading A16) or
+    min(that, span) when a streaming search span is set (config 5)."""
+    n_search = nint - max_delay
+    if span > 0:
+        n_search = min(n_search, span)
+    return max(0, n_search // dt)
+
+
+def dedisperse_resample(vis: np.ndarray, delay_dm: np.ndarray, dt: int, j: int) -> np.ndarray:
+    """complex128 [nbl][nchan]: Stokes-I visibility of resampled integration j.
+
+    s[bl][ch] = mean over q < dt and over pol of vis[j*dt + q + delay[ch]][bl][ch][pol]
+    (readings A5 native-resolution delays, A6 decimating boxcar, A7 Stokes I = pol mean)."""
+    nint, nbl, nchan, npol = vis.shape
+    s = np.zeros((nbl, nchan), dtype=np.complex128)
+    for c in range(nchan):
+        for q in range(dt):
+            t = j * dt + q + int(delay_dm[c])
+            s[:, c] += vis[t, :, c, :].astype(np.complex128).sum(axis=1)
+    return s / (dt * npol)
+
+
+# --------------------------------------------------------------------------- O4
+def grid_visibilities(s: np.ndarray, iu: np.ndarray, iv: np.ndarray, keep: np.ndarray,
+                      npix: int) -> np.ndarray:
+    """complex128 [npix][npix] grid G[iv mod N][iu mod N] += s and its Hermitian
+    conjugate at the mirrored cell (reading A8; no fftshift in storage, A12)."""
+    g = np.zeros((npix, npix), dtype=np.complex128)
+    a = iu[keep].astype(np.int64)
+    e = iv[keep].astype(np.int64)
+    val = s[keep]
+    np.add.at(g, (e % npix, a % npix), val)                 # unbuffered scatter-add
+    np.add.at(g, ((-e) % npix, (-a) % npix), np.conj(val))
+    return g
+
+
+# --------------------------------------------------------------------------- O5
+def image_from_grid(g: np.ndarray, n_w: int) -> np.ndarray:
+    """float64 [npix][npix]: Re(ifft2(G)) * N^2 / (2 N_w); a unit point source at
+    the phase centre gives 1.0 (reading A8).  numpy ifft2 has the +i sign."""
+    n = g.shape[0]
+    return np.real(np.fft.ifft2(g)) * (n * n) / (2.0 * n_w)
+
+
+def image_direct_dft(s: np.ndarray, iu: np.ndarray, iv: np.ndarray, keep: np.ndarray,
+                     npix: int) -> np.ndarray:
+    """The same image as the direct sum (1/N_w) sum_kept Re(s e^{+2 pi i (iu x + iv y)/N});
+    O(N^2 N_vis): tiny grids only.  Used to pin O4+O5."""
+    n_w = int(keep.sum())
+    y, x = np.mgrid[0:npix, 0:npix]
+    img = np.zeros((npix, npix), dtype=np.float64)
+    nbl, nchan = s.shape
+    for b in range(nbl):
+        for c in range(nchan):
+            if keep[b, c]:
+                ph = 2.0 * np.pi * (int(iu[b, c]) * x + int(iv[b, c]) * y) / npix
+                img += s[b, c].real * np.cos(ph) - s[b, c].imag * np.sin(ph)
+    return img / n_w
+
+
+# --------------------------------------------------------------------------- O6
+def image_stats(img: np.ndarray):
+    """(peak, y, x, sigma, snr): maximum pixel (first in row-major order on ties),
+    sigma = 1.4826 * median(|img - median(img)|) over all pixels, snr = peak/sigma
+    (0 when sigma == 0) -- readings A9, A10."""
+    flat = img.reshape(-1)
+    k = int(np.argmax(flat))
+    peak = float(flat[k])
+    y, x = divmod(k, img.shape[1])
+    med = float(np.median(flat))
+    sigma = MAD_TO_SIGMA * float(np.median(np.abs(flat - med)))
+    snr = peak / sigma if sigma > 0.0 else 0.0
+    return peak, y, x, sigma, snr
+
+
+# --------------------------------------------------------------------------- O3-O7
+def search_image(vis, delays, iu, iv, keep, npix, dm_idx, dt, j) -> np.ndarray:
+    """Image of one (dm, dt, j): O3 -> O4 -> O5."""
+    s = dedisperse_resample(vis, delays[dm_idx], dt, j)
+    g = grid_visibilities(s, iu, iv, keep, npix)
+    return image_from_grid(g, int(keep.sum()))
+
+
+def search(vis: np.ndarray, freqs_hz, uvw_m, inttime_s: float, npix: int, cell_rad: float,
+           dm_list, dt_list: Sequence[int], threshold: float,
+           chan_weights: Optional[np.ndarray] = None, span: int = 0,
+           keys: Optional[Iterable[Tuple[int, int, int]]] = None,
+           return_all_stats: bool = False):
+    """The whole loop of Fig. 2 for one segment.
+
+    Returns the list of Candidate with snr >= threshold (order: dm, dt, j).  With
+    ``keys`` only those (dm_idx, dt_idx, j) are evaluated (sampled parity at full
+    sizes).  With ``return_all_stats`` also returns {key: (peak,y,x,sigma,snr)}.
+    """
+    nint = vis.shape[0]
+    delays = delay_table(freqs_hz, dm_list, inttime_s)
+    iu, iv, keep = cell_table(uvw_m, freqs_hz, npix, cell_rad, chan_weights)
+    n_w = int(keep.sum())
+    cands: List[Candidate] = []
+    stats = {}
+    if keys is None:
+        keys = []
+        for d in range(len(dm_list)):
+            md = int(delays[d].max())
+            for k, dt in enumerate(dt_list):
+                keys.extend((d, k, j) for j in range(n_images(nint, md, dt, span)))
+    for (d, k, j) in keys:
+        dt = int(dt_list[k])
+        s = dedisperse_resample(vis, delays[d], dt, j)
+        g = grid_visibilities(s, iu, iv, keep, npix)
+        img = image_from_grid(g, n_w) if n_w > 0 else np.zeros((npix, npix))
+        peak, y, x, sigma, snr = image_stats(img)
+        if return_all_stats:
+            stats[(d, k, j)] = (peak, y, x, sigma, snr)
+        if snr >= threshold:
+            l = x if x < npix // 2 else x - npix
+            m = y if y < npix // 2 else y - npix
+            cands.append(Candidate(d, k, j, l, m, peak, sigma, snr))
+    if return_all_stats:
+        return cands, stats
+    return cands

@@ -1,0 +1,241 @@
+"""Pins for the oracle's dedispersion, gridding, imaging, statistics and the whole loop
+(O3-O7): direct DFT, Parseval, analytic noise variance, closed-form source response,
+linearity, shift invariance and a pure-Python brute force.  CPU only."""
+import cmath
+import math
+
+import numpy as np
+import pytest
+
+import oracle as O
+import workloads as W
+from workloads.generate import Transient
+
+
+def _setup(name="tiny"):
+    cfg = W.get_config(name)
+    f = W.channel_freqs_hz(cfg)
+    uvw = W.baseline_uvw_m(cfg)
+    cell = W.default_cell_rad(cfg, uvw)
+    dms = W.dm_list(cfg)
+    delays = O.delay_table(f, dms, cfg.inttime_s)
+    iu, iv, keep = O.cell_table(uvw, f, cfg.npix, cell)
+    return cfg, f, uvw, cell, dms, delays, iu, iv, keep
+
+
+# ------------------------------------------------------------------ O4 + O5
+def test_fft_image_equals_direct_dft():
+    """P5: gridded-FFT image == direct sum over samples; ifft2 imaginary part vanishes;
+    image mean is 0 when no sample lands in cell (0,0)."""
+    cfg, f, uvw, cell, dms, delays, iu, iv, keep = _setup()
+    vis = W.make_segment(cfg)
+    s = O.dedisperse_resample(vis, delays[3], 1, 7)
+    g = O.grid_visibilities(s, iu, iv, keep, cfg.npix)
+    img = O.image_from_grid(g, int(keep.sum()))
+    ref = O.image_direct_dft(s, iu, iv, keep, cfg.npix)
+    assert np.abs(img - ref).max() < 1e-12 * np.abs(ref).max() * 100
+    full = np.fft.ifft2(g)
+    assert np.abs(full.imag).max() < 1e-14 * np.abs(full.real).max() * 100
+    assert not ((iu == 0) & (iv == 0) & keep).any()
+    assert abs(img.mean()) < 1e-15
+
+
+def test_parseval():
+    """P6: mean(img^2) = sum|G|^2 / (2 N_w)^2."""
+    cfg, f, uvw, cell, dms, delays, iu, iv, keep = _setup()
+    vis = W.make_segment(cfg)
+    s = O.dedisperse_resample(vis, delays[1], 1, 3)
+    g = O.grid_visibilities(s, iu, iv, keep, cfg.npix)
+    img = O.image_from_grid(g, int(keep.sum()))
+    lhs = (img ** 2).mean()
+    rhs = (np.abs(g) ** 2).sum() / (2.0 * keep.sum()) ** 2
+    assert abs(lhs - rhs) < 1e-13 * rhs
+
+
+def test_unit_source_at_phase_centre_gives_one():
+    """A8 normalisation; also Stokes I = mean of the pols (A7)."""
+    cfg, f, uvw, cell, dms, delays, iu, iv, keep = _setup()
+    vis = np.zeros((cfg.nint, cfg.nbl, cfg.nchan, cfg.npol), dtype=np.complex64)
+    vis[5, :, :, 0] = 1.5
+    vis[5, :, :, 1] = 0.5
+    img = O.search_image(vis, delays, iu, iv, keep, cfg.npix, 0, 1, 5)
+    assert abs(img[0, 0] - 1.0) < 1e-12 and img.max() == img[0, 0]
+
+
+def test_noise_variance_analytic():
+    """P7: pure noise with unit variance per part -> pixel variance 1/(N_w N_pol);
+    the MAD sigma agrees with the rms sigma on noise."""
+    cfg, f, uvw, cell, dms, delays, iu, iv, keep = _setup()
+    vis = W.make_segment(cfg, inject=False)
+    n_w = int(keep.sum())
+    ms, mads = [], []
+    for t in range(cfg.nint):
+        img = O.search_image(vis, delays, iu, iv, keep, cfg.npix, 0, 1, t)
+        ms.append((img ** 2).mean())
+        mads.append(O.image_stats(img)[3])
+    expect = 1.0 / (n_w * cfg.npol)
+    assert abs(expect - 0.018634 ** 2) < 1e-3 * expect        # SURVEY P7 value for config 1
+    assert abs(np.mean(ms) - expect) < 0.03 * expect
+    assert abs(np.mean(mads) - math.sqrt(expect)) < 0.03 * math.sqrt(expect)
+
+
+# ------------------------------------------------------------------ signal
+def _closed_form_peak(uvw, f, cell, npix, iu, iv, keep, amp, l, m):
+    """P8: (A/N_w) sum cos(2 pi ((iu du - u_lambda) l + (iv du - v_lambda) m) cell)."""
+    du = 1.0 / (npix * cell)
+    ul = uvw[:, 0:1] * f[None, :] / O.C_LIGHT
+    vl = uvw[:, 1:2] * f[None, :] / O.C_LIGHT
+    ph = 2 * np.pi * ((iu * du - ul) * l + (iv * du - vl) * m) * cell
+    return amp * np.cos(ph[keep]).sum() / keep.sum()
+
+
+@pytest.mark.parametrize("width,t0", [(1, 20), (2, 10)])
+def test_noiseless_injection_closed_form(width, t0):
+    """P8 + A12: matched DM and width -> peak value by the gridding-decorrelation closed
+    form, at pixel (y, x) = (m mod N, l mod N); (8,-5) -> (59, 8)."""
+    cfg, f, uvw, cell, dms, delays, iu, iv, keep = _setup()
+    src = Transient(2.0, 8, -5, float(dms[3]), width, t0)        # DM 60 is trial 3
+    vis = W.make_segment(cfg, noise=False, sources=[src])
+    img = O.search_image(vis, delays, iu, iv, keep, cfg.npix, 3, width, t0 // width)
+    peak, y, x, sigma, snr = O.image_stats(img)
+    assert (y, x) == (59, 8)
+    expect = _closed_form_peak(uvw, f, cell, cfg.npix, iu, iv, keep, 2.0, 8, -5)
+    assert abs(peak - expect) < 1e-6 * expect      # complex64 input rounding only
+    assert 1.90 < expect < 1.99                    # 1.93 for its antenna draw
+    # a neighbouring integration holds nothing
+    other = O.search_image(vis, delays, iu, iv, keep, cfg.npix, 3, width, t0 // width + 2)
+    assert np.abs(other).max() < 1e-12
+
+
+def test_tiny_config_recovery():
+    """P10: config 1 injects DM 50 between trials 40 and 60: best candidate at trial 40 or
+    60, pixel (8,-5), arrival time near t0 = 20, S/N well above threshold."""
+    cfg, f, uvw, cell, dms, delays, iu, iv, keep = _setup()
+    vis = W.make_segment(cfg)
+    cands = O.search(vis, f, uvw, cfg.inttime_s, cfg.npix, cell, dms, cfg.dt_list, cfg.threshold)
+    assert 20 <= len(cands) <= 80
+    best = max(cands, key=lambda c: c.snr)
+    assert dms[best.dm_idx] in (40.0, 60.0)
+    assert (best.l_pix, best.m_pix) == (8, -5)
+    assert abs(best.t_idx - 20) <= 2 and 10.0 < best.snr < 30.0
+    # pure noise: nothing above 6 sigma
+    quiet = O.search(W.make_segment(cfg, inject=False), f, uvw, cfg.inttime_s, cfg.npix, cell,
+                     dms, cfg.dt_list, cfg.threshold)
+    assert len(quiet) <= 1
+
+
+# ------------------------------------------------------------------ O3 properties
+def test_boxcar_linearity_and_snapshot():
+    """P11: image(dm, dt, j) = mean_q image(dm, 1, j dt + q); DM 0, dt 1 = snapshot."""
+    cfg, f, uvw, cell, dms, delays, iu, iv, keep = _setup()
+    vis = W.make_segment(cfg)
+    for dt in (2, 4):
+        j = 3
+        a = O.search_image(vis, delays, iu, iv, keep, cfg.npix, 5, dt, j)
+        b = np.mean([O.search_image(vis, delays, iu, iv, keep, cfg.npix, 5, 1, j * dt + q)
+                     for q in range(dt)], axis=0)
+        assert np.abs(a - b).max() < 1e-12
+    snap = O.image_direct_dft(vis[9].astype(np.complex128).mean(axis=2), iu, iv, keep, cfg.npix)
+    assert np.abs(O.search_image(vis, delays, iu, iv, keep, cfg.npix, 0, 1, 9) - snap).max() < 1e-12
+
+
+def test_dedispersion_reads_delayed_rows():
+    """O3 index check: a marker placed at row t + delay[ch] in one channel only shows up at t."""
+    cfg, f, uvw, cell, dms, delays, iu, iv, keep = _setup()
+    vis = np.zeros((cfg.nint, cfg.nbl, cfg.nchan, cfg.npol), dtype=np.complex64)
+    d = delays[4]
+    ch, t = 3, 6
+    vis[t + d[ch], :, ch, :] = 1.0
+    s = O.dedisperse_resample(vis, d, 1, t)
+    assert (s[:, ch] == 1.0).all() and np.abs(s).sum() == cfg.nbl
+    assert np.abs(O.dedisperse_resample(vis, d, 1, t + 1)).sum() == 0
+    s2 = O.dedisperse_resample(vis, d, 2, t // 2)
+    assert np.allclose(s2[:, ch], 0.5)
+
+
+def test_shift_invariance():
+    """P12: delaying the input by k integrations shifts every candidate's t by k."""
+    cfg, f, uvw, cell, dms, delays, iu, iv, keep = _setup()
+    vis = W.make_segment(cfg)
+    k = 4
+    shifted = np.concatenate([W.noise_rows(cfg, range(1000, 1000 + k)), vis[:-k]])
+    a = O.search(vis, f, uvw, cfg.inttime_s, cfg.npix, cell, dms, cfg.dt_list, 8.0)
+    b = O.search(shifted, f, uvw, cfg.inttime_s, cfg.npix, cell, dms, cfg.dt_list, 8.0)
+    ka = {(c.dm_idx, c.t_idx + k): c for c in a}
+    kb = {(c.dm_idx, c.t_idx): c for c in b if c.t_idx >= k}
+    common = [key for key in ka if key in kb]
+    assert len(common) >= 5
+    for key in common:
+        assert abs(ka[key].snr - kb[key].snr) < 1e-9 and ka[key].l_pix == kb[key].l_pix
+
+
+# ------------------------------------------------------------------ O6
+def test_image_stats_known_values():
+    img = np.arange(16, dtype=np.float64).reshape(4, 4)        # median 7.5, MAD 4
+    peak, y, x, sigma, snr = O.image_stats(img)
+    assert (peak, y, x) == (15.0, 3, 3)
+    assert sigma == 1.4826 * 4.0 and snr == 15.0 / (1.4826 * 4.0)
+    tie = np.zeros((4, 4))
+    tie[1, 2] = tie[2, 1] = 3.0
+    assert O.image_stats(tie)[1:3] == (1, 2)                   # first in row-major order
+    assert O.image_stats(np.zeros((4, 4)))[3:] == (0.0, 0.0)  # sigma 0 -> snr 0
+    neg = -np.ones((4, 4))
+    neg[0, 1] = -0.5
+    assert O.image_stats(neg)[0] == -0.5                       # positive-going maximum only (A10)
+
+
+# ------------------------------------------------------------------ brute force
+def test_brute_force_tiny_problem():
+    """P13: 3 antennas, 4 channels, npix 8: every image by the DFT sum in pure Python."""
+    rng = np.random.default_rng(5)
+    nint, nbl, nchan, npol, npix = 12, 3, 4, 2, 8
+    uvw = rng.uniform(-60, 60, size=(nbl, 3))
+    f = np.array([1.0e9, 1.1e9, 1.2e9, 1.3e9])
+    tint = 0.01
+    cell = 1.0 / (2.5 * np.hypot(uvw[:, 0], uvw[:, 1]).max() * f.max() / O.C_LIGHT)
+    dms = [0.0, 30.0, 55.0]
+    dts = [1, 2]
+    w = np.array([1, 1, 0, 1], dtype=np.float32)
+    vis = (rng.standard_normal((nint, nbl, nchan, npol)) +
+           1j * rng.standard_normal((nint, nbl, nchan, npol))).astype(np.complex64)
+    cands, stats = O.search(vis, f, uvw, tint, npix, cell, dms, dts, 0.5, chan_weights=w,
+                            return_all_stats=True)
+    du = 1.0 / (npix * cell)
+    fmax = max(f) / 1e9
+    seen = 0
+    for d, dm in enumerate(dms):
+        delay = [math.floor(4.148808e-3 * dm * (1 / (fc / 1e9) ** 2 - 1 / fmax ** 2) / tint + 0.5)
+                 for fc in f]
+        for k, dt in enumerate(dts):
+            nj = (nint - max(delay)) // dt
+            for j in range(nj):
+                samples = []
+                for b in range(nbl):
+                    for c in range(nchan):
+                        if w[c] == 0:
+                            continue
+                        a = math.floor(uvw[b, 0] * f[c] / O.C_LIGHT / du + 0.5)
+                        e = math.floor(uvw[b, 1] * f[c] / O.C_LIGHT / du + 0.5)
+                        if not (-npix // 2 <= a < npix // 2 and -npix // 2 <= e < npix // 2):
+                            continue
+                        acc = 0j
+                        for q in range(dt):
+                            for p in range(npol):
+                                acc += complex(vis[j * dt + q + delay[c], b, c, p])
+                        samples.append((a, e, acc / (dt * npol)))
+                img = [[sum((sv * cmath.exp(2j * math.pi * (a * x + e * y) / npix)).real
+                            for a, e, sv in samples) / len(samples)
+                        for x in range(npix)] for y in range(npix)]
+                flat = [v for row in img for v in row]
+                peak = max(flat)
+                pos = flat.index(peak)
+                srt = sorted(flat)
+                med = 0.5 * (srt[31] + srt[32])
+                dev = sorted(abs(v - med) for v in flat)
+                sigma = 1.4826 * 0.5 * (dev[31] + dev[32])
+                got = stats[(d, k, j)]
+                assert abs(got[0] - peak) < 1e-12 and (got[1], got[2]) == divmod(pos, npix)
+                assert abs(got[3] - sigma) < 1e-12 and abs(got[4] - peak / sigma) < 1e-9
+                seen += 1
+    assert seen == len(stats) and seen >= 30
+    assert all(c.snr >= 0.5 for c in cands) and len(cands) == sum(v[4] >= 0.5 for v in stats.values())
