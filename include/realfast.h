@@ -1,0 +1,140 @@
+/* realfast.h -- C-ABI of the B200-native realfast search hot path.
+ *
+ * What the library computes (PAPER.md = Law et al., arXiv 1802.03084; readings
+ * A1-A20 are listed in DESIGN.md):
+ *
+ *   for every DM trial x sampling time dt x output integration j of one segment
+ *   of fast-sampled visibilities (the two dashed loops of Fig. 2):
+ *     (a) shift each channel by its integer dispersion delay,
+ *     (b) average dt integrations and the polarisations (Stokes I),
+ *     (c) grid all baselines x channels on the uv plane, nearest cell, with the
+ *         Hermitian conjugate,
+ *     (d) form the image with a 2-D inverse FFT,
+ *     (e) reduce it to peak, robust sigma and S/N and keep it if S/N >= threshold
+ *         (PAPER.md:86-88).
+ *
+ * All device work is hand-written CUDA for sm_100a; there is no CPU fallback.
+ * Every function returns RF_OK (0) or a negative error code, never throws, never
+ * exits, never prints.  Unless said otherwise pointers are HOST pointers.
+ */
+#ifndef REALFAST_B200_H
+#define REALFAST_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RF_OK          0
+#define RF_ERR_ARG    (-1)  /* null pointer, size out of range, non-finite value        */
+#define RF_ERR_CUDA   (-2)  /* a CUDA runtime call failed; see rf_last_error()           */
+#define RF_ERR_NOMEM  (-3)  /* host or device allocation failed                          */
+#define RF_ERR_STATE  (-4)  /* call not valid for this plan (e.g. index out of range)    */
+
+typedef struct rf_plan rf_plan;      /* opaque; owns all device tables and workspace */
+
+/* One candidate: the image of (dm_idx, dt_idx, t_idx) had peak/sigma >= threshold.
+ * t_idx is the index j in the dt-resampled series (native start = j * dt).
+ * l_pix/m_pix are the signed pixel offsets of the peak in [-npix/2, npix/2): image
+ * column x maps to l (via u), row y to m (via v); x >= npix/2 means x - npix (A12).  */
+typedef struct {
+    int32_t dm_idx, dt_idx, t_idx;
+    int32_t l_pix, m_pix;
+    float   peak, sigma, snr;
+} rf_cand;                            /* 32 bytes */
+
+/* Candidate sink, caller-owned DEVICE memory.  rf_search zeroes *count on the
+ * stream before searching; count keeps counting past capacity (overflow = count >
+ * capacity, extra candidates dropped).  Order of items is unspecified.          */
+typedef struct {
+    rf_cand* items;       /* device, capacity entries */
+    int32_t  capacity;
+    int32_t* count;       /* device, one int32 */
+} rf_cand_out;
+
+/* Counters of the last rf_search (read after synchronising its stream). */
+typedef struct {
+    int64_t images;           /* (dm, dt, j) images searched                              */
+    int64_t vis_gridded;      /* Stokes-I samples gridded = sum_images N_w * dt           */
+    int32_t n_kept;           /* N_w: (baseline, channel) samples kept by the cell table  */
+    int32_t n_dropped;        /* samples outside the grid or with zero channel weight      */
+    int32_t stats_overflow;   /* images whose median/MAD fell outside the histogram range */
+    int32_t kernel_launches;  /* kernels enqueued by the last rf_search                   */
+} rf_counters;
+
+/* Create a plan = the pipeline "state": everything that determines
+ * the result except the visibilities.  All arrays are copied.
+ *   freqs_hz [nchan]   channel centres, any order; delays are relative to max(freqs)
+ *   uvw_m    [nbl][3]  baseline (u,v,w) in metres, one per segment; w is ignored
+ *   npol               1, 2 or 4 polarisation products, averaged into Stokes I
+ *   nint               integrations per segment; inttime_s seconds each
+ *   npix               image side, power of two in 64..4096; cell_rad pixel size (rad)
+ *   dm_list  [ndm]     pc/cm^3, any order; dt_list [ndt] widths >= 1 in integrations
+ *   threshold_sigma    candidates have snr >= threshold (compared in float32)
+ * Tables (a) delay[dm][ch] = floor(K DM (f^-2 - fmax^-2)/t_int + 0.5), K = 4.148808e-3
+ * s GHz^2, and the uv cell table iu = floor(u f/c * npix*cell + 0.5) are computed on
+ * the device in float64 and are bit-exact against the same expressions in IEEE-754.
+ * Errors: RF_ERR_ARG on any invalid argument; RF_ERR_CUDA / RF_ERR_NOMEM.        */
+int rf_plan_create(rf_plan** out,
+                   const double* freqs_hz, int nchan,
+                   const double* uvw_m, int nbl,
+                   int npol, int nint, double inttime_s,
+                   int npix, double cell_rad,
+                   const double* dm_list, int ndm,
+                   const int32_t* dt_list, int ndt,
+                   float threshold_sigma);
+
+/* Enqueue the whole search of one segment on `cuda_stream` (a cudaStream_t, may be
+ * 0) and return without synchronising.
+ *   vis_dev  DEVICE pointer, complex64 [nint][nbl][nchan][npol] (re,im float32 pairs),
+ *            16-byte aligned, borrowed read-only until the stream passes this work.
+ * One rf_search in flight per plan (the workspace is per plan).                  */
+int rf_search(rf_plan* plan, const void* vis_dev, void* cuda_stream, rf_cand_out* cand_out);
+
+int rf_plan_destroy(rf_plan* plan);
+
+/* Channel weights (0 = flagged: neither read nor counted in N_w; anything else = 1);
+ * rebuilds the gridding tables (A17).  w [nchan] host floats.                     */
+int rf_plan_set_chan_weights(rf_plan* plan, const float* w);
+
+/* Replace the baseline uvw (and optionally the cell size: cell_rad <= 0 keeps it);
+ * rebuilds the cell and gridding tables (hour angle changes between segments).    */
+int rf_plan_set_uvw(rf_plan* plan, const double* uvw_m, double cell_rad);
+
+/* Streaming (config 5): search only native integrations t < n_native_ints for every
+ * DM (still bounded by nint - maxdelay(dm)); 0 restores "all valid" (A16).        */
+int rf_plan_set_search_span(rf_plan* plan, int n_native_ints);
+
+/* Copy the integer tables to HOST arrays (either may be NULL):
+ *   delay_host [ndm][nchan]; cell_host [nbl][nchan][2] = (iu, iv) signed cells.
+ *   keep_host [nbl][nchan] = 1 if the sample is gridded.                          */
+int rf_plan_get_tables(rf_plan* plan, int32_t* delay_host, int32_t* cell_host, uint8_t* keep_host);
+
+/* Number of images the plan searches, per rf_search; per (dm, dt) count via
+ * rf_plan_num_t(plan, dm_idx, dt_idx).                                            */
+int64_t rf_plan_num_images(const rf_plan* plan);
+int     rf_plan_num_t(const rf_plan* plan, int dm_idx, int dt_idx);
+
+/* Pixel-parity hook: write the float32 image [npix][npix] (row y, column x, no
+ * fftshift) of one (dm_idx, dt_idx, t_idx) to DEVICE memory, and optionally its
+ * statistics (peak, sigma, snr as the search computes them) to a device rf_cand.
+ * Runs the same kernels as rf_search.  Enqueues on the stream, no sync.           */
+int rf_debug_image(rf_plan* plan, const void* vis_dev, int dm_idx, int dt_idx, int t_idx,
+                   float* image_dev, rf_cand* stats_dev, void* cuda_stream);
+
+/* Counters of the most recent rf_search on this plan; synchronises nothing: call
+ * after the caller has synchronised the stream.                                   */
+int rf_plan_get_counters(rf_plan* plan, rf_counters* out);
+
+/* Tuning knob (not part of the result): images per batch of the two-pass pipeline;
+ * 0 restores the default chosen from npix and the L2 size.                        */
+int rf_plan_set_batch(rf_plan* plan, int images_per_batch);
+
+/* Thread-local description of the last error returned on this thread. */
+const char* rf_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* REALFAST_B200_H */

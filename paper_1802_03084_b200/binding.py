@@ -1,0 +1,191 @@
+"""ctypes binding with the same names as include/realfast.h: argument marshalling only.
+
+Every step of the search runs in the CUDA kernels of librealfast_b200.so; torch is used
+here for device memory and streams.  If the library is missing, loading fails loudly --
+there is no fallback path.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB: Optional[C.CDLL] = None
+
+RF_OK = 0
+EXPORTS = [
+    "rf_plan_create", "rf_search", "rf_plan_destroy", "rf_plan_set_chan_weights", "rf_plan_set_uvw",
+    "rf_plan_set_search_span", "rf_plan_get_tables", "rf_plan_num_images", "rf_plan_num_t",
+    "rf_debug_image", "rf_plan_get_counters", "rf_plan_set_batch", "rf_last_error",
+]
+
+# numpy view of rf_cand (32 bytes)
+CAND_DTYPE = np.dtype([("dm_idx", "<i4"), ("dt_idx", "<i4"), ("t_idx", "<i4"), ("l_pix", "<i4"),
+                       ("m_pix", "<i4"), ("peak", "<f4"), ("sigma", "<f4"), ("snr", "<f4")])
+assert CAND_DTYPE.itemsize == 32
+
+
+class RealfastError(RuntimeError):
+    pass
+
+
+class _CandOut(C.Structure):
+    _fields_ = [("items", C.c_void_p), ("capacity", C.c_int32), ("count", C.c_void_p)]
+
+
+class _Counters(C.Structure):
+    _fields_ = [("images", C.c_int64), ("vis_gridded", C.c_int64), ("n_kept", C.c_int32),
+                ("n_dropped", C.c_int32), ("stats_overflow", C.c_int32), ("kernel_launches", C.c_int32)]
+
+
+def lib_path() -> str:
+    return os.path.join(_HERE, "librealfast_b200.so")
+
+
+def load_library() -> C.CDLL:
+    """dlopen the in-tree library and declare the prototypes; raises if it is not built."""
+    global _LIB
+    if _LIB is not None:
+        return _LIB
+    path = lib_path()
+    if not os.path.exists(path):
+        raise RealfastError(f"{path} is not built: run `python -m paper_1802_03084_b200.build` "
+                            "(or __graft_entry__.build()); there is no CPU fallback")
+    lib = C.CDLL(path)
+    dp, ip, vp = C.POINTER(C.c_double), C.POINTER(C.c_int32), C.c_void_p
+    lib.rf_plan_create.argtypes = [C.POINTER(vp), dp, C.c_int, dp, C.c_int, C.c_int, C.c_int, C.c_double,
+                                   C.c_int, C.c_double, dp, C.c_int, ip, C.c_int, C.c_float]
+    lib.rf_search.argtypes = [vp, vp, vp, C.POINTER(_CandOut)]
+    lib.rf_plan_destroy.argtypes = [vp]
+    lib.rf_plan_set_chan_weights.argtypes = [vp, C.POINTER(C.c_float)]
+    lib.rf_plan_set_uvw.argtypes = [vp, dp, C.c_double]
+    lib.rf_plan_set_search_span.argtypes = [vp, C.c_int]
+    lib.rf_plan_set_batch.argtypes = [vp, C.c_int]
+    lib.rf_plan_get_tables.argtypes = [vp, ip, ip, C.POINTER(C.c_uint8)]
+    lib.rf_plan_num_images.argtypes = [vp]
+    lib.rf_plan_num_images.restype = C.c_int64
+    lib.rf_plan_num_t.argtypes = [vp, C.c_int, C.c_int]
+    lib.rf_debug_image.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, vp, vp, vp]
+    lib.rf_plan_get_counters.argtypes = [vp, C.POINTER(_Counters)]
+    lib.rf_last_error.restype = C.c_char_p
+    for name in EXPORTS:
+        if name not in ("rf_plan_num_images", "rf_last_error"):
+            getattr(lib, name).restype = C.c_int
+    _LIB = lib
+    return lib
+
+
+def _check(rc: int) -> None:
+    if rc != RF_OK:
+        raise RealfastError(f"realfast error {rc}: {load_library().rf_last_error().decode()}")
+
+
+def _dptr(a: np.ndarray):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+class Plan:
+    """rf_plan wrapper.  Methods mirror the C entry points one to one."""
+
+    def __init__(self, freqs_hz, uvw_m, npol: int, nint: int, inttime_s: float, npix: int,
+                 cell_rad: float, dm_list, dt_list: Sequence[int], threshold: float):
+        self._lib = load_library()
+        self._h = C.c_void_p()
+        f = np.ascontiguousarray(freqs_hz, dtype=np.float64)
+        u = np.ascontiguousarray(uvw_m, dtype=np.float64)
+        d = np.ascontiguousarray(dm_list, dtype=np.float64)
+        t = np.ascontiguousarray(dt_list, dtype=np.int32)
+        if u.ndim != 2 or u.shape[1] != 3:
+            raise ValueError("uvw_m must be [nbl][3]")
+        self.nchan, self.nbl, self.npol, self.nint = f.size, u.shape[0], npol, nint
+        self.npix, self.ndm, self.ndt = npix, d.size, t.size
+        _check(self._lib.rf_plan_create(C.byref(self._h), _dptr(f), f.size, _dptr(u), u.shape[0], npol, nint,
+                                        inttime_s, npix, cell_rad, _dptr(d), d.size,
+                                        t.ctypes.data_as(C.POINTER(C.c_int32)), t.size, threshold))
+
+    # -- lifetime
+    def destroy(self) -> None:
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._lib.rf_plan_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    # -- rf_plan_set_*
+    def set_chan_weights(self, w) -> None:
+        w = np.ascontiguousarray(w, dtype=np.float32)
+        assert w.size == self.nchan
+        _check(self._lib.rf_plan_set_chan_weights(self._h, w.ctypes.data_as(C.POINTER(C.c_float))))
+
+    def set_uvw(self, uvw_m, cell_rad: float = 0.0) -> None:
+        u = np.ascontiguousarray(uvw_m, dtype=np.float64)
+        assert u.shape == (self.nbl, 3)
+        _check(self._lib.rf_plan_set_uvw(self._h, _dptr(u), cell_rad))
+
+    def set_search_span(self, n: int) -> None:
+        _check(self._lib.rf_plan_set_search_span(self._h, n))
+
+    def set_batch(self, n: int) -> None:
+        _check(self._lib.rf_plan_set_batch(self._h, n))
+
+    # -- queries
+    def get_tables(self):
+        delay = np.empty((self.ndm, self.nchan), dtype=np.int32)
+        cell = np.empty((self.nbl, self.nchan, 2), dtype=np.int32)
+        keep = np.empty((self.nbl, self.nchan), dtype=np.uint8)
+        _check(self._lib.rf_plan_get_tables(self._h, delay.ctypes.data_as(C.POINTER(C.c_int32)),
+                                            cell.ctypes.data_as(C.POINTER(C.c_int32)),
+                                            keep.ctypes.data_as(C.POINTER(C.c_uint8))))
+        return delay, cell, keep
+
+    def num_images(self) -> int:
+        return int(self._lib.rf_plan_num_images(self._h))
+
+    def num_t(self, dm_idx: int, dt_idx: int) -> int:
+        return int(self._lib.rf_plan_num_t(self._h, dm_idx, dt_idx))
+
+    def get_counters(self) -> dict:
+        c = _Counters()
+        _check(self._lib.rf_plan_get_counters(self._h, C.byref(c)))
+        return {k: getattr(c, k) for k, _ in _Counters._fields_}
+
+    # -- rf_search / rf_debug_image: device pointers and a stream, nothing else
+    def search_raw(self, vis_ptr: int, stream: int, items_ptr: int, capacity: int, count_ptr: int) -> None:
+        out = _CandOut(items_ptr, capacity, count_ptr)
+        _check(self._lib.rf_search(self._h, vis_ptr, stream, C.byref(out)))
+
+    def search(self, vis, capacity: int = 1 << 16, stream=None, sync: bool = True):
+        """vis: torch complex64 CUDA tensor [nint][nbl][nchan][npol].  Returns (cands, count) where
+        cands is a numpy structured array (CAND_DTYPE) of min(count, capacity) records."""
+        import torch
+        assert vis.is_cuda and vis.dtype == torch.complex64 and vis.is_contiguous()
+        assert tuple(vis.shape) == (self.nint, self.nbl, self.nchan, self.npol), tuple(vis.shape)
+        st = torch.cuda.current_stream(vis.device) if stream is None else stream
+        items = torch.empty(max(1, capacity) * 32, dtype=torch.uint8, device=vis.device)
+        count = torch.zeros(1, dtype=torch.int32, device=vis.device)
+        self.search_raw(vis.data_ptr(), st.cuda_stream, items.data_ptr(), capacity, count.data_ptr())
+        if not sync:
+            return items, count
+        st.synchronize()
+        n = int(count.item())
+        rec = items[: min(n, capacity) * 32].cpu().numpy().view(CAND_DTYPE).copy()
+        return rec, n
+
+    def debug_image(self, vis, dm_idx: int, dt_idx: int, t_idx: int, stream=None):
+        """Returns (image float32 [npix][npix] numpy, stats record) of one (dm, dt, t)."""
+        import torch
+        assert vis.is_cuda and vis.dtype == torch.complex64 and vis.is_contiguous()
+        st = torch.cuda.current_stream(vis.device) if stream is None else stream
+        img = torch.empty((self.npix, self.npix), dtype=torch.float32, device=vis.device)
+        stats = torch.zeros(32, dtype=torch.uint8, device=vis.device)
+        _check(self._lib.rf_debug_image(self._h, vis.data_ptr(), dm_idx, dt_idx, t_idx, img.data_ptr(),
+                                        stats.data_ptr(), st.cuda_stream))
+        st.synchronize()
+        return img.cpu().numpy(), stats.cpu().numpy().view(CAND_DTYPE)[0].copy()

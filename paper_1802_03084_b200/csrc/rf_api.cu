@@ -1,0 +1,166 @@
+// rf_api.cu -- the C-ABI of include/realfast.h: validation, plan lifetime, error strings.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "rf_internal.h"
+
+namespace rf {
+static thread_local char g_err[512] = "";
+void set_error(const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+}  // namespace rf
+
+using rf::set_error;
+
+namespace {
+
+bool finite_pos(double x) { return std::isfinite(x) && x > 0.0; }
+
+int rebuild_geometry(rf_plan* p) {
+    int rc;
+    if ((rc = rf::build_cell_table(p)) != RF_OK) return rc;
+    if ((rc = rf::build_grid_lists(p)) != RF_OK) return rc;
+    if ((rc = rf::build_image_list(p)) != RF_OK) return rc;   // vis_gridded depends on N_w
+    return RF_OK;
+}
+
+void free_tables(rf_plan* p) {
+    rf::DeviceTables& d = p->d;
+    cudaFree(d.delay); cudaFree(d.cell); cudaFree(d.keep); cudaFree(d.entries);
+    cudaFree(d.warp_chunk); cudaFree(d.images); cudaFree(d.freqs); cudaFree(d.uvw); cudaFree(d.dms);
+    d = rf::DeviceTables{};
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* rf_last_error(void) { return rf::g_err; }
+
+int rf_plan_create(rf_plan** out, const double* freqs_hz, int nchan, const double* uvw_m, int nbl,
+                   int npol, int nint, double inttime_s, int npix, double cell_rad,
+                   const double* dm_list, int ndm, const int32_t* dt_list, int ndt,
+                   float threshold_sigma) {
+    if (out) *out = nullptr;
+    if (!out || !freqs_hz || !uvw_m || !dm_list || !dt_list) { set_error("null pointer argument"); return RF_ERR_ARG; }
+    if (nchan <= 0 || nbl <= 0 || nint <= 0 || ndm <= 0 || ndt <= 0) { set_error("counts must be positive"); return RF_ERR_ARG; }
+    if (nchan > 4096) { set_error("nchan %d > 4096", nchan); return RF_ERR_ARG; }
+    if ((long long)nbl * nchan >= (1ll << 24)) { set_error("nbl*nchan must be < 2^24"); return RF_ERR_ARG; }
+    if (npol != 1 && npol != 2 && npol != 4) { set_error("npol must be 1, 2 or 4"); return RF_ERR_ARG; }
+    if (npix < 64 || npix > 4096 || (npix & (npix - 1))) { set_error("npix must be a power of two in 64..4096"); return RF_ERR_ARG; }
+    if (!finite_pos(inttime_s) || !finite_pos(cell_rad)) { set_error("inttime and cell must be finite and positive"); return RF_ERR_ARG; }
+    if (!std::isfinite(threshold_sigma)) { set_error("threshold must be finite"); return RF_ERR_ARG; }
+    for (int i = 0; i < nchan; i++) if (!finite_pos(freqs_hz[i])) { set_error("freqs_hz[%d] not finite/positive", i); return RF_ERR_ARG; }
+    for (int i = 0; i < 3 * nbl; i++) if (!std::isfinite(uvw_m[i])) { set_error("uvw_m[%d] not finite", i); return RF_ERR_ARG; }
+    for (int i = 0; i < ndm; i++) if (!std::isfinite(dm_list[i]) || dm_list[i] < 0) { set_error("dm_list[%d] must be finite and >= 0", i); return RF_ERR_ARG; }
+    for (int i = 0; i < ndt; i++) if (dt_list[i] <= 0) { set_error("dt_list[%d] must be >= 1", i); return RF_ERR_ARG; }
+
+    rf_plan* p = new (std::nothrow) rf_plan();
+    if (!p) { set_error("host allocation failed"); return RF_ERR_NOMEM; }
+    p->nchan = nchan; p->nbl = nbl; p->npol = npol; p->nint = nint; p->npix = npix;
+    p->ndm = ndm; p->ndt = ndt; p->inttime = inttime_s; p->cell = cell_rad; p->threshold = threshold_sigma;
+    p->freqs.assign(freqs_hz, freqs_hz + nchan);
+    p->uvw.assign(uvw_m, uvw_m + 3 * (size_t)nbl);
+    p->dms.assign(dm_list, dm_list + ndm);
+    p->dts.assign(dt_list, dt_list + ndt);
+    p->weights.assign(nchan, 1.0f);
+    p->nbins = 2048;
+    int rc = rf::build_delay_table(p);
+    if (rc == RF_OK) rc = rebuild_geometry(p);
+    if (rc != RF_OK) { rf_plan_destroy(p); return rc; }
+    *out = p;
+    return RF_OK;
+}
+
+int rf_plan_destroy(rf_plan* p) {
+    if (!p) return RF_OK;
+    rf::free_workspace(p);
+    free_tables(p);
+    delete p;
+    return RF_OK;
+}
+
+int rf_search(rf_plan* p, const void* vis_dev, void* cuda_stream, rf_cand_out* out) {
+    if (!p || !vis_dev || !out || !out->count || (out->capacity > 0 && !out->items) || out->capacity < 0) {
+        set_error("null pointer argument");
+        return RF_ERR_ARG;
+    }
+    if (reinterpret_cast<uintptr_t>(vis_dev) & 15) { set_error("vis_dev must be 16-byte aligned"); return RF_ERR_ARG; }
+    return rf::launch_search(p, vis_dev, static_cast<cudaStream_t>(cuda_stream), out);
+}
+
+int rf_plan_set_chan_weights(rf_plan* p, const float* w) {
+    if (!p || !w) { set_error("null pointer argument"); return RF_ERR_ARG; }
+    for (int i = 0; i < p->nchan; i++) p->weights[i] = (w[i] != 0.0f) ? 1.0f : 0.0f;
+    return rebuild_geometry(p);
+}
+
+int rf_plan_set_uvw(rf_plan* p, const double* uvw_m, double cell_rad) {
+    if (!p || !uvw_m) { set_error("null pointer argument"); return RF_ERR_ARG; }
+    for (int i = 0; i < 3 * p->nbl; i++) if (!std::isfinite(uvw_m[i])) { set_error("uvw_m[%d] not finite", i); return RF_ERR_ARG; }
+    if (cell_rad > 0) {
+        if (!std::isfinite(cell_rad)) { set_error("cell must be finite"); return RF_ERR_ARG; }
+        p->cell = cell_rad;
+    }
+    p->uvw.assign(uvw_m, uvw_m + 3 * (size_t)p->nbl);
+    return rebuild_geometry(p);
+}
+
+int rf_plan_set_search_span(rf_plan* p, int n) {
+    if (!p || n < 0) { set_error("invalid span"); return RF_ERR_ARG; }
+    p->span = n;
+    return rf::build_image_list(p);
+}
+
+int rf_plan_set_batch(rf_plan* p, int n) {
+    if (!p || n < 0) { set_error("invalid batch"); return RF_ERR_ARG; }
+    p->user_batch = n;
+    return RF_OK;
+}
+
+int rf_plan_get_tables(rf_plan* p, int32_t* delay_host, int32_t* cell_host, uint8_t* keep_host) {
+    if (!p) { set_error("null plan"); return RF_ERR_ARG; }
+    if (delay_host) memcpy(delay_host, p->h_delay.data(), p->h_delay.size() * sizeof(int32_t));
+    if (cell_host) memcpy(cell_host, p->h_cell.data(), p->h_cell.size() * sizeof(int32_t));
+    if (keep_host) memcpy(keep_host, p->h_keep.data(), p->h_keep.size());
+    return RF_OK;
+}
+
+int64_t rf_plan_num_images(const rf_plan* p) { return p ? p->n_images : 0; }
+
+int rf_plan_num_t(const rf_plan* p, int dm_idx, int dt_idx) {
+    if (!p || dm_idx < 0 || dm_idx >= p->ndm || dt_idx < 0 || dt_idx >= p->ndt) return RF_ERR_ARG;
+    return p->h_num_t[(size_t)dm_idx * p->ndt + dt_idx];
+}
+
+int rf_debug_image(rf_plan* p, const void* vis_dev, int dm_idx, int dt_idx, int t_idx,
+                   float* image_dev, rf_cand* stats_dev, void* cuda_stream) {
+    if (!p || !vis_dev) { set_error("null pointer argument"); return RF_ERR_ARG; }
+    if (dm_idx < 0 || dm_idx >= p->ndm || dt_idx < 0 || dt_idx >= p->ndt) { set_error("trial index out of range"); return RF_ERR_STATE; }
+    const int dt = p->dts[dt_idx];
+    if (t_idx < 0 || (long long)(t_idx + 1) * dt > p->nint - p->h_maxdelay[dm_idx]) { set_error("t_idx out of range"); return RF_ERR_STATE; }
+    return rf::launch_debug_image(p, vis_dev, dm_idx, dt_idx, t_idx, image_dev, stats_dev,
+                                  static_cast<cudaStream_t>(cuda_stream));
+}
+
+int rf_plan_get_counters(rf_plan* p, rf_counters* out) {
+    if (!p || !out) { set_error("null pointer argument"); return RF_ERR_ARG; }
+    int32_t c[4] = {0, 0, 0, 0};
+    if (p->ws.counters) RF_CUDA_CHECK(cudaMemcpy(c, p->ws.counters, sizeof(c), cudaMemcpyDeviceToHost));
+    out->images = p->n_images;
+    out->vis_gridded = p->vis_gridded;
+    out->n_kept = p->n_kept;
+    out->n_dropped = p->n_dropped;
+    out->stats_overflow = c[0];
+    out->kernel_launches = p->last_launches;
+    return RF_OK;
+}
+
+}  // extern "C"

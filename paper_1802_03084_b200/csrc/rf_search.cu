@@ -1,0 +1,195 @@
+// rf_search.cu -- workspace, kernel dispatch and the batch loop of rf_search.
+//
+// The search loop over (DM trial x sampling time x integration) (Fig. 2) is
+// flattened at plan time into a device-resident image list; rf_search walks it in batches
+// sized so that the half-plane hand-off H between the two FFT passes stays L2-resident.
+#include <algorithm>
+#include <cstdio>
+
+#include "rf_kernels.cuh"
+
+namespace rf {
+
+namespace {
+
+template <int N> size_t smem_pass1(int nchan, int ncolgrp) {
+    return (size_t)ncolgrp * (fft_padded_size(N) + 1) * sizeof(float2) +
+           FftCfg<N>::TW_TOTAL * sizeof(float2) + (size_t)nchan * sizeof(int) + 8 * sizeof(float);
+}
+template <int N> size_t smem_pass2(int nbins) {
+    return (size_t)(kThreads / FftCfg<N>::TPF) * fft_padded_size(N) * sizeof(float2) +
+           FftCfg<N>::TW_TOTAL * sizeof(float2) + (size_t)3 * nbins * sizeof(uint32_t) +
+           (16 + 16 + 8 + 4) * 4;
+}
+
+template <int N, int NPOL, int NCOL>
+int launch_pass1(const SearchParams& sp, int nchan, cudaStream_t st) {
+    auto kern = k_grid_colfft<N, NPOL, NCOL>;
+    const size_t smem = smem_pass1<N>(nchan, NCOL);
+    static size_t configured = 0;
+    if (smem > configured) {
+        RF_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured = smem;
+    }
+    kern<<<dim3(sp.n_img, sp.ngroups), kThreads, smem, st>>>(sp);
+    RF_CUDA_CHECK(cudaGetLastError());
+    return RF_OK;
+}
+
+template <int N, int NCOL>
+int launch_pass1_npol(const SearchParams& sp, int nchan, int npol, cudaStream_t st) {
+    switch (npol) {
+        case 1: return launch_pass1<N, 1, NCOL>(sp, nchan, st);
+        case 2: return launch_pass1<N, 2, NCOL>(sp, nchan, st);
+        case 4: return launch_pass1<N, 4, NCOL>(sp, nchan, st);
+    }
+    set_error("unsupported npol %d", npol);
+    return RF_ERR_ARG;
+}
+
+template <int N>
+int launch_pass2(const SearchParams& sp, cudaStream_t st) {
+    auto kern = k_rowfft_stats<N>;
+    const size_t smem = smem_pass2<N>(sp.nbins);
+    static size_t configured = 0;
+    if (smem > configured) {
+        RF_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured = smem;
+    }
+    kern<<<dim3(sp.rsplit, (sp.n_img + 1) / 2), kThreads, smem, st>>>(sp);
+    RF_CUDA_CHECK(cudaGetLastError());
+    return RF_OK;
+}
+
+int launch_batch(rf_plan* p, const SearchParams& sp, cudaStream_t st) {
+    int rc;
+    switch (p->npix) {
+#define RF_CASE(N, NCOL)                                                                    \
+    case N:                                                                                 \
+        if ((rc = launch_pass1_npol<N, NCOL>(sp, p->nchan, p->npol, st)) != RF_OK) return rc; \
+        return launch_pass2<N>(sp, st);
+        RF_CASE(64, 16)
+        RF_CASE(128, 16)
+        RF_CASE(256, 16)
+        RF_CASE(512, 16)
+        RF_CASE(1024, 8)
+        RF_CASE(2048, 4)
+        RF_CASE(4096, 4)
+#undef RF_CASE
+    }
+    set_error("unsupported npix %d", p->npix);
+    return RF_ERR_ARG;
+}
+
+SearchParams base_params(rf_plan* p, const void* vis) {
+    SearchParams sp{};
+    sp.vis = reinterpret_cast<const float*>(vis);
+    sp.delay = p->d.delay;
+    sp.entries = p->d.entries;
+    sp.warp_chunk = p->d.warp_chunk;
+    sp.H = p->ws.H;
+    sp.sumsq = p->ws.sumsq;
+    sp.hist = p->ws.hist;
+    sp.peak_val = p->ws.peak_val;
+    sp.peak_pos = p->ws.peak_pos;
+    sp.ticket = p->ws.ticket;
+    sp.counters = p->ws.counters;
+    sp.nchan = p->nchan;
+    sp.ncol = p->ncol;
+    sp.cpad = p->cpad;
+    sp.ngroups = p->ngroups;
+    sp.nbins = p->nbins;
+    sp.rsplit = p->ws.rsplit;
+    sp.row_floats = (long long)p->nbl * p->nchan * p->npol * 2;
+    sp.norm = p->n_kept > 0 ? (float)(1.0 / (2.0 * (double)p->n_kept * (double)p->npol)) : 0.f;
+    sp.threshold = p->threshold;
+    return sp;
+}
+
+}  // namespace
+
+void free_workspace(rf_plan* p) {
+    Workspace& w = p->ws;
+    cudaFree(w.H); cudaFree(w.sumsq); cudaFree(w.hist); cudaFree(w.peak_val); cudaFree(w.peak_pos);
+    cudaFree(w.ticket); cudaFree(w.counters); cudaFree(w.dbg_desc);
+    w = Workspace{};
+}
+
+// Batch = images whose half-plane hand-off fits a fixed L2 budget; row split chosen so that
+// pass 2 launches at least two CTAs per SM.
+int ensure_workspace(rf_plan* p) {
+    const size_t h_per_img = (size_t)p->npix * p->cpad;          // float2 elements
+    int batch = p->user_batch;
+    if (batch <= 0) {
+        const size_t budget = (size_t)64 << 20;                  // bytes of H kept in flight
+        batch = (int)std::min<size_t>(512, std::max<size_t>(2, budget / (h_per_img * sizeof(float2))));
+    }
+    batch = std::max(2, batch & ~1);
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const int max_split = std::max(1, (int)((long long)p->npix * p->npix / 4096));
+    int rsplit = 1;
+    while ((batch / 2) * rsplit < 2 * sms && rsplit * 2 <= max_split) rsplit *= 2;
+    Workspace& w = p->ws;
+    if (w.H && w.batch == batch && w.rsplit == rsplit && w.h_elems == h_per_img * batch) return RF_OK;
+    free_workspace(p);
+    w.batch = batch;
+    w.rsplit = rsplit;
+    w.h_elems = h_per_img * batch;
+    RF_CUDA_CHECK(cudaMalloc((void**)&w.H, w.h_elems * sizeof(float2)));
+    RF_CUDA_CHECK(cudaMalloc((void**)&w.sumsq, (size_t)batch * p->ngroups * sizeof(float)));
+    RF_CUDA_CHECK(cudaMalloc((void**)&w.hist, (size_t)batch * p->nbins * sizeof(uint32_t)));
+    RF_CUDA_CHECK(cudaMalloc((void**)&w.peak_val, (size_t)batch * rsplit * sizeof(float)));
+    RF_CUDA_CHECK(cudaMalloc((void**)&w.peak_pos, (size_t)batch * rsplit * sizeof(int32_t)));
+    RF_CUDA_CHECK(cudaMalloc((void**)&w.ticket, (size_t)(batch / 2) * sizeof(uint32_t)));
+    RF_CUDA_CHECK(cudaMalloc((void**)&w.counters, 4 * sizeof(int32_t)));
+    RF_CUDA_CHECK(cudaMalloc((void**)&w.dbg_desc, sizeof(ImgDesc)));
+    RF_CUDA_CHECK(cudaMemset(w.hist, 0, (size_t)batch * p->nbins * sizeof(uint32_t)));
+    RF_CUDA_CHECK(cudaMemset(w.ticket, 0, (size_t)(batch / 2) * sizeof(uint32_t)));
+    RF_CUDA_CHECK(cudaMemset(w.counters, 0, 4 * sizeof(int32_t)));
+    return RF_OK;
+}
+
+int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out) {
+    int rc = ensure_workspace(p);
+    if (rc != RF_OK) return rc;
+    RF_CUDA_CHECK(cudaMemsetAsync(out->count, 0, sizeof(int32_t), st));
+    RF_CUDA_CHECK(cudaMemsetAsync(p->ws.counters, 0, 4 * sizeof(int32_t), st));
+    SearchParams sp = base_params(p, vis);
+    sp.cand_items = out->items;
+    sp.cand_count = out->count;
+    sp.cand_capacity = out->capacity;
+    p->last_launches = 0;
+    if (p->n_kept == 0) return RF_OK;      // nothing gridded: every image is zero, snr := 0
+    for (int64_t base = 0; base < p->n_images; base += p->ws.batch) {
+        sp.images = p->d.images + base;
+        sp.n_img = (int)std::min<int64_t>(p->ws.batch, p->n_images - base);
+        if ((rc = launch_batch(p, sp, st)) != RF_OK) return rc;
+        p->last_launches += 2;
+    }
+    return RF_OK;
+}
+
+int launch_debug_image(rf_plan* p, const void* vis, int dm_idx, int dt_idx, int t_idx,
+                       float* image_dev, rf_cand* stats_dev, cudaStream_t st) {
+    int rc = ensure_workspace(p);
+    if (rc != RF_OK) return rc;
+    ImgDesc d{dm_idx, dt_idx, t_idx, p->dts[dt_idx]};
+    RF_CUDA_CHECK(cudaMemcpyAsync(p->ws.dbg_desc, &d, sizeof(d), cudaMemcpyHostToDevice, st));
+    RF_CUDA_CHECK(cudaStreamSynchronize(st));   // `d` lives on this stack frame (debug hook only)
+    SearchParams sp = base_params(p, vis);
+    sp.images = p->ws.dbg_desc;
+    sp.n_img = 1;
+    sp.image_out = image_dev;
+    sp.stats_out = stats_dev;
+    sp.cand_count = nullptr;
+    if (p->n_kept == 0) {
+        if (image_dev) RF_CUDA_CHECK(cudaMemsetAsync(image_dev, 0, (size_t)p->npix * p->npix * sizeof(float), st));
+        if (stats_dev) RF_CUDA_CHECK(cudaMemsetAsync(stats_dev, 0, sizeof(rf_cand), st));
+        return RF_OK;
+    }
+    return launch_batch(p, sp, st);
+}
+
+}  // namespace rf

@@ -1,0 +1,212 @@
+// rf_tables.cu -- plan-time tables: (a) dispersion-delay table, (c) uv-cell table and the
+// uv-column binning that lets gridding accumulate in shared memory without atomics.
+//
+// (a) PAPER.md:45 (footnote 1): tau = 4.15 ms DM / nu^2  -> reading A1-A4:
+//     delay[dm][ch] = floor(K*dm*(1/(f*f) - 1/(fmax*fmax))/t_int + 0.5), float64, no FMA.
+// (c) PAPER.md:72, 84: FFT imaging without a gridding kernel -> nearest cell (reading A8).
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+
+#include "rf_internal.h"
+
+namespace rf {
+
+namespace {
+
+constexpr double kDispersion = 4.148808e-3;   // s GHz^2 cm^3 / pc
+constexpr double kLight = 299792458.0;        // m / s
+
+// Every operation is an explicitly rounded IEEE float64 op (no contraction to FMA), in the
+// order the definition is written, so the table is bit-exact against any IEEE evaluation.
+__global__ void k_delay_table(const double* __restrict__ freqs_hz, const double* __restrict__ dms,
+                              int nchan, int ndm, double fmax_ghz, double inttime,
+                              int32_t* __restrict__ delay) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nchan * ndm) return;
+    int ch = i % nchan, d = i / nchan;
+    double f = __ddiv_rn(freqs_hz[ch], 1e9);
+    double a = __ddiv_rn(1.0, __dmul_rn(f, f));
+    double b = __ddiv_rn(1.0, __dmul_rn(fmax_ghz, fmax_ghz));
+    double x = __ddiv_rn(__dmul_rn(__dmul_rn(kDispersion, dms[d]), __dsub_rn(a, b)), inttime);
+    delay[i] = (int32_t)floor(__dadd_rn(x, 0.5));
+}
+
+__global__ void k_cell_table(const double* __restrict__ uvw, const double* __restrict__ freqs_hz,
+                             const float* __restrict__ weights, int nbl, int nchan, int npix,
+                             double du, int32_t* __restrict__ cell, uint8_t* __restrict__ keep) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nbl * nchan) return;
+    int ch = i % nchan, bl = i / nchan;
+    double f = freqs_hz[ch];
+    double ul = __ddiv_rn(__dmul_rn(uvw[3 * bl + 0], f), kLight);
+    double vl = __ddiv_rn(__dmul_rn(uvw[3 * bl + 1], f), kLight);
+    // clamp before the int conversion so absurd geometry cannot overflow int32
+    double a = fmin(fmax(floor(__dadd_rn(__ddiv_rn(ul, du), 0.5)), -1.0e9), 1.0e9);
+    double e = fmin(fmax(floor(__dadd_rn(__ddiv_rn(vl, du), 0.5)), -1.0e9), 1.0e9);
+    int iu = (int)a, iv = (int)e;
+    int half = npix / 2;
+    bool ok = iu >= -half && iu < half && iv >= -half && iv < half && weights[ch] != 0.0f;
+    cell[2 * i + 0] = iu;
+    cell[2 * i + 1] = iv;
+    keep[i] = ok ? 1 : 0;
+}
+
+template <class T> int upload(T** dst, const T* src, size_t n) {
+    if (*dst) { cudaFree(*dst); *dst = nullptr; }
+    if (n == 0) return RF_OK;
+    if (cudaMalloc((void**)dst, n * sizeof(T)) != cudaSuccess) {
+        cudaGetLastError();
+        set_error("device allocation of %zu bytes failed", n * sizeof(T));
+        return RF_ERR_NOMEM;
+    }
+    RF_CUDA_CHECK(cudaMemcpy(*dst, src, n * sizeof(T), cudaMemcpyHostToDevice));
+    return RF_OK;
+}
+
+}  // namespace
+
+int build_delay_table(rf_plan* p) {
+    int rc;
+    if ((rc = upload(&p->d.freqs, p->freqs.data(), p->freqs.size())) != RF_OK) return rc;
+    if ((rc = upload(&p->d.dms, p->dms.data(), p->dms.size())) != RF_OK) return rc;
+    size_t n = (size_t)p->ndm * p->nchan;
+    if (p->d.delay) { cudaFree(p->d.delay); p->d.delay = nullptr; }
+    RF_CUDA_CHECK(cudaMalloc((void**)&p->d.delay, n * sizeof(int32_t)));
+    double fmax = *std::max_element(p->freqs.begin(), p->freqs.end()) / 1e9;
+    k_delay_table<<<(unsigned)((n + 255) / 256), 256>>>(p->d.freqs, p->d.dms, p->nchan, p->ndm, fmax,
+                                                        p->inttime, p->d.delay);
+    RF_CUDA_CHECK(cudaGetLastError());
+    p->h_delay.resize(n);
+    RF_CUDA_CHECK(cudaMemcpy(p->h_delay.data(), p->d.delay, n * sizeof(int32_t), cudaMemcpyDeviceToHost));
+    p->h_maxdelay.assign(p->ndm, 0);
+    for (int d = 0; d < p->ndm; d++)
+        for (int c = 0; c < p->nchan; c++)
+            p->h_maxdelay[d] = std::max(p->h_maxdelay[d], p->h_delay[(size_t)d * p->nchan + c]);
+    return RF_OK;
+}
+
+int build_cell_table(rf_plan* p) {
+    int rc;
+    if ((rc = upload(&p->d.uvw, p->uvw.data(), p->uvw.size())) != RF_OK) return rc;
+    float* d_w = nullptr;
+    if ((rc = upload(&d_w, p->weights.data(), p->weights.size())) != RF_OK) return rc;
+    size_t n = (size_t)p->nbl * p->nchan;
+    if (p->d.cell) { cudaFree(p->d.cell); p->d.cell = nullptr; }
+    if (p->d.keep) { cudaFree(p->d.keep); p->d.keep = nullptr; }
+    RF_CUDA_CHECK(cudaMalloc((void**)&p->d.cell, 2 * n * sizeof(int32_t)));
+    RF_CUDA_CHECK(cudaMalloc((void**)&p->d.keep, n));
+    double du = 1.0 / (p->npix * p->cell);
+    k_cell_table<<<(unsigned)((n + 255) / 256), 256>>>(p->d.uvw, p->d.freqs, d_w, p->nbl, p->nchan,
+                                                       p->npix, du, p->d.cell, p->d.keep);
+    RF_CUDA_CHECK(cudaGetLastError());
+    p->h_cell.resize(2 * n);
+    p->h_keep.resize(n);
+    RF_CUDA_CHECK(cudaMemcpy(p->h_cell.data(), p->d.cell, 2 * n * sizeof(int32_t), cudaMemcpyDeviceToHost));
+    RF_CUDA_CHECK(cudaMemcpy(p->h_keep.data(), p->d.keep, n, cudaMemcpyDeviceToHost));
+    cudaFree(d_w);
+    p->n_kept = 0;
+    for (size_t i = 0; i < n; i++) p->n_kept += p->h_keep[i];
+    p->n_dropped = (int)n - p->n_kept;
+    return RF_OK;
+}
+
+// Route every kept sample to the half plane 0 <= column <= N/2 (the other half is its
+// Hermitian mirror and is never stored), sort by (column group, column, row, bl, ch), cut
+// each group into kWarpsPerCta ranges at cell boundaries and pad each range to whole
+// 32-lane chunks.  Inside a chunk equal cells are contiguous, so a segmented warp scan
+// followed by ONE plain read-modify-write per cell replaces shared-memory atomics, and the
+// summation order is fixed (bitwise reproducible grids).
+int build_grid_lists(rf_plan* p) {
+    const int N = p->npix, half = N / 2;
+    struct Raw { uint32_t col, row, elem, ch, conj; };
+    std::vector<Raw> raw;
+    raw.reserve((size_t)p->n_kept + 1024);
+    int maxcol = -1;
+    for (int bl = 0; bl < p->nbl; bl++)
+        for (int ch = 0; ch < p->nchan; ch++) {
+            size_t i = (size_t)bl * p->nchan + ch;
+            if (!p->h_keep[i]) continue;
+            int iu = p->h_cell[2 * i], iv = p->h_cell[2 * i + 1];
+            int c0 = ((iu % N) + N) % N, r0 = ((iv % N) + N) % N;
+            int c1 = ((-iu % N) + N) % N, r1 = ((-iv % N) + N) % N;
+            if (c0 <= half) { raw.push_back({(uint32_t)c0, (uint32_t)r0, (uint32_t)i, (uint32_t)ch, 0u}); maxcol = std::max(maxcol, c0); }
+            if (c1 <= half) { raw.push_back({(uint32_t)c1, (uint32_t)r1, (uint32_t)i, (uint32_t)ch, 1u}); maxcol = std::max(maxcol, c1); }
+        }
+    std::sort(raw.begin(), raw.end(), [](const Raw& a, const Raw& b) {
+        if (a.col != b.col) return a.col < b.col;
+        if (a.row != b.row) return a.row < b.row;
+        if (a.elem != b.elem) return a.elem < b.elem;
+        return a.conj < b.conj;
+    });
+    const int kColsPerGroup = p->colgrp = cols_per_group(N);
+    p->ncol = std::max(1, maxcol + 1);
+    p->cpad = (p->ncol + kColsPerGroup - 1) / kColsPerGroup * kColsPerGroup;
+    p->ngroups = p->cpad / kColsPerGroup;
+    p->n_entries = (int64_t)raw.size();
+
+    std::vector<GridEntry> entries;
+    std::vector<int32_t> warp_chunk(p->ngroups * kWarpsPerCta + 1, 0);
+    entries.reserve(raw.size() + (size_t)p->ngroups * kWarpsPerCta * 32);
+    size_t pos = 0;
+    for (int g = 0; g < p->ngroups; g++) {
+        size_t gbeg = pos;
+        while (pos < raw.size() && (int)(raw[pos].col / kColsPerGroup) == g) pos++;
+        size_t gend = pos, cnt = gend - gbeg;
+        size_t cut = gbeg;
+        for (int w = 0; w < kWarpsPerCta; w++) {
+            warp_chunk[g * kWarpsPerCta + w] = (int32_t)(entries.size() / 32);
+            // ideal end of this warp's range, moved forward to the next cell boundary
+            size_t want = gbeg + cnt * (w + 1) / kWarpsPerCta;
+            size_t end = std::max(want, cut);
+            if (w == kWarpsPerCta - 1) end = gend;
+            while (end < gend && end > gbeg && raw[end].col == raw[end - 1].col && raw[end].row == raw[end - 1].row) end++;
+            for (size_t s = cut; s < end; s += 32) {
+                size_t e = std::min(end, s + 32);
+                for (size_t k = s; k < s + 32; k++) {
+                    GridEntry ge{0u, 0u};
+                    if (k < e) {
+                        const Raw& r = raw[k];
+                        size_t h = k;   // first lane of this cell inside the chunk
+                        while (h > s && raw[h - 1].col == r.col && raw[h - 1].row == r.row) h--;
+                        bool tail = (k + 1 == e) || raw[k + 1].col != r.col || raw[k + 1].row != r.row;
+                        ge.w0 = r.elem | ((uint32_t)(k - h) << 24) | (tail ? (1u << 29) : 0u) |
+                                (r.conj << 30) | (1u << 31);
+                        ge.w1 = r.ch | (r.row << 12) | ((r.col % kColsPerGroup) << 24);
+                    }
+                    entries.push_back(ge);
+                }
+            }
+            cut = end;
+        }
+    }
+    warp_chunk[p->ngroups * kWarpsPerCta] = (int32_t)(entries.size() / 32);
+    p->n_chunks = (int64_t)entries.size() / 32;
+    int rc;
+    if ((rc = upload(&p->d.entries, entries.data(), entries.size())) != RF_OK) return rc;
+    if ((rc = upload(&p->d.warp_chunk, warp_chunk.data(), warp_chunk.size())) != RF_OK) return rc;
+    return RF_OK;
+}
+
+// Loop + segment semantics (readings A6, A16): all j with
+// (j+1)*dt <= min(nint - maxdelay(dm), span).
+int build_image_list(rf_plan* p) {
+    std::vector<ImgDesc> imgs;
+    p->h_num_t.assign((size_t)p->ndm * p->ndt, 0);
+    p->vis_gridded = 0;
+    for (int d = 0; d < p->ndm; d++) {
+        int nsearch = p->nint - p->h_maxdelay[d];
+        if (p->span > 0) nsearch = std::min(nsearch, p->span);
+        for (int k = 0; k < p->ndt; k++) {
+            int dt = p->dts[k];
+            int nj = nsearch > 0 ? nsearch / dt : 0;
+            p->h_num_t[(size_t)d * p->ndt + k] = nj;
+            for (int j = 0; j < nj; j++) imgs.push_back({d, k, j, dt});
+            p->vis_gridded += (int64_t)nj * dt * p->n_kept;
+        }
+    }
+    p->n_images = (int64_t)imgs.size();
+    return upload(&p->d.images, imgs.data(), imgs.size());
+}
+
+}  // namespace rf

@@ -1,0 +1,183 @@
+"""GPU parity: the CUDA path (through the C-ABI) against the float64 oracle on the same
+seeded inputs.  Bars (BASELINE.json:north_star): delay table, cell indices and candidate keys
+away from the threshold bit-exact; pixels within 1e-4 x image rms; S/N within 1e-3 relative."""
+import numpy as np
+import pytest
+
+import oracle as O
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+PIX_TOL = 1e-4      # x image rms
+SNR_TOL = 1e-3      # relative
+NEAR_THR = 2e-3     # reading A11: |snr - thr| <= 2e-3 thr may fall on either side
+
+
+def _torch():
+    import torch
+    assert torch.cuda.is_available()
+    return torch
+
+
+def _plan_for(cfg, uvw=None, cell=None, weights=None, **over):
+    import paper_1802_03084_b200 as R
+    f = W.channel_freqs_hz(cfg)
+    uvw = W.baseline_uvw_m(cfg) if uvw is None else uvw
+    cell = W.default_cell_rad(cfg, uvw) if cell is None else cell
+    plan = R.Plan(f, uvw, cfg.npol, over.get("nint", cfg.nint), cfg.inttime_s, over.get("npix", cfg.npix),
+                  cell, over.get("dms", W.dm_list(cfg)), over.get("dts", cfg.dt_list),
+                  over.get("threshold", cfg.threshold))
+    if weights is not None:
+        plan.set_chan_weights(weights)
+    return plan, f, uvw, cell
+
+
+def _check_tables(plan, cfg, f, uvw, cell, dms, weights=None, npix=None):
+    delay, cells, keep = plan.get_tables()
+    assert np.array_equal(delay, O.delay_table(f, dms, cfg.inttime_s))
+    iu, iv, k = O.cell_table(uvw, f, npix or cfg.npix, cell, weights)
+    assert np.array_equal(cells[..., 0], iu) and np.array_equal(cells[..., 1], iv)
+    assert np.array_equal(keep.astype(bool), k)
+
+
+def _compare_candidates(gpu, oracle_cands, stats, thr):
+    """Key sets equal away from the threshold; positions equal; S/N within tolerance."""
+    g = {(int(c["dm_idx"]), int(c["dt_idx"]), int(c["t_idx"])): c for c in gpu}
+    o = {c.key: c for c in oracle_cands}
+    for key in set(g) ^ set(o):
+        snr = stats[key][4] if stats is not None else (o[key].snr if key in o else float(g[key]["snr"]))
+        assert abs(snr - thr) <= NEAR_THR * thr, f"candidate {key} only on one side, oracle snr {snr}"
+    for key in set(g) & set(o):
+        assert abs(float(g[key]["snr"]) - o[key].snr) <= SNR_TOL * o[key].snr, key
+        assert abs(float(g[key]["peak"]) - o[key].peak) <= 1e-4 * abs(o[key].peak) + 1e-7, key
+        assert (int(g[key]["l_pix"]), int(g[key]["m_pix"])) == (o[key].l_pix, o[key].m_pix), key
+    return len(set(g) & set(o))
+
+
+@pytest.mark.parametrize("name", ["tiny", "lband", "sband", "hires"])
+def test_tables_bit_exact(name):
+    cfg = W.get_config(name)
+    w = W.chan_weights(cfg) if cfg.n_flagged else None
+    plan, f, uvw, cell = _plan_for(cfg, weights=w)
+    _check_tables(plan, cfg, f, uvw, cell, W.dm_list(cfg), w)
+    delays = O.delay_table(f, W.dm_list(cfg), cfg.inttime_s)
+    total = sum(O.n_images(cfg.nint, int(delays[d].max()), dt) for d in range(cfg.ndm) for dt in cfg.dt_list)
+    assert plan.num_images() == total
+    plan.destroy()
+
+
+def test_tiny_full_parity():
+    """Config 1 in full: every image's statistics and the candidate list."""
+    torch = _torch()
+    cfg = W.get_config("tiny")
+    plan, f, uvw, cell = _plan_for(cfg)
+    vis = W.make_segment(cfg)
+    dvis = torch.from_numpy(vis).cuda()
+    cands, stats = O.search(vis, f, uvw, cfg.inttime_s, cfg.npix, cell, W.dm_list(cfg), cfg.dt_list,
+                            cfg.threshold, return_all_stats=True)
+    gpu, n = plan.search(dvis)
+    assert n == len(gpu)
+    matched = _compare_candidates(gpu, cands, stats, cfg.threshold)
+    assert matched >= 20
+    assert plan.get_counters()["stats_overflow"] == 0
+    # pixel parity + per-image statistics on a spread of images, including the brightest
+    delays = O.delay_table(f, W.dm_list(cfg), cfg.inttime_s)
+    iu, iv, keep = O.cell_table(uvw, f, cfg.npix, cell)
+    keys = [(0, 0, 0), (2, 0, 21), (3, 0, 19), (7, 0, 32), (5, 0, 13), (1, 0, 59)]
+    for (d, k, j) in keys:
+        ref = O.search_image(vis, delays, iu, iv, keep, cfg.npix, d, cfg.dt_list[k], j)
+        img, st = plan.debug_image(dvis, d, k, j)
+        rms = np.sqrt((ref ** 2).mean())
+        assert np.abs(img - ref).max() <= PIX_TOL * rms, (d, k, j)
+        peak, y, x, sigma, snr = O.image_stats(ref)
+        assert abs(float(st["snr"]) - snr) <= SNR_TOL * snr
+        assert abs(float(st["sigma"]) - sigma) <= SNR_TOL * sigma
+        assert (int(st["l_pix"]) % cfg.npix, int(st["m_pix"]) % cfg.npix) == (x, y)
+    plan.destroy()
+
+
+def test_tiny_all_image_statistics():
+    """Every image of config 1: S/N of the search (threshold 0 -> every image is emitted)."""
+    torch = _torch()
+    cfg = W.get_config("tiny")
+    plan, f, uvw, cell = _plan_for(cfg, threshold=0.0)
+    vis = W.make_segment(cfg)
+    _, stats = O.search(vis, f, uvw, cfg.inttime_s, cfg.npix, cell, W.dm_list(cfg), cfg.dt_list, 0.0,
+                        return_all_stats=True)
+    gpu, n = plan.search(torch.from_numpy(vis).cuda(), capacity=1024)
+    assert n == len(stats) == plan.num_images()
+    worst = 0.0
+    for c in gpu:
+        ref = stats[(int(c["dm_idx"]), int(c["dt_idx"]), int(c["t_idx"]))]
+        worst = max(worst, abs(float(c["snr"]) - ref[4]) / ref[4])
+        assert (int(c["m_pix"]) % cfg.npix, int(c["l_pix"]) % cfg.npix) == (ref[1], ref[2])
+    assert worst <= SNR_TOL, worst
+    plan.destroy()
+
+
+def _sample_keys(cfg, delays, n, seed):
+    rng = np.random.default_rng(seed)
+    keys = set()
+    while len(keys) < n:
+        d = int(rng.integers(cfg.ndm))
+        k = int(rng.integers(len(cfg.dt_list)))
+        nj = O.n_images(cfg.nint, int(delays[d].max()), cfg.dt_list[k])
+        if nj > 0:
+            keys.add((d, k, int(rng.integers(nj))))
+    return sorted(keys)
+
+
+def _transient_keys(cfg, delays, dms, max_keys=12):
+    """Images at the trial nearest each injected transient (matched width, arrival time)."""
+    keys = []
+    for src in W.transients(cfg):
+        d = int(np.argmin(np.abs(dms - src.dm)))
+        k = int(np.argmin([abs(dt - src.width) for dt in cfg.dt_list]))
+        dt = cfg.dt_list[k]
+        j = src.t0 // dt
+        if j < O.n_images(cfg.nint, int(delays[d].max()), dt):
+            keys.append((d, k, j))
+    return keys[:max_keys]
+
+
+@pytest.mark.parametrize("name,nsample", [("lband", 10), ("sband", 3), ("hires", 1)])
+def test_full_size_sampled_parity(name, nsample):
+    """BASELINE.json configs 2-4 at full size, in the launch configuration bench.py times:
+    whole rf_search, then sampled images (random + at the injected transients) against the oracle."""
+    torch = _torch()
+    cfg = W.get_config(name)
+    w = W.chan_weights(cfg) if cfg.n_flagged else None
+    plan, f, uvw, cell = _plan_for(cfg, weights=w)
+    dms = W.dm_list(cfg)
+    vis = W.make_segment(cfg)
+    dvis = torch.from_numpy(vis).cuda()
+    gpu, n = plan.search(dvis)
+    ctr = plan.get_counters()
+    assert ctr["images"] == plan.num_images() and n == len(gpu)
+    assert ctr["stats_overflow"] == 0
+    g = {(int(c["dm_idx"]), int(c["dt_idx"]), int(c["t_idx"])): c for c in gpu}
+    assert len(g) == len(gpu)
+    delays = O.delay_table(f, dms, cfg.inttime_s)
+    iu, iv, keep = O.cell_table(uvw, f, cfg.npix, cell, w)
+    keys = _transient_keys(cfg, delays, dms, 3 if name != "lband" else 10) + _sample_keys(cfg, delays, nsample, 7)
+    n_w = int(keep.sum())
+    found = 0
+    for (d, k, j) in keys:
+        s = O.dedisperse_resample(vis, delays[d], cfg.dt_list[k], j)
+        ref = O.image_from_grid(O.grid_visibilities(s, iu, iv, keep, cfg.npix), n_w)
+        peak, y, x, sigma, snr = O.image_stats(ref)
+        img, st = plan.debug_image(dvis, d, k, j)
+        rms = np.sqrt((ref ** 2).mean())
+        assert np.abs(img - ref).max() <= PIX_TOL * rms, (d, k, j)
+        assert abs(float(st["snr"]) - snr) <= SNR_TOL * snr, (d, k, j)
+        in_list = (d, k, j) in g
+        if abs(snr - cfg.threshold) > NEAR_THR * cfg.threshold:
+            assert in_list == (snr >= cfg.threshold), (d, k, j, snr)
+        if in_list:
+            found += 1
+            c = g[(d, k, j)]
+            assert abs(float(c["snr"]) - snr) <= SNR_TOL * snr
+            assert (int(c["l_pix"]) % cfg.npix, int(c["m_pix"]) % cfg.npix) == (x, y)
+    assert found >= 1, "no injected transient was recovered"
+    plan.destroy()
