@@ -208,10 +208,65 @@ __device__ float robust_sigma_from_hist(const HistView& hv, float total, int lan
     return 1.4826f * mad;
 }
 
+
+// ------------------------------------------------------------------------------------------
+// Exact order statistics for images small enough to stay in shared memory (npix <= 128):
+// MSB-first radix select on order-preserving keys, 4 passes of 8 bits, whole CTA.
+__device__ __forceinline__ uint32_t float_key(float f) {
+    uint32_t u = __float_as_uint(f);
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float key_float(uint32_t k) {
+    return __uint_as_float((k & 0x80000000u) ? (k & 0x7fffffffu) : ~k);
+}
+// k-th smallest (0-based) of data[0..M); h256 = 258 words of shared scratch.  All threads call.
+__device__ float select_kth(const float* data, int M, int k, uint32_t* h256) {
+    uint32_t prefix = 0u, mask = 0u;
+    const int tid = threadIdx.x;
+    for (int shift = 24; shift >= 0; shift -= 8) {
+        __syncthreads();
+        h256[tid] = 0u;                               // blockDim.x == 256
+        __syncthreads();
+        for (int i = tid; i < M; i += kThreads) {
+            const uint32_t key = float_key(data[i]);
+            if ((key & mask) == prefix) atomicAdd(&h256[(key >> shift) & 255u], 1u);
+        }
+        __syncthreads();
+        if (tid == 0) {
+            int cum = 0, d = 0;
+            for (; d < 255; d++) {
+                const int c = (int)h256[d];
+                if (cum + c > k) break;
+                cum += c;
+            }
+            h256[256] = (uint32_t)d;
+            h256[257] = (uint32_t)(k - cum);
+        }
+        __syncthreads();
+        prefix |= h256[256] << shift;
+        k = (int)h256[257];
+        mask |= 255u << shift;
+    }
+    __syncthreads();
+    return key_float(prefix);
+}
+// 1.4826 * median(|x - median(x)|), numpy's even-count median (mean of the two middle values).
+// Overwrites data with the absolute deviations.  All threads call; all get the result.
+__device__ float exact_sigma(float* data, int M, uint32_t* h256) {
+    const float med = 0.5f * (select_kth(data, M, M / 2 - 1, h256) + select_kth(data, M, M / 2, h256));
+    for (int i = threadIdx.x; i < M; i += kThreads) data[i] = fabsf(data[i] - med);
+    __syncthreads();
+    const float mad = 0.5f * (select_kth(data, M, M / 2 - 1, h256) + select_kth(data, M, M / 2, h256));
+    return 1.4826f * mad;
+}
+
 // ------------------------------------------------------------------------------------------
 // Pass 2.  grid = (rsplit, npairs); block = 256.  Dynamic smem:
 //   xbuf [G2][fft_padded_size(N)] float2 | tw | hist [2][nbins] u32 | cum [nbins] u32 | scratch
-template <int N>
+//   | (EXACT only) simg [2][N*N] float
+// EXACT (npix <= 128, row split 1): the two images stay in shared memory and median / MAD are
+// exact order statistics; otherwise they come from a 2048-bin histogram over +-3.5 sigma_rms.
+template <int N, bool EXACT>
 __global__ void __launch_bounds__(kThreads) k_rowfft_stats(const SearchParams p) {
     using C = FftCfg<N>;
     constexpr int G2 = kThreads / C::TPF;
@@ -225,6 +280,7 @@ __global__ void __launch_bounds__(kThreads) k_rowfft_stats(const SearchParams p)
     int* s_pos = reinterpret_cast<int*>(s_val + 16);                  // [2][8]
     float* s_misc = reinterpret_cast<float*>(s_pos + 16);             // [8]
     int* s_flag = reinterpret_cast<int*>(s_misc + 8);                 // [4]
+    float* simg = reinterpret_cast<float*>(s_flag + 4);               // [2][N*N] (EXACT)
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int pair = blockIdx.y, rs = blockIdx.x;
@@ -290,18 +346,26 @@ __global__ void __launch_bounds__(kThreads) k_rowfft_stats(const SearchParams p)
 #pragma unroll
             for (int e = 15; e >= 0; e--) if (v[e].y == mb) pos_b = y * N + t + C::TPF * e;
         }
-        if (iw_a > 0.f) {
+        if (EXACT) {
 #pragma unroll
             for (int e = 0; e < 16; e++) {
-                int bin = __float2int_rd((v[e].x - lo_a) * iw_a);
-                atomicAdd(&hist[min(max(bin, 0), nbm1)], 1u);
+                simg[y * N + t + C::TPF * e] = v[e].x;
+                simg[N * N + y * N + t + C::TPF * e] = v[e].y;
             }
-        }
-        if (has_b && iw_b > 0.f) {
+        } else {
+            if (iw_a > 0.f) {
 #pragma unroll
-            for (int e = 0; e < 16; e++) {
-                int bin = __float2int_rd((v[e].y - lo_b) * iw_b);
-                atomicAdd(&hist[p.nbins + min(max(bin, 0), nbm1)], 1u);
+                for (int e = 0; e < 16; e++) {
+                    int bin = __float2int_rd((v[e].x - lo_a) * iw_a);
+                    atomicAdd(&hist[min(max(bin, 0), nbm1)], 1u);
+                }
+            }
+            if (has_b && iw_b > 0.f) {
+#pragma unroll
+                for (int e = 0; e < 16; e++) {
+                    int bin = __float2int_rd((v[e].y - lo_b) * iw_b);
+                    atomicAdd(&hist[p.nbins + min(max(bin, 0), nbm1)], 1u);
+                }
             }
         }
         if (p.image_out != nullptr && pair == 0) {
@@ -335,7 +399,7 @@ __global__ void __launch_bounds__(kThreads) k_rowfft_stats(const SearchParams p)
     __syncthreads();
 
     // ---- merge across the row split; the last CTA of the pair finalises
-    if (p.rsplit > 1) {
+    if (!EXACT && p.rsplit > 1) {
         for (int i = tid; i < 2 * p.nbins; i += kThreads) {
             const uint32_t c = hist[i];
             if (c) atomicAdd(&p.hist[(size_t)slot_a * p.nbins + i], c);   // slots a, b are adjacent
@@ -372,28 +436,35 @@ __global__ void __launch_bounds__(kThreads) k_rowfft_stats(const SearchParams p)
     // ---- median / MAD / S/N / threshold, one image at a time
     for (int which = 0; which < (has_b ? 2 : 1); which++) {
         const uint32_t* h = hist + which * p.nbins;
-        // exclusive prefix sum of nbins counters: per-thread chunk + warp scan + warp totals
-        const int per = p.nbins / kThreads;             // nbins is a multiple of 256
-        uint32_t local = 0;
-        for (int i = 0; i < per; i++) local += h[tid * per + i];
-        uint32_t inc = local;
+        float sigma_exact = 0.f;
+        if (EXACT) {
+            sigma_exact = exact_sigma(simg + which * N * N, N * N, cum);
+        } else {
+            // exclusive prefix sum of nbins counters: per-thread chunk + warp scan + warp totals
+            const int per = p.nbins / kThreads;             // nbins is a multiple of 256
+            uint32_t local = 0;
+            for (int i = 0; i < per; i++) local += h[tid * per + i];
+            uint32_t inc = local;
 #pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            uint32_t o = __shfl_up_sync(0xffffffffu, inc, d);
-            if (lane >= d) inc += o;
+            for (int d = 1; d < 32; d <<= 1) {
+                uint32_t o = __shfl_up_sync(0xffffffffu, inc, d);
+                if (lane >= d) inc += o;
+            }
+            __shared__ uint32_t wtot[kWarpsPerCta];
+            if (lane == 31) wtot[warp] = inc;
+            __syncthreads();
+            uint32_t base = inc - local;
+            for (int w = 0; w < warp; w++) base += wtot[w];
+            for (int i = 0; i < per; i++) { cum[tid * per + i] = base; base += h[tid * per + i]; }
+            __syncthreads();
         }
-        __shared__ uint32_t wtot[kWarpsPerCta];
-        if (lane == 31) wtot[warp] = inc;
-        __syncthreads();
-        uint32_t base = inc - local;
-        for (int w = 0; w < warp; w++) base += wtot[w];
-        for (int i = 0; i < per; i++) { cum[tid * per + i] = base; base += h[tid * per + i]; }
-        __syncthreads();
         if (warp == 0) {
             const float sig_rms = which ? sig_b : sig_a;
             int overflow = 0;
             float sigma = 0.f;
-            if (sig_rms > 0.f) {
+            if (EXACT) {
+                sigma = sigma_exact;
+            } else if (sig_rms > 0.f) {
                 HistView hv{h, cum, p.nbins, -kHistRange * sig_rms, (float)p.nbins / (2.f * kHistRange * sig_rms)};
                 sigma = robust_sigma_from_hist(hv, (float)N * (float)N, lane, &overflow);
             }

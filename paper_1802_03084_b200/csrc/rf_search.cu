@@ -16,10 +16,11 @@ template <int N> size_t smem_pass1(int nchan, int ncolgrp) {
     return (size_t)ncolgrp * (fft_padded_size(N) + 1) * sizeof(float2) +
            FftCfg<N>::TW_TOTAL * sizeof(float2) + (size_t)nchan * sizeof(int) + 8 * sizeof(float);
 }
+template <int N> constexpr bool exact_stats() { return N <= 128; }
 template <int N> size_t smem_pass2(int nbins) {
     return (size_t)(kThreads / FftCfg<N>::TPF) * fft_padded_size(N) * sizeof(float2) +
            FftCfg<N>::TW_TOTAL * sizeof(float2) + (size_t)3 * nbins * sizeof(uint32_t) +
-           (16 + 16 + 8 + 4) * 4;
+           (16 + 16 + 8 + 4) * 4 + (exact_stats<N>() ? (size_t)2 * N * N * sizeof(float) : 0);
 }
 
 template <int N, int NPOL, int NCOL>
@@ -49,7 +50,7 @@ int launch_pass1_npol(const SearchParams& sp, int nchan, int npol, cudaStream_t 
 
 template <int N>
 int launch_pass2(const SearchParams& sp, cudaStream_t st) {
-    auto kern = k_rowfft_stats<N>;
+    auto kern = k_rowfft_stats<N, exact_stats<N>()>;
     const size_t smem = smem_pass2<N>(sp.nbins);
     static size_t configured = 0;
     if (smem > configured) {
@@ -131,6 +132,8 @@ int ensure_workspace(rf_plan* p) {
     const int max_split = std::max(1, (int)((long long)p->npix * p->npix / 4096));
     int rsplit = 1;
     while ((batch / 2) * rsplit < 2 * sms && rsplit * 2 <= max_split) rsplit *= 2;
+    if (p->npix <= 128) rsplit = 1;                              // exact statistics keep whole images per CTA
+    p->nbins = p->npix <= 256 ? 4096 : 2048;
     Workspace& w = p->ws;
     if (w.H && w.batch == batch && w.rsplit == rsplit && w.h_elems == h_per_img * batch) return RF_OK;
     free_workspace(p);
