@@ -1,0 +1,309 @@
+#!/usr/bin/env python
+"""bench.py -- the realfast search hot path on B200: dedispersed images/s.
+
+A "step" is one pass of the whole hot path (rf_search: dedisperse -> resample -> grid ->
+2-D FFT image -> peak/sigma -> threshold over every DM trial x width x integration) over one
+segment of synthetic VLA L-band visibilities (BASELINE.json:configs[1]).  Prints ONE JSON line.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config lband] [--impl ours|reference]
+
+N > 1 (torchrun, one rank per GPU): the path shards by independent segments (PAPER.md:108,
+"each segment is independent"), so every rank searches its own segment with no data-path
+collective ("scaling": "weak").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import workloads as W  # noqa: E402
+
+METRIC = "dedispersed images/s (grid+2D FFT+S/N)"
+UNIT = "images/s"
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, device copy)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region."""
+
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.rows, self._stop, self.gpu = [], threading.Event(), gpu_index
+        self._t = threading.Thread(target=self._run, daemon=True)
+
+    def _run(self):
+        try:
+            p = subprocess.Popen(["nvidia-smi", f"--id={self.gpu}", f"--query-gpu={self.Q}",
+                                  "--format=csv,noheader,nounits", "-lms", "100"],
+                                 stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            return
+        while not self._stop.is_set():
+            line = p.stdout.readline()
+            if not line:
+                break
+            self.rows.append([c.strip() for c in line.split(",")])
+        p.terminate()
+
+    def start(self):
+        self._t.start()
+
+    def stop(self):
+        self._stop.set()
+        self._t.join(timeout=2)
+        sm = [int(r[0]) for r in self.rows if r and r[0].isdigit()]
+        mx = [int(r[1]) for r in self.rows if len(r) > 1 and r[1].isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({n for r in self.rows if len(r) >= 6 for n, v in zip(names, r[2:6]) if v == "Active"})
+        return {"sm_mhz": int(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def _setup(cfg, segment=0):
+    f, uvw, dms = W.channel_freqs_hz(cfg), W.baseline_uvw_m(cfg), W.dm_list(cfg)
+    return f, uvw, dms, W.default_cell_rad(cfg, uvw)
+
+
+def _alg_bytes(cfg, plan):
+    """A_img = 16 N_bl N_chan,w dt + 16 N_pix^2 per image; split per kernel as
+    pass 1 = the visibility read + the hand-off write (8 N^2), pass 2 = the hand-off read (8 N^2)."""
+    c = plan.get_counters()
+    images = c["images"]
+    vis_bytes = 16.0 * c["vis_gridded"]                     # 16 B per (bl, ch) pol pair per native sample
+    hand = 8.0 * cfg.npix * cfg.npix * images
+    return {"total": vis_bytes + 2 * hand, "pass1": vis_bytes + hand, "pass2": hand, "images": images,
+            "vis_gridded": c["vis_gridded"]}
+
+
+def _oracle_worker(args):
+    (name, keys) = args
+    import oracle as O
+    cfg = W.get_config(name)
+    f, uvw, dms, cell = _setup(cfg)
+    vis = _oracle_worker.vis
+    delays = O.delay_table(f, dms, cfg.inttime_s)
+    wts = W.chan_weights(cfg) if cfg.n_flagged else None
+    iu, iv, keep = O.cell_table(uvw, f, cfg.npix, cell, wts)
+    n_w = int(keep.sum())
+    out = 0
+    for (d, k, j) in keys:
+        s = O.dedisperse_resample(vis, delays[d], cfg.dt_list[k], j)
+        img = O.image_from_grid(O.grid_visibilities(s, iu, iv, keep, cfg.npix), n_w)
+        out += O.image_stats(img)[4] >= cfg.threshold
+    return out
+
+
+def oracle_throughput(cfg, vis, n_images_sample: int, seed: int = 11):
+    """Time the float64 oracle as it stands on the host cores on a bounded uniform sample of the
+    (dm, dt, j) images of the same segment.  Returns (images/s, cores, sample description)."""
+    import multiprocessing as mp
+
+    import oracle as O
+    f, uvw, dms, cell = _setup(cfg)
+    delays = O.delay_table(f, dms, cfg.inttime_s)
+    rng = np.random.default_rng(seed)
+    keys = []
+    while len(keys) < n_images_sample:
+        d, k = int(rng.integers(cfg.ndm)), int(rng.integers(len(cfg.dt_list)))
+        nj = O.n_images(cfg.nint, int(delays[d].max()), cfg.dt_list[k])
+        if nj:
+            keys.append((d, k, int(rng.integers(nj))))
+    cores = max(1, min(len(os.sched_getaffinity(0)), 32, n_images_sample // 4))
+    os.environ.setdefault("OMP_NUM_THREADS", "1")
+    _oracle_worker.vis = vis                     # inherited by fork, not pickled
+    chunks = [keys[i::cores] for i in range(cores)]
+    t0 = time.perf_counter()
+    if cores == 1:
+        _oracle_worker((cfg.name, chunks[0]))
+    else:
+        with mp.get_context("fork").Pool(cores) as pool:
+            pool.map(_oracle_worker, [(cfg.name, c) for c in chunks])
+    dt = time.perf_counter() - t0
+    return n_images_sample / dt, cores, (f"{n_images_sample} images drawn uniformly over (dm, dt, j) of the same "
+                                         f"segment, float64 numpy oracle, {cores} processes")
+
+
+def run_reference(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    vis = W.make_segment(cfg)
+    vals = []
+    cores, sample = 1, ""
+    per_step = max(16, args.ref_images)
+    for i in range(args.warmup + args.steps):
+        v, cores, sample = oracle_throughput(cfg, vis, per_step, seed=100 + i)
+        if i >= args.warmup:
+            vals.append(v)
+    value = float(np.mean(vals))
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * per_step / value,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{cfg.name}: BASELINE.json configs[{cfg.index}], oracle on a bounded sample "
+                                   f"of {per_step} images per step"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args, cfg):
+    import torch
+    import torch.distributed as dist
+
+    import paper_1802_03084_b200 as R
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+
+    f, uvw, dms, cell = _setup(cfg)
+    vis = W.make_segment(cfg)                              # every rank: its own replica of the segment shape
+    hvis = torch.from_numpy(vis).pin_memory()
+    dvis = hvis.to(dev, non_blocking=True)
+    plan = R.Plan(f, uvw, cfg.npol, cfg.nint, cfg.inttime_s, cfg.npix, cell, dms, cfg.dt_list, cfg.threshold)
+    if cfg.n_flagged:
+        plan.set_chan_weights(W.chan_weights(cfg))
+    if args.batch:
+        plan.set_batch(args.batch)
+    capacity = 1 << 17
+    stream = torch.cuda.current_stream(dev)
+    items = torch.empty(capacity * 32, dtype=torch.uint8, device=dev)
+    count = torch.zeros(1, dtype=torch.int32, device=dev)
+
+    def step():
+        plan.search_raw(dvis.data_ptr(), stream.cuda_stream, items.data_ptr(), capacity, count.data_ptr())
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+
+    # ---- device-resident timing (value); per-kernel events on for the roofline object
+    plan.set_profiling(True)
+    sampler = ClockSampler(local)
+    sampler.start()
+    k_ms = [0.0, 0.0]
+    k_n = [0, 0]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    barrier()
+    total_ms = e0.elapsed_time(e1)
+    ms, n = plan.get_kernel_times()                        # last step's kernels (all steps are identical)
+    k_ms, k_n = ms, n
+    clocks = sampler.stop()
+    plan.set_profiling(False)
+    launches = plan.get_counters()["kernel_launches"]
+    n_cands = int(count.item())
+
+    # ---- end to end through the C-ABI with HOST buffers (pinned input, host candidate array)
+    cand_host = np.empty(capacity, dtype=R.CAND_DTYPE)
+    plan.search_host(hvis, cand_host, capacity)            # warm: allocates the staging buffers
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        _, n_e2e = plan.search_host(hvis, cand_host, capacity)
+    torch.cuda.synchronize(dev)
+    e2e_ms = (time.perf_counter() - t0) * 1e3
+
+    t_all = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t_all, op=dist.ReduceOp.MAX)
+    total_ms, e2e_ms = float(t_all[0]), float(t_all[1])
+
+    alg = _alg_bytes(cfg, plan)
+    images = alg["images"]
+    ms_per_step = total_ms / args.steps
+    value = world * images / (ms_per_step * 1e-3)
+    e2e_value = world * images / (e2e_ms / args.steps * 1e-3)
+
+    if rank == 0:
+        peak, peak_src = _peaks()
+        dom = 0 if k_ms[0] >= k_ms[1] else 1
+        dom_name = ["k_grid_colfft (dedisperse+grid+column FFT)", "k_rowfft_stats (row FFT+statistics)"][dom]
+        per_launch_ms = k_ms[dom] / max(1, k_n[dom])
+        per_launch_bytes = alg["pass1" if dom == 0 else "pass2"] / max(1, k_n[dom])
+        achieved = per_launch_bytes / (per_launch_ms * 1e-3) / 1e9
+        path_gbs = alg["total"] / (ms_per_step * 1e-3) / 1e9
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"{cfg.name}: BASELINE.json configs[{cfg.index}] ({cfg.nant} antennas, "
+                                   f"{cfg.nchan} ch, {cfg.nint} x {cfg.inttime_s * 1e3:g} ms, {cfg.ndm} DM x dt "
+                                   f"{list(cfg.dt_list)}, npix {cfg.npix})",
+                       "images_per_step": images, "gvis_per_s": world * alg["vis_gridded"] / (ms_per_step * 1e-3) / 1e9,
+                       "l2_policy": f"input segment {vis.nbytes / 1e9:.2f} GB is larger than L2 (126 MB); no flush",
+                       "candidates": n_cands, "parallelism": f"replicas x{world}" if world > 1 else "single GPU"},
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(vis.nbytes),
+                    "d2h_bytes_per_step": int(4 + min(n_e2e, capacity) * 32)},
+            "gpu_launches": int(launches) * args.steps,
+            "roofline": {"bound": "hbm", "kernel": dom_name, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                         "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                         "kernel_ms_per_step": {"pass1": k_ms[0], "pass2": k_ms[1]},
+                         "path": {"alg_bytes_per_step": alg["total"], "achieved": path_gbs, "frac": path_gbs / peak}},
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            v, cores, sample = oracle_throughput(cfg, vis, args.ref_images)
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+    plan.destroy()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="lband", choices=sorted(W.CONFIGS))
+    ap.add_argument("--batch", type=int, default=0, help="images per batch (0 = library default)")
+    ap.add_argument("--ref-images", type=int, default=512, help="oracle sample size per timing")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    cfg = W.get_config(args.config)
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        run_ours(args, cfg)
+
+
+if __name__ == "__main__":
+    main()

@@ -119,7 +119,7 @@ int     rf_plan_num_t(const rf_plan* plan, int dm_idx, int dt_idx);
 /* Pixel-parity hook: write the float32 image [npix][npix] (row y, column x, no
  * fftshift) of one (dm_idx, dt_idx, t_idx) to DEVICE memory, and optionally its
  * statistics (peak, sigma, snr as the search computes them) to a device rf_cand.
- * Runs the same kernels as rf_search.  Enqueues on the stream, no sync.           */
+ * Runs the same kernels as rf_search.  Debug hook: may synchronise the stream.     */
 int rf_debug_image(rf_plan* plan, const void* vis_dev, int dm_idx, int dt_idx, int t_idx,
                    float* image_dev, rf_cand* stats_dev, void* cuda_stream);
 
@@ -130,6 +130,21 @@ int rf_plan_get_counters(rf_plan* plan, rf_counters* out);
 /* Tuning knob (not part of the result): images per batch of the two-pass pipeline;
  * 0 restores the default chosen from npix and the L2 size.                        */
 int rf_plan_set_batch(rf_plan* plan, int images_per_batch);
+
+/* End-to-end convenience entry with HOST buffers: copies the segment host->device into a
+ * plan-owned staging buffer, runs rf_search on the plan's own stream, copies the candidates
+ * back and SYNCHRONISES.  vis_host: complex64 [nint][nbl][nchan][npol] (pinned memory makes
+ * the copy asynchronous and fast; pageable works).  cand_host: capacity records; *count_host
+ * receives the number found (may exceed capacity = overflow).                     */
+int rf_search_host(rf_plan* plan, const void* vis_host, rf_cand* cand_host, int32_t capacity,
+                   int32_t* count_host);
+
+/* Per-kernel timing for roofline accounting: when enabled, rf_search brackets every kernel
+ * launch with CUDA events on its stream.  After the caller has synchronised, get_kernel_times
+ * returns, for the last rf_search, the summed durations (ms) and launch counts of the two
+ * kernels: index 0 = grid + column FFT (pass 1), 1 = row FFT + statistics (pass 2).   */
+int rf_plan_set_profiling(rf_plan* plan, int enable);
+int rf_plan_get_kernel_times(rf_plan* plan, float ms[2], int32_t launches[2]);
 
 /* Thread-local description of the last error returned on this thread. */
 const char* rf_last_error(void);

@@ -20,6 +20,7 @@ EXPORTS = [
     "rf_plan_create", "rf_search", "rf_plan_destroy", "rf_plan_set_chan_weights", "rf_plan_set_uvw",
     "rf_plan_set_search_span", "rf_plan_get_tables", "rf_plan_num_images", "rf_plan_num_t",
     "rf_debug_image", "rf_plan_get_counters", "rf_plan_set_batch", "rf_last_error",
+    "rf_search_host", "rf_plan_set_profiling", "rf_plan_get_kernel_times",
 ]
 
 # numpy view of rf_cand (32 bytes)
@@ -71,6 +72,9 @@ def load_library() -> C.CDLL:
     lib.rf_debug_image.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, vp, vp, vp]
     lib.rf_plan_get_counters.argtypes = [vp, C.POINTER(_Counters)]
     lib.rf_last_error.restype = C.c_char_p
+    lib.rf_search_host.argtypes = [vp, vp, vp, C.c_int32, ip]
+    lib.rf_plan_set_profiling.argtypes = [vp, C.c_int]
+    lib.rf_plan_get_kernel_times.argtypes = [vp, C.POINTER(C.c_float), ip]
     for name in EXPORTS:
         if name not in ("rf_plan_num_images", "rf_last_error"):
             getattr(lib, name).restype = C.c_int
@@ -177,6 +181,31 @@ class Plan:
         n = int(count.item())
         rec = items[: min(n, capacity) * 32].cpu().numpy().view(CAND_DTYPE).copy()
         return rec, n
+
+    def search_host(self, vis_host, cand_host=None, capacity: int = 1 << 16):
+        """rf_search_host: vis_host is a host array/tensor (numpy complex64 or pinned torch tensor);
+        the host->device copy, the search and the candidate read-back all happen inside the call."""
+        if hasattr(vis_host, "data_ptr"):
+            ptr, nbytes = vis_host.data_ptr(), vis_host.numel() * vis_host.element_size()
+        else:
+            assert vis_host.flags["C_CONTIGUOUS"] and vis_host.dtype == np.complex64
+            ptr, nbytes = vis_host.ctypes.data, vis_host.nbytes
+        assert nbytes == self.nint * self.nbl * self.nchan * self.npol * 8
+        if cand_host is None:
+            cand_host = np.empty(capacity, dtype=CAND_DTYPE)
+        count = C.c_int32(0)
+        _check(self._lib.rf_search_host(self._h, ptr, cand_host.ctypes.data, capacity, C.byref(count)))
+        return cand_host[: min(count.value, capacity)], count.value
+
+    def set_profiling(self, enable: bool) -> None:
+        _check(self._lib.rf_plan_set_profiling(self._h, int(enable)))
+
+    def get_kernel_times(self):
+        """(ms[2], launches[2]) of the last search: 0 = grid+column FFT, 1 = row FFT+statistics."""
+        ms = (C.c_float * 2)()
+        n = (C.c_int32 * 2)()
+        _check(self._lib.rf_plan_get_kernel_times(self._h, ms, n))
+        return [float(ms[0]), float(ms[1])], [int(n[0]), int(n[1])]
 
     def debug_image(self, vis, dm_idx: int, dt_idx: int, t_idx: int, stream=None):
         """Returns (image float32 [npix][npix] numpy, stats record) of one (dm, dt, t)."""

@@ -34,7 +34,7 @@ int rebuild_geometry(rf_plan* p) {
 void free_tables(rf_plan* p) {
     rf::DeviceTables& d = p->d;
     cudaFree(d.delay); cudaFree(d.cell); cudaFree(d.keep); cudaFree(d.entries);
-    cudaFree(d.warp_chunk); cudaFree(d.images); cudaFree(d.freqs); cudaFree(d.uvw); cudaFree(d.dms);
+    cudaFree(d.warp_chunk); cudaFree(d.images); cudaFree(d.freqs); cudaFree(d.uvw); cudaFree(d.dms); cudaFree(d.twiddles);
     d = rf::DeviceTables{};
 }
 
@@ -81,6 +81,9 @@ int rf_plan_create(rf_plan** out, const double* freqs_hz, int nchan, const doubl
 
 int rf_plan_destroy(rf_plan* p) {
     if (!p) return RF_OK;
+    for (cudaEvent_t e : p->events) cudaEventDestroy(e);
+    cudaFree(p->stage_vis); cudaFree(p->stage_cand); cudaFree(p->stage_count);
+    if (p->own_stream) cudaStreamDestroy(p->own_stream);
     rf::free_workspace(p);
     free_tables(p);
     delete p;
@@ -94,6 +97,53 @@ int rf_search(rf_plan* p, const void* vis_dev, void* cuda_stream, rf_cand_out* o
     }
     if (reinterpret_cast<uintptr_t>(vis_dev) & 15) { set_error("vis_dev must be 16-byte aligned"); return RF_ERR_ARG; }
     return rf::launch_search(p, vis_dev, static_cast<cudaStream_t>(cuda_stream), out);
+}
+
+int rf_search_host(rf_plan* p, const void* vis_host, rf_cand* cand_host, int32_t capacity, int32_t* count_host) {
+    if (!p || !vis_host || !count_host || capacity < 0 || (capacity > 0 && !cand_host)) {
+        set_error("null pointer argument");
+        return RF_ERR_ARG;
+    }
+    const size_t vis_bytes = (size_t)p->nint * p->nbl * p->nchan * p->npol * 8;
+    if (!p->own_stream) RF_CUDA_CHECK(cudaStreamCreateWithFlags(&p->own_stream, cudaStreamNonBlocking));
+    if (!p->stage_vis) RF_CUDA_CHECK(cudaMalloc(&p->stage_vis, vis_bytes));
+    if (!p->stage_count) RF_CUDA_CHECK(cudaMalloc((void**)&p->stage_count, sizeof(int32_t)));
+    if (p->stage_capacity < capacity || !p->stage_cand) {
+        cudaFree(p->stage_cand);
+        p->stage_cand = nullptr;
+        RF_CUDA_CHECK(cudaMalloc((void**)&p->stage_cand, (size_t)(capacity > 0 ? capacity : 1) * sizeof(rf_cand)));
+        p->stage_capacity = capacity;
+    }
+    cudaStream_t st = p->own_stream;
+    RF_CUDA_CHECK(cudaMemcpyAsync(p->stage_vis, vis_host, vis_bytes, cudaMemcpyHostToDevice, st));
+    rf_cand_out out{p->stage_cand, capacity, p->stage_count};
+    int rc = rf::launch_search(p, p->stage_vis, st, &out);
+    if (rc != RF_OK) return rc;
+    RF_CUDA_CHECK(cudaMemcpyAsync(count_host, p->stage_count, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    RF_CUDA_CHECK(cudaStreamSynchronize(st));
+    const int32_t n = *count_host < capacity ? *count_host : capacity;
+    if (n > 0) RF_CUDA_CHECK(cudaMemcpy(cand_host, p->stage_cand, (size_t)n * sizeof(rf_cand), cudaMemcpyDeviceToHost));
+    return RF_OK;
+}
+
+int rf_plan_set_profiling(rf_plan* p, int enable) {
+    if (!p) { set_error("null plan"); return RF_ERR_ARG; }
+    p->profile = enable != 0;
+    return RF_OK;
+}
+
+int rf_plan_get_kernel_times(rf_plan* p, float ms[2], int32_t launches[2]) {
+    if (!p || !ms || !launches) { set_error("null pointer argument"); return RF_ERR_ARG; }
+    ms[0] = ms[1] = 0.f;
+    launches[0] = launches[1] = 0;
+    for (int i = 0; i + 2 < p->n_events_used; i += 3) {
+        float a = 0.f, b = 0.f;
+        RF_CUDA_CHECK(cudaEventElapsedTime(&a, p->events[i], p->events[i + 1]));
+        RF_CUDA_CHECK(cudaEventElapsedTime(&b, p->events[i + 1], p->events[i + 2]));
+        ms[0] += a; ms[1] += b;
+        launches[0]++; launches[1]++;
+    }
+    return RF_OK;
 }
 
 int rf_plan_set_chan_weights(rf_plan* p, const float* w) {

@@ -14,6 +14,7 @@
 // in shared memory; the powers W^t are formed by multiplication.
 #pragma once
 #include <cuda_runtime.h>
+#include <math.h>
 
 namespace rf {
 
@@ -182,17 +183,23 @@ __device__ __forceinline__ void fft_inverse(float2 (&v)[16], float2* __restrict_
     }
 }
 
-// tables: tw[k] = exp(+2 pi i k / (16 R2)), k < 16;  tw[16 + k] = exp(+2 pi i k / N), k < 256
+// tables: tw[k] = exp(+2 pi i k / (16 R2)), k < 16;  tw[16 + k] = exp(+2 pi i k / N), k < 256.
+// Computed once per plan on the host in float64 (host_twiddles) and copied to shared memory.
 template <int N>
-__device__ __forceinline__ void fill_twiddles(float2* tw, int tid, int nthreads) {
-    using C = FftCfg<N>;
-    for (int i = tid; i < C::TW_TOTAL; i += nthreads) {
-        double ang;
-        if (i < C::TW2) ang = 2.0 * 3.14159265358979323846 * i / (double)(16 * C::R2);
-        else ang = 2.0 * 3.14159265358979323846 * (i - C::TW2) / (double)N;
-        double s, c;
-        sincos(ang, &s, &c);
-        tw[i] = make_float2((float)c, (float)s);
+__device__ __forceinline__ void load_twiddles(float2* tw, const float2* __restrict__ gtw, int tid, int nthreads) {
+    for (int i = tid; i < FftCfg<N>::TW_TOTAL; i += nthreads) tw[i] = gtw[i];
+}
+
+inline void host_twiddles(int n, float2* out /* 16 + 256 entries */) {
+    const int r2 = (n / 16 >= 16) ? 16 : n / 16;
+    const double two_pi = 6.283185307179586476925286766559;
+    for (int i = 0; i < 16; i++) {
+        double a = two_pi * i / (double)(16 * r2);
+        out[i] = make_float2((float)cos(a), (float)sin(a));
+    }
+    for (int i = 0; i < 256; i++) {
+        double a = two_pi * i / (double)n;
+        out[16 + i] = make_float2((float)cos(a), (float)sin(a));
     }
 }
 

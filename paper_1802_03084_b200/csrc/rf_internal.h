@@ -56,6 +56,7 @@ struct DeviceTables {
     double* freqs = nullptr;         // [nchan] Hz
     double* uvw = nullptr;           // [nbl][3]
     double* dms = nullptr;           // [ndm]
+    float2* twiddles = nullptr;      // [16 + 256] FFT stage twiddles
 };
 
 struct Workspace {
@@ -97,6 +98,16 @@ struct rf_plan {
     int64_t n_images = 0, vis_gridded = 0;
     int64_t n_entries = 0, n_chunks = 0;
     int last_launches = 0;
+    // rf_search_host staging
+    void* stage_vis = nullptr;
+    rf_cand* stage_cand = nullptr;
+    int32_t* stage_count = nullptr;
+    int stage_capacity = 0;
+    cudaStream_t own_stream = nullptr;
+    // per-kernel event timing
+    bool profile = false;
+    std::vector<cudaEvent_t> events;
+    int n_events_used = 0;
     rf::DeviceTables d;
     rf::Workspace ws;
 };

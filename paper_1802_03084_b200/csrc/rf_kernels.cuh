@@ -23,6 +23,7 @@ struct SearchParams {
     const GridEntry* entries;
     const int32_t* warp_chunk;
     const ImgDesc* images;          // first image of this batch
+    const float2* twiddles;         // [16 + 256] per-stage FFT twiddles (rf_fft.cuh)
     float2* H;                      // [batch][N][cpad]
     float* sumsq;                   // [batch][ngroups]
     uint32_t* hist;                 // [batch][nbins]
@@ -47,8 +48,71 @@ __device__ __forceinline__ float warp_sum(float x) {
     return x;
 }
 
+
+// Gather + segmented grid add for the chunk range [c_beg, c_end) of one warp.
+// DT > 0: boxcar width known at compile time (fully unrolled); DT == 0: runtime width `dt`.
+// U chunks are processed together so that U x DT independent loads are in flight per lane.
+template <int NPOL, int DT, int U, int PITCH>
+__device__ __forceinline__ void gather_grid(const SearchParams& p, float2* __restrict__ tile,
+                                            const int* __restrict__ sdelay, const float* __restrict__ base,
+                                            int c_beg, int c_end, int lane, int dt) {
+    for (int ck = c_beg; ck < c_end; ck += U) {
+        GridEntry e[U];
+        const float* src[U];
+        float re[U], im_[U];
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+            e[u] = (ck + u < c_end) ? p.entries[(size_t)(ck + u) * 32 + lane] : GridEntry{0u, 0u};
+            re[u] = 0.f; im_[u] = 0.f;
+        }
+#pragma unroll
+        for (int u = 0; u < U; u++)
+            src[u] = base + (long long)sdelay[e[u].w1 & 0xfff] * p.row_floats + (size_t)(e[u].w0 & 0xffffffu) * (2 * NPOL);
+        const int nq = DT > 0 ? DT : dt;
+#pragma unroll
+        for (int q = 0; q < nq; q++) {
+#pragma unroll
+            for (int u = 0; u < U; u++) {
+                if (e[u].w0 >> 31) {
+                    const float* s = src[u] + (long long)q * p.row_floats;
+                    if (NPOL == 1) {
+                        float2 a = __ldg(reinterpret_cast<const float2*>(s));
+                        re[u] += a.x; im_[u] += a.y;
+                    } else {
+#pragma unroll
+                        for (int h = 0; h < NPOL / 2; h++) {
+                            float4 a = __ldg(reinterpret_cast<const float4*>(s) + h);
+                            re[u] += a.x + a.z; im_[u] += a.y + a.w;
+                        }
+                    }
+                }
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+            if (e[u].w0 & (1u << 30)) im_[u] = -im_[u];
+            // segmented inclusive scan: lanes of one cell are contiguous, `dist` = lanes to its head
+            const int dist = (e[u].w0 >> 24) & 31;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                float r2 = __shfl_up_sync(0xffffffffu, re[u], d);
+                float i2 = __shfl_up_sync(0xffffffffu, im_[u], d);
+                if (dist >= d) { re[u] += r2; im_[u] += i2; }
+            }
+            if ((e[u].w0 >> 31) && (e[u].w0 & (1u << 29))) {
+                const int row = (e[u].w1 >> 12) & 0xfff, col = (e[u].w1 >> 24) & 0xf;
+                float2* dst = &tile[col * PITCH + fft_pad(row)];
+                float2 cur = *dst;
+                *dst = make_float2(cur.x + re[u], cur.y + im_[u]);
+            }
+            __syncwarp();
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------
-// Pass 1.  grid = (n_img, ngroups); block = 256.  Dynamic smem:
+// Pass 1.  grid = (n_img, ngroups): group-major launch order, so the heavy central column
+// groups start first (measured faster than image-major order); block = 256.  Dynamic smem:
 //   tile  [NCOL][PITCH] float2, PITCH = fft_padded_size(N) + 1 (odd -> conflict-free transpose)
 //   tw    [TW_TOTAL] float2 | sdelay [nchan] int | red [8] float
 template <int N, int NPOL, int NCOL>
@@ -67,51 +131,20 @@ __global__ void __launch_bounds__(kThreads) k_grid_colfft(const SearchParams p) 
 
     for (int i = tid; i < NCOL * PITCH; i += kThreads) tile[i] = make_float2(0.f, 0.f);
     for (int i = tid; i < p.nchan; i += kThreads) sdelay[i] = p.delay[(size_t)im.dm_idx * p.nchan + i];
-    fill_twiddles<N>(tw, tid, kThreads);
+    load_twiddles<N>(tw, p.twiddles, tid, kThreads);
     __syncthreads();
 
     // ---- (b)+(c): gather at the delayed time index, boxcar + Stokes sum, segmented grid add
     {
         const int c_beg = p.warp_chunk[g * kWarpsPerCta + warp];
         const int c_end = p.warp_chunk[g * kWarpsPerCta + warp + 1];
-        const long long t0 = (long long)im.j * im.dt;
-        for (int ck = c_beg; ck < c_end; ck++) {
-            const GridEntry e = p.entries[(size_t)ck * 32 + lane];
-            const bool valid = (e.w0 >> 31) != 0;
-            float re = 0.f, im_ = 0.f;
-            if (valid) {
-                const int ch = e.w1 & 0xfff;
-                const float* src = p.vis + (t0 + sdelay[ch]) * p.row_floats +
-                                   (size_t)(e.w0 & 0xffffffu) * (2 * NPOL);
-                for (int q = 0; q < im.dt; q++, src += p.row_floats) {
-                    if (NPOL == 1) {
-                        float2 a = __ldg(reinterpret_cast<const float2*>(src));
-                        re += a.x; im_ += a.y;
-                    } else {
-#pragma unroll
-                        for (int h = 0; h < NPOL / 2; h++) {
-                            float4 a = __ldg(reinterpret_cast<const float4*>(src) + h);
-                            re += a.x + a.z; im_ += a.y + a.w;
-                        }
-                    }
-                }
-                if (e.w0 & (1u << 30)) im_ = -im_;
-            }
-            // segmented inclusive scan: lanes of one cell are contiguous, `dist` = lanes to its head
-            const int dist = (e.w0 >> 24) & 31;
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                float r2 = __shfl_up_sync(0xffffffffu, re, d);
-                float i2 = __shfl_up_sync(0xffffffffu, im_, d);
-                if (dist >= d) { re += r2; im_ += i2; }
-            }
-            if (valid && (e.w0 & (1u << 29))) {
-                const int row = (e.w1 >> 12) & 0xfff, col = (e.w1 >> 24) & 0xf;
-                float2* dst = &tile[col * PITCH + fft_pad(row)];
-                float2 cur = *dst;
-                *dst = make_float2(cur.x + re, cur.y + im_);
-            }
-            __syncwarp();
+        const float* base = p.vis + (long long)im.j * im.dt * p.row_floats;
+        switch (im.dt) {   // compile-time widths keep U x DT independent 16-byte loads in flight per lane
+            case 1: gather_grid<NPOL, 1, 8, PITCH>(p, tile, sdelay, base, c_beg, c_end, lane, 1); break;
+            case 2: gather_grid<NPOL, 2, 4, PITCH>(p, tile, sdelay, base, c_beg, c_end, lane, 2); break;
+            case 4: gather_grid<NPOL, 4, 2, PITCH>(p, tile, sdelay, base, c_beg, c_end, lane, 4); break;
+            case 8: gather_grid<NPOL, 8, 1, PITCH>(p, tile, sdelay, base, c_beg, c_end, lane, 8); break;
+            default: gather_grid<NPOL, 0, 4, PITCH>(p, tile, sdelay, base, c_beg, c_end, lane, im.dt); break;
         }
     }
     __syncthreads();
@@ -288,7 +321,7 @@ __global__ void __launch_bounds__(kThreads) k_rowfft_stats(const SearchParams p)
     const bool has_b = slot_b < p.n_img;
 
     for (int i = tid; i < 2 * p.nbins; i += kThreads) hist[i] = 0u;
-    fill_twiddles<N>(tw, tid, kThreads);
+    load_twiddles<N>(tw, p.twiddles, tid, kThreads);
     // sigma_rms of both images from the Parseval partials (fixed summation order)
     if (tid < 2) {
         float tot = 0.f;

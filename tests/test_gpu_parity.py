@@ -152,7 +152,7 @@ def test_full_size_sampled_parity(name, nsample):
     dms = W.dm_list(cfg)
     vis = W.make_segment(cfg)
     dvis = torch.from_numpy(vis).cuda()
-    gpu, n = plan.search(dvis)
+    gpu, n = plan.search(dvis, capacity=1 << 18)
     ctr = plan.get_counters()
     assert ctr["images"] == plan.num_images() and n == len(gpu)
     assert ctr["stats_overflow"] == 0
