@@ -181,3 +181,51 @@ def test_full_size_sampled_parity(name, nsample):
             assert (int(c["l_pix"]) % cfg.npix, int(c["m_pix"]) % cfg.npix) == (x, y)
     assert found >= 1, "no injected transient was recovered"
     plan.destroy()
+
+
+def test_streaming_segments():
+    """Config 5: consecutive overlapping segments of the L-band array; every DM searches native
+    t < stride only (each absolute time exactly once), uvw changes per segment (rf_plan_set_uvw)."""
+    torch = _torch()
+    from workloads.generate import segment_ha_hours
+    cfg = W.get_config("stream")
+    dms = W.dm_list(cfg)
+    plan, f, uvw0, cell0 = _plan_for(cfg)
+    plan.set_search_span(cfg.stride_int)
+    delays = O.delay_table(f, dms, cfg.inttime_s)
+    assert int(delays.max()) == cfg.nint - cfg.stride_int          # overlap = max delay = 624
+    assert plan.num_images() == 48000                              # SURVEY section 8 table
+    segs = sorted({src.t0 // cfg.stride_int for src in W.transients(cfg)})[:2]
+    recovered = 0
+    for seg in segs:
+        uvw = W.baseline_uvw_m(cfg, segment_ha_hours(cfg, seg))
+        cell = W.default_cell_rad(cfg, uvw)
+        plan.set_uvw(uvw, cell)
+        _check_tables(plan, cfg, f, uvw, cell, dms)
+        vis = W.make_segment(cfg, seg)
+        dvis = torch.from_numpy(vis).cuda()
+        gpu, n = plan.search(dvis, capacity=1 << 17)
+        assert n == len(gpu) and plan.get_counters()["images"] == 48000
+        for k, dt in enumerate(cfg.dt_list):
+            sel = gpu[gpu["dt_idx"] == k]
+            assert (sel["t_idx"] < cfg.stride_int // dt).all()
+        g = {(int(c["dm_idx"]), int(c["dt_idx"]), int(c["t_idx"])): c for c in gpu}
+        iu, iv, keep = O.cell_table(uvw, f, cfg.npix, cell)
+        keys = []
+        for src in W.transients(cfg):
+            if src.t0 // cfg.stride_int == seg:
+                d = int(np.argmin(np.abs(dms - src.dm)))
+                k = int(np.argmin([abs(dt - src.width) for dt in cfg.dt_list]))
+                keys.append((d, k, (src.t0 - seg * cfg.stride_int) // cfg.dt_list[k]))
+        keys += [(5, 0, 399), (63, 3, 49), (30, 1, 0)]
+        for (d, k, j) in keys:
+            ref = O.search_image(vis, delays, iu, iv, keep, cfg.npix, d, cfg.dt_list[k], j)
+            peak, y, x, sigma, snr = O.image_stats(ref)
+            img, st = plan.debug_image(dvis, d, k, j)
+            assert np.abs(img - ref).max() <= PIX_TOL * np.sqrt((ref ** 2).mean())
+            assert abs(float(st["snr"]) - snr) <= SNR_TOL * snr
+            if abs(snr - cfg.threshold) > NEAR_THR * cfg.threshold:
+                assert ((d, k, j) in g) == (snr >= cfg.threshold)
+            recovered += (d, k, j) in g
+    assert recovered >= 1
+    plan.destroy()
