@@ -141,10 +141,18 @@ int rf_search_host(rf_plan* plan, const void* vis_host, rf_cand* cand_host, int3
 
 /* Per-kernel timing for roofline accounting: when enabled, rf_search brackets every kernel
  * launch with CUDA events on its stream.  After the caller has synchronised, get_kernel_times
- * returns, for the last rf_search, the summed durations (ms) and launch counts of the two
- * kernels: index 0 = grid + column FFT (pass 1), 1 = row FFT + statistics (pass 2).   */
+ * returns, for the last rf_search, the summed durations (ms) and launch counts per kernel
+ * kind: index 0 = grid + column FFT (pass 1, either variant), 1 = row FFT + statistics
+ * (pass 2, either variant), 2 = Stokes-I transpose (prep of the boxcar tree), 3 = unused. */
 int rf_plan_set_profiling(rf_plan* plan, int enable);
-int rf_plan_get_kernel_times(rf_plan* plan, float ms[2], int32_t launches[2]);
+int rf_plan_get_kernel_times(rf_plan* plan, float ms[4], int32_t launches[4]);
+
+/* Resampling strategy (results agree within rounding; B3).  use_tree != 0
+ * (default): power-of-two widths up to 8 are formed in the IMAGE domain as running sums of the
+ * dt = 1 rows inside the row-FFT kernel (boxcar linearity); every other width, and everything
+ * when use_tree == 0 or npix < 256, is averaged at the visibility read, one gridding and
+ * transform per (dm, dt, j).  Rebuilds the work lists.                             */
+int rf_plan_set_mode(rf_plan* plan, int use_tree);
 
 /* Thread-local description of the last error returned on this thread. */
 const char* rf_last_error(void);

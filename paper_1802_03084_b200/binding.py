@@ -20,7 +20,7 @@ EXPORTS = [
     "rf_plan_create", "rf_search", "rf_plan_destroy", "rf_plan_set_chan_weights", "rf_plan_set_uvw",
     "rf_plan_set_search_span", "rf_plan_get_tables", "rf_plan_num_images", "rf_plan_num_t",
     "rf_debug_image", "rf_plan_get_counters", "rf_plan_set_batch", "rf_last_error",
-    "rf_search_host", "rf_plan_set_profiling", "rf_plan_get_kernel_times",
+    "rf_search_host", "rf_plan_set_profiling", "rf_plan_get_kernel_times", "rf_plan_set_mode",
 ]
 
 # numpy view of rf_cand (32 bytes)
@@ -74,6 +74,7 @@ def load_library() -> C.CDLL:
     lib.rf_last_error.restype = C.c_char_p
     lib.rf_search_host.argtypes = [vp, vp, vp, C.c_int32, ip]
     lib.rf_plan_set_profiling.argtypes = [vp, C.c_int]
+    lib.rf_plan_set_mode.argtypes = [vp, C.c_int]
     lib.rf_plan_get_kernel_times.argtypes = [vp, C.POINTER(C.c_float), ip]
     for name in EXPORTS:
         if name not in ("rf_plan_num_images", "rf_last_error"):
@@ -201,11 +202,15 @@ class Plan:
         _check(self._lib.rf_plan_set_profiling(self._h, int(enable)))
 
     def get_kernel_times(self):
-        """(ms[2], launches[2]) of the last search: 0 = grid+column FFT, 1 = row FFT+statistics."""
-        ms = (C.c_float * 2)()
-        n = (C.c_int32 * 2)()
+        """(ms[4], launches[4]) of the last search: 0 = grid+column FFT, 1 = row FFT+statistics, 2 = prep."""
+        ms = (C.c_float * 4)()
+        n = (C.c_int32 * 4)()
         _check(self._lib.rf_plan_get_kernel_times(self._h, ms, n))
-        return [float(ms[0]), float(ms[1])], [int(n[0]), int(n[1])]
+        return [float(v) for v in ms], [int(v) for v in n]
+
+    def set_mode(self, use_tree: bool) -> None:
+        """rf_plan_set_mode: image-domain boxcar tree (default) or per-image resampling at the read."""
+        _check(self._lib.rf_plan_set_mode(self._h, int(use_tree)))
 
     def debug_image(self, vis, dm_idx: int, dt_idx: int, t_idx: int, stream=None):
         """Returns (image float32 [npix][npix] numpy, stats record) of one (dm, dt, t)."""

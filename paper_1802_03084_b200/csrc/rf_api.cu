@@ -33,8 +33,8 @@ int rebuild_geometry(rf_plan* p) {
 
 void free_tables(rf_plan* p) {
     rf::DeviceTables& d = p->d;
-    cudaFree(d.delay); cudaFree(d.cell); cudaFree(d.keep); cudaFree(d.entries);
-    cudaFree(d.warp_chunk); cudaFree(d.images); cudaFree(d.freqs); cudaFree(d.uvw); cudaFree(d.dms); cudaFree(d.twiddles);
+    cudaFree(d.delay); cudaFree(d.cell); cudaFree(d.keep); cudaFree(d.gen.entries); cudaFree(d.gen.warp_chunk);
+    cudaFree(d.tree.entries); cudaFree(d.tree.warp_chunk); cudaFree(d.blocks); cudaFree(d.images); cudaFree(d.freqs); cudaFree(d.uvw); cudaFree(d.dms); cudaFree(d.twiddles);
     d = rf::DeviceTables{};
 }
 
@@ -72,6 +72,7 @@ int rf_plan_create(rf_plan** out, const double* freqs_hz, int nchan, const doubl
     p->dts.assign(dt_list, dt_list + ndt);
     p->weights.assign(nchan, 1.0f);
     p->nbins = 2048;
+    rf::configure_tree(p);
     int rc = rf::build_delay_table(p);
     if (rc == RF_OK) rc = rebuild_geometry(p);
     if (rc != RF_OK) { rf_plan_destroy(p); return rc; }
@@ -132,18 +133,25 @@ int rf_plan_set_profiling(rf_plan* p, int enable) {
     return RF_OK;
 }
 
-int rf_plan_get_kernel_times(rf_plan* p, float ms[2], int32_t launches[2]) {
+int rf_plan_get_kernel_times(rf_plan* p, float ms[4], int32_t launches[4]) {
     if (!p || !ms || !launches) { set_error("null pointer argument"); return RF_ERR_ARG; }
-    ms[0] = ms[1] = 0.f;
-    launches[0] = launches[1] = 0;
-    for (int i = 0; i + 2 < p->n_events_used; i += 3) {
-        float a = 0.f, b = 0.f;
-        RF_CUDA_CHECK(cudaEventElapsedTime(&a, p->events[i], p->events[i + 1]));
-        RF_CUDA_CHECK(cudaEventElapsedTime(&b, p->events[i + 1], p->events[i + 2]));
-        ms[0] += a; ms[1] += b;
-        launches[0]++; launches[1]++;
+    for (int k = 0; k < 4; k++) { ms[k] = 0.f; launches[k] = 0; }
+    for (int i = 1; i < p->n_events_used; i++) {
+        const int kind = p->event_kind[i];
+        if (kind < 0 || kind > 3) continue;
+        float a = 0.f;
+        RF_CUDA_CHECK(cudaEventElapsedTime(&a, p->events[i - 1], p->events[i]));
+        ms[kind] += a;
+        launches[kind]++;
     }
     return RF_OK;
+}
+
+int rf_plan_set_mode(rf_plan* p, int use_tree) {
+    if (!p) { set_error("null plan"); return RF_ERR_ARG; }
+    p->use_tree = use_tree != 0;
+    rf::configure_tree(p);
+    return rebuild_geometry(p);
 }
 
 int rf_plan_set_chan_weights(rf_plan* p, const float* w) {

@@ -43,15 +43,28 @@ struct GridEntry {
     uint32_t w0, w1;
 };
 
+// One block of the image-domain boxcar tree: TB consecutive native integrations of one DM.
+struct BlockDesc {
+    int32_t dm_idx, tb, nsearch, pad;
+};
+
+// Half-plane gridding lists for one choice of columns-per-CTA.
+struct GridLists {
+    GridEntry* entries = nullptr;    // device [n_chunks * 32]
+    int32_t* warp_chunk = nullptr;   // device [ngroups * kWarpsPerCta + 1]
+    int colgrp = 0, cpad = 0, ngroups = 0;
+    int64_t n_chunks = 0;
+};
+
 struct DeviceTables {
     // integer tables (a), (c)
     int32_t* delay = nullptr;        // [ndm][nchan]
     int32_t* cell = nullptr;         // [nbl][nchan][2]
     uint8_t* keep = nullptr;         // [nbl][nchan]
-    // gridding lists
-    GridEntry* entries = nullptr;    // [n_chunks * 32]
-    int32_t* warp_chunk = nullptr;   // [ngroups * kWarpsPerCta + 1] first chunk of each warp range
-    ImgDesc* images = nullptr;       // [n_images]
+    // gridding lists: generic path (colgrp = cols_per_group) and boxcar-tree path
+    GridLists gen, tree;
+    ImgDesc* images = nullptr;       // [n_gen_images] images searched by the generic path
+    BlockDesc* blocks = nullptr;     // [n_blocks] blocks searched by the tree path
     // plan inputs on device
     double* freqs = nullptr;         // [nchan] Hz
     double* uvw = nullptr;           // [nbl][3]
@@ -70,6 +83,13 @@ struct Workspace {
     ImgDesc* dbg_desc = nullptr;     // one descriptor for rf_debug_image
     int batch = 0, rsplit = 1;
     size_t h_elems = 0;
+    // boxcar-tree path
+    float2* visI = nullptr;          // [nbl*nchan][tpitch] Stokes-I (pol sum), time fastest
+    float2* Ht = nullptr;            // [blk_batch][npix][cpad_tree][TB]
+    float* sumsq_t = nullptr;        // [blk_batch][2*TB-1][ngroups_tree]
+    BlockDesc* dbg_block = nullptr;
+    int blk_batch = 0;
+    size_t visI_elems = 0, ht_elems = 0;
 };
 
 }  // namespace rf
@@ -79,6 +99,7 @@ struct rf_plan {
     double inttime = 0, cell = 0;
     float threshold = 0;
     int span = 0;                    // streaming search span (0 = all valid)
+    bool use_tree = true;            // image-domain boxcar tree for power-of-two dt (rf_plan_set_mode)
     int user_batch = 0;
     std::vector<double> freqs, uvw, dms;
     std::vector<int32_t> dts;
@@ -91,12 +112,15 @@ struct rf_plan {
     // derived
     int n_kept = 0, n_dropped = 0;
     int ncol = 0;                    // occupied half-plane columns 0..ncol-1 (ncol <= npix/2+1)
-    int colgrp = 16;                 // columns per pass-1 CTA = rf::cols_per_group(npix)
-    int cpad = 0;                    // ncol rounded up to colgrp
-    int ngroups = 0;
+    // boxcar tree (image-domain resampling): TB = largest power-of-two dt handled by the tree
+    // (0 = tree path off); level l <-> dt = 2^l; tree_dt_idx[l] = index in dt_list or -1
+    int tree_tb = 0;
+    int tree_dt_idx[4] = {-1, -1, -1, -1};
+    int tpitch = 0;                  // time pitch of visI (>= nint + TB, multiple of 16)
+    int64_t n_blocks = 0, n_gen_images = 0;
     int nbins = 2048;
     int64_t n_images = 0, vis_gridded = 0;
-    int64_t n_entries = 0, n_chunks = 0;
+    int64_t n_entries = 0;
     int last_launches = 0;
     // rf_search_host staging
     void* stage_vis = nullptr;
@@ -107,6 +131,7 @@ struct rf_plan {
     // per-kernel event timing
     bool profile = false;
     std::vector<cudaEvent_t> events;
+    std::vector<int> event_kind;
     int n_events_used = 0;
     rf::DeviceTables d;
     rf::Workspace ws;
@@ -116,8 +141,10 @@ namespace rf {
 // rf_tables.cu
 int build_delay_table(rf_plan* p);            // device kernel (float64) -> d.delay, h_delay
 int build_cell_table(rf_plan* p);             // device kernel (float64) -> d.cell/keep, host copies
-int build_grid_lists(rf_plan* p);             // host binning of the cell table -> d.entries, d.warp_chunk
-int build_image_list(rf_plan* p);             // (dm, dt, j) loop -> d.images
+int build_grid_lists(rf_plan* p);             // host binning of the cell table -> d.gen, d.tree
+int build_image_list(rf_plan* p);             // (dm, dt, j) loop -> d.images (generic) + d.blocks (tree)
+int tree_cols_per_group(int npix, int tb);
+void configure_tree(rf_plan* p);              // which dt values ride the boxcar tree    // columns per pass-1 CTA of the tree path
 // rf_search.cu
 int ensure_workspace(rf_plan* p);
 void free_workspace(rf_plan* p);

@@ -6,7 +6,7 @@
 #include <algorithm>
 #include <cstdio>
 
-#include "rf_kernels.cuh"
+#include "rf_tree_kernels.cuh"
 
 namespace rf {
 
@@ -62,28 +62,31 @@ int launch_pass2(const SearchParams& sp, cudaStream_t st) {
     return RF_OK;
 }
 
-int mark(rf_plan* p, cudaStream_t st) {
+// Event bracketing for per-kernel timing: `kind` is the kernel that ran SINCE the previous
+// mark (-1 = none: a start mark); 0 = grid + column FFT, 1 = row FFT + statistics, 2 = prep.
+int mark(rf_plan* p, cudaStream_t st, int kind) {
     if (!p->profile) return RF_OK;
     if (p->n_events_used == (int)p->events.size()) {
         cudaEvent_t e;
         RF_CUDA_CHECK(cudaEventCreate(&e));
         p->events.push_back(e);
+        p->event_kind.push_back(-1);
     }
+    p->event_kind[p->n_events_used] = kind;
     RF_CUDA_CHECK(cudaEventRecord(p->events[p->n_events_used++], st));
     return RF_OK;
 }
 
-// events: [start, after pass 1, after pass 2] per batch when profiling
 int launch_batch(rf_plan* p, const SearchParams& sp, cudaStream_t st) {
     int rc;
-    if ((rc = mark(p, st)) != RF_OK) return rc;
+    if ((rc = mark(p, st, -1)) != RF_OK) return rc;
     switch (p->npix) {
 #define RF_CASE(N, NCOL)                                                                    \
     case N:                                                                                 \
         if ((rc = launch_pass1_npol<N, NCOL>(sp, p->nchan, p->npol, st)) != RF_OK) return rc; \
-        if ((rc = mark(p, st)) != RF_OK) return rc;                                         \
+        if ((rc = mark(p, st, 0)) != RF_OK) return rc;                                      \
         if ((rc = launch_pass2<N>(sp, st)) != RF_OK) return rc;                             \
-        return mark(p, st);
+        return mark(p, st, 1);
         RF_CASE(64, 16)
         RF_CASE(128, 16)
         RF_CASE(256, 16)
@@ -97,12 +100,135 @@ int launch_batch(rf_plan* p, const SearchParams& sp, cudaStream_t st) {
     return RF_ERR_ARG;
 }
 
+// ---------------------------------------------------------------- boxcar-tree path
+template <int N> int tree_nbins(int tb) { return N <= 1024 ? 2048 : (N == 2048 ? 4096 : (tb == 2 ? 8192 : 4096)); }
+
+template <int N, int TB> size_t smem_tree1(int nchan, int ncol) {
+    return (size_t)TB * ncol * (fft_padded_size(N) + 1) * sizeof(float2) + FftCfg<N>::TW_TOTAL * sizeof(float2) +
+           (size_t)nchan * sizeof(int) + (size_t)kWarpsPerCta * (2 * TB - 1) * sizeof(float);
+}
+template <int N, int TB> size_t smem_tree2(int nbins) {
+    const size_t xb = (size_t)(kThreads / FftCfg<N>::TPF) * fft_padded_size(N) * sizeof(float2);
+    const size_t fin = (size_t)2 * nbins * sizeof(uint32_t);
+    return std::max(xb, fin) + FftCfg<N>::TW_TOTAL * sizeof(float2) + (size_t)TB * nbins * sizeof(uint32_t) +
+           64 * 4 + (size_t)2 * kWarpsPerCta * (2 * TB - 1) * 4;
+}
+
+template <int N, int TB, int NCOL>
+int launch_tree(rf_plan* p, const TreeParams& tp, cudaStream_t st) {
+    int rc;
+    {
+        auto kern = k_tree_grid_colfft<N, TB, NCOL>;
+        const size_t smem = smem_tree1<N, TB>(p->nchan, NCOL);
+        static size_t configured = 0;
+        if (smem > configured) {
+            RF_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            configured = smem;
+        }
+        if ((rc = mark(p, st, -1)) != RF_OK) return rc;
+        kern<<<dim3(tp.n_blk, tp.ngroups), kThreads, smem, st>>>(tp);
+        RF_CUDA_CHECK(cudaGetLastError());
+        if ((rc = mark(p, st, 0)) != RF_OK) return rc;
+    }
+    {
+        auto kern = k_tree_rowfft_stats<N, TB>;
+        const size_t smem = smem_tree2<N, TB>(tp.nbins);
+        static size_t configured = 0;
+        if (smem > configured) {
+            RF_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            configured = smem;
+        }
+        kern<<<dim3(tp.n_blk), kThreads, smem, st>>>(tp);
+        RF_CUDA_CHECK(cudaGetLastError());
+        if ((rc = mark(p, st, 1)) != RF_OK) return rc;
+    }
+    return RF_OK;
+}
+
+int launch_tree_batch(rf_plan* p, TreeParams& tp, cudaStream_t st) {
+    const int key = p->npix * 16 + p->tree_tb;
+    switch (key) {
+#define RF_TCASE(N, TB, NCOL) case N * 16 + TB: tp.nbins = tree_nbins<N>(TB); return launch_tree<N, TB, NCOL>(p, tp, st);
+        RF_TCASE(256, 2, 16) RF_TCASE(256, 4, 8) RF_TCASE(256, 8, 4)
+        RF_TCASE(512, 2, 8) RF_TCASE(512, 4, 4) RF_TCASE(512, 8, 2)
+        RF_TCASE(1024, 2, 4) RF_TCASE(1024, 4, 2) RF_TCASE(1024, 8, 1)
+        RF_TCASE(2048, 2, 2) RF_TCASE(2048, 4, 1)
+        RF_TCASE(4096, 2, 2) RF_TCASE(4096, 4, 1)
+#undef RF_TCASE
+    }
+    set_error("unsupported tree configuration npix %d tb %d", p->npix, p->tree_tb);
+    return RF_ERR_ARG;
+}
+
+int launch_prep(rf_plan* p, const void* vis, cudaStream_t st) {
+    const int nelem = p->nbl * p->nchan;
+    dim3 grid((nelem + 31) / 32, (p->tpitch + 31) / 32), block(32, 8);
+    const float* v = reinterpret_cast<const float*>(vis);
+    int rc;
+    if ((rc = mark(p, st, -1)) != RF_OK) return rc;
+    switch (p->npol) {
+        case 1: k_stokes_transpose<1><<<grid, block, 0, st>>>(v, p->ws.visI, p->nint, nelem, p->tpitch); break;
+        case 2: k_stokes_transpose<2><<<grid, block, 0, st>>>(v, p->ws.visI, p->nint, nelem, p->tpitch); break;
+        default: k_stokes_transpose<4><<<grid, block, 0, st>>>(v, p->ws.visI, p->nint, nelem, p->tpitch); break;
+    }
+    RF_CUDA_CHECK(cudaGetLastError());
+    return mark(p, st, 2);
+}
+
+TreeParams tree_params(rf_plan* p) {
+    TreeParams tp{};
+    tp.visI = p->ws.visI;
+    tp.delay = p->d.delay;
+    tp.entries = p->d.tree.entries;
+    tp.warp_chunk = p->d.tree.warp_chunk;
+    tp.twiddles = p->d.twiddles;
+    tp.Ht = p->ws.Ht;
+    tp.sumsq = p->ws.sumsq_t;
+    tp.counters = p->ws.counters;
+    tp.dbg_img = -1;
+    tp.tpitch = p->tpitch;
+    tp.nchan = p->nchan;
+    tp.ncol = p->ncol;
+    tp.cpad = p->d.tree.cpad;
+    tp.ngroups = p->d.tree.ngroups;
+    for (int l = 0; l < 4; l++) tp.dt_idx[l] = p->tree_dt_idx[l];
+    tp.norm = p->n_kept > 0 ? (float)(1.0 / (2.0 * (double)p->n_kept * (double)p->npol)) : 0.f;
+    tp.threshold = p->threshold;
+    return tp;
+}
+
+int ensure_tree_workspace(rf_plan* p) {
+    if (p->tree_tb == 0) return RF_OK;
+    Workspace& w = p->ws;
+    const size_t visI_elems = (size_t)p->nbl * p->nchan * p->tpitch;
+    if (!w.visI || w.visI_elems != visI_elems) {
+        cudaFree(w.visI); w.visI = nullptr;
+        RF_CUDA_CHECK(cudaMalloc((void**)&w.visI, visI_elems * sizeof(float2)));
+        w.visI_elems = visI_elems;
+    }
+    const size_t h_per_blk = (size_t)p->npix * p->d.tree.cpad * p->tree_tb;   // float2 elements
+    int blk_batch = p->user_batch > 0 ? std::max(1, p->user_batch / p->tree_tb) : 0;
+    if (blk_batch <= 0) {
+        const size_t budget = (size_t)3 << 30;
+        blk_batch = (int)std::min<size_t>(4096, std::max<size_t>(1, budget / (h_per_blk * sizeof(float2))));
+    }
+    if (!w.Ht || w.blk_batch != blk_batch || w.ht_elems != h_per_blk * blk_batch) {
+        cudaFree(w.Ht); cudaFree(w.sumsq_t); w.Ht = nullptr; w.sumsq_t = nullptr;
+        RF_CUDA_CHECK(cudaMalloc((void**)&w.Ht, h_per_blk * blk_batch * sizeof(float2)));
+        RF_CUDA_CHECK(cudaMalloc((void**)&w.sumsq_t, (size_t)blk_batch * (2 * p->tree_tb - 1) * p->d.tree.ngroups * sizeof(float)));
+        w.blk_batch = blk_batch;
+        w.ht_elems = h_per_blk * blk_batch;
+    }
+    if (!w.dbg_block) RF_CUDA_CHECK(cudaMalloc((void**)&w.dbg_block, sizeof(BlockDesc)));
+    return RF_OK;
+}
+
 SearchParams base_params(rf_plan* p, const void* vis) {
     SearchParams sp{};
     sp.vis = reinterpret_cast<const float*>(vis);
     sp.delay = p->d.delay;
-    sp.entries = p->d.entries;
-    sp.warp_chunk = p->d.warp_chunk;
+    sp.entries = p->d.gen.entries;
+    sp.warp_chunk = p->d.gen.warp_chunk;
     sp.twiddles = p->d.twiddles;
     sp.H = p->ws.H;
     sp.sumsq = p->ws.sumsq;
@@ -113,8 +239,8 @@ SearchParams base_params(rf_plan* p, const void* vis) {
     sp.counters = p->ws.counters;
     sp.nchan = p->nchan;
     sp.ncol = p->ncol;
-    sp.cpad = p->cpad;
-    sp.ngroups = p->ngroups;
+    sp.cpad = p->d.gen.cpad;
+    sp.ngroups = p->d.gen.ngroups;
     sp.nbins = p->nbins;
     sp.rsplit = p->ws.rsplit;
     sp.row_floats = (long long)p->nbl * p->nchan * p->npol * 2;
@@ -129,6 +255,7 @@ void free_workspace(rf_plan* p) {
     Workspace& w = p->ws;
     cudaFree(w.H); cudaFree(w.sumsq); cudaFree(w.hist); cudaFree(w.peak_val); cudaFree(w.peak_pos);
     cudaFree(w.ticket); cudaFree(w.counters); cudaFree(w.dbg_desc);
+    cudaFree(w.visI); cudaFree(w.Ht); cudaFree(w.sumsq_t); cudaFree(w.dbg_block);
     w = Workspace{};
 }
 
@@ -141,7 +268,7 @@ int ensure_workspace(rf_plan* p) {
         RF_CUDA_CHECK(cudaMalloc((void**)&p->d.twiddles, sizeof(tw)));
         RF_CUDA_CHECK(cudaMemcpy(p->d.twiddles, tw, sizeof(tw), cudaMemcpyHostToDevice));
     }
-    const size_t h_per_img = (size_t)p->npix * p->cpad;          // float2 elements
+    const size_t h_per_img = (size_t)p->npix * p->d.gen.cpad;    // float2 elements
     int batch = p->user_batch;
     if (batch <= 0) {
         // Measured on B200 (L-band): larger batches win (fewer launch tails) even though the
@@ -165,7 +292,7 @@ int ensure_workspace(rf_plan* p) {
     w.rsplit = rsplit;
     w.h_elems = h_per_img * batch;
     RF_CUDA_CHECK(cudaMalloc((void**)&w.H, w.h_elems * sizeof(float2)));
-    RF_CUDA_CHECK(cudaMalloc((void**)&w.sumsq, (size_t)batch * p->ngroups * sizeof(float)));
+    RF_CUDA_CHECK(cudaMalloc((void**)&w.sumsq, (size_t)batch * p->d.gen.ngroups * sizeof(float)));
     RF_CUDA_CHECK(cudaMalloc((void**)&w.hist, (size_t)batch * p->nbins * sizeof(uint32_t)));
     RF_CUDA_CHECK(cudaMalloc((void**)&w.peak_val, (size_t)batch * rsplit * sizeof(float)));
     RF_CUDA_CHECK(cudaMalloc((void**)&w.peak_pos, (size_t)batch * rsplit * sizeof(int32_t)));
@@ -180,19 +307,36 @@ int ensure_workspace(rf_plan* p) {
 
 int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out) {
     int rc = ensure_workspace(p);
+    if (rc == RF_OK) rc = ensure_tree_workspace(p);
     if (rc != RF_OK) return rc;
     RF_CUDA_CHECK(cudaMemsetAsync(out->count, 0, sizeof(int32_t), st));
     RF_CUDA_CHECK(cudaMemsetAsync(p->ws.counters, 0, 4 * sizeof(int32_t), st));
+    p->last_launches = 0;
+    p->n_events_used = 0;
+    if (p->n_kept == 0) return RF_OK;      // nothing gridded: every image is zero, snr := 0
+    // ---- power-of-two widths: blocks of TB integrations through the boxcar tree
+    if (p->tree_tb > 0 && p->n_blocks > 0) {
+        if ((rc = launch_prep(p, vis, st)) != RF_OK) return rc;
+        p->last_launches += 1;
+        TreeParams tp = tree_params(p);
+        tp.cand_items = out->items;
+        tp.cand_count = out->count;
+        tp.cand_capacity = out->capacity;
+        for (int64_t base = 0; base < p->n_blocks; base += p->ws.blk_batch) {
+            tp.blocks = p->d.blocks + base;
+            tp.n_blk = (int)std::min<int64_t>(p->ws.blk_batch, p->n_blocks - base);
+            if ((rc = launch_tree_batch(p, tp, st)) != RF_OK) return rc;
+            p->last_launches += 2;
+        }
+    }
+    // ---- every other width: one gridding + transform per image
     SearchParams sp = base_params(p, vis);
     sp.cand_items = out->items;
     sp.cand_count = out->count;
     sp.cand_capacity = out->capacity;
-    p->last_launches = 0;
-    p->n_events_used = 0;
-    if (p->n_kept == 0) return RF_OK;      // nothing gridded: every image is zero, snr := 0
-    for (int64_t base = 0; base < p->n_images; base += p->ws.batch) {
+    for (int64_t base = 0; base < p->n_gen_images; base += p->ws.batch) {
         sp.images = p->d.images + base;
-        sp.n_img = (int)std::min<int64_t>(p->ws.batch, p->n_images - base);
+        sp.n_img = (int)std::min<int64_t>(p->ws.batch, p->n_gen_images - base);
         if ((rc = launch_batch(p, sp, st)) != RF_OK) return rc;
         p->last_launches += 2;
     }
@@ -202,7 +346,27 @@ int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out
 int launch_debug_image(rf_plan* p, const void* vis, int dm_idx, int dt_idx, int t_idx,
                        float* image_dev, rf_cand* stats_dev, cudaStream_t st) {
     int rc = ensure_workspace(p);
+    if (rc == RF_OK) rc = ensure_tree_workspace(p);
     if (rc != RF_OK) return rc;
+    for (int l = 0; l < 4 && p->tree_tb > 0 && p->n_kept > 0; l++) {
+        if (p->tree_dt_idx[l] != dt_idx) continue;
+        // the image is node (l, i) of block tb of this DM
+        const int per = p->tree_tb >> l;
+        int nsearch = p->nint - p->h_maxdelay[dm_idx];
+        if (p->span > 0) nsearch = std::min(nsearch, p->span);
+        BlockDesc b{dm_idx, t_idx / per, nsearch, 0};
+        RF_CUDA_CHECK(cudaMemcpyAsync(p->ws.dbg_block, &b, sizeof(b), cudaMemcpyHostToDevice, st));
+        RF_CUDA_CHECK(cudaStreamSynchronize(st));
+        if ((rc = launch_prep(p, vis, st)) != RF_OK) return rc;
+        TreeParams tp = tree_params(p);
+        tp.blocks = p->ws.dbg_block;
+        tp.n_blk = 1;
+        tp.image_out = image_dev;
+        tp.stats_out = stats_dev;
+        tp.dbg_img = tree_off(p->tree_tb, l) + t_idx % per;
+        tp.cand_count = nullptr;
+        return launch_tree_batch(p, tp, st);
+    }
     ImgDesc d{dm_idx, dt_idx, t_idx, p->dts[dt_idx]};
     RF_CUDA_CHECK(cudaMemcpyAsync(p->ws.dbg_desc, &d, sizeof(d), cudaMemcpyHostToDevice, st));
     RF_CUDA_CHECK(cudaStreamSynchronize(st));   // `d` lives on this stack frame (debug hook only)

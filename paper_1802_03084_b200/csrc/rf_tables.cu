@@ -139,74 +139,117 @@ int build_grid_lists(rf_plan* p) {
         if (a.elem != b.elem) return a.elem < b.elem;
         return a.conj < b.conj;
     });
-    const int kColsPerGroup = p->colgrp = cols_per_group(N);
     p->ncol = std::max(1, maxcol + 1);
-    p->cpad = (p->ncol + kColsPerGroup - 1) / kColsPerGroup * kColsPerGroup;
-    p->ngroups = p->cpad / kColsPerGroup;
     p->n_entries = (int64_t)raw.size();
 
-    std::vector<GridEntry> entries;
-    std::vector<int32_t> warp_chunk(p->ngroups * kWarpsPerCta + 1, 0);
-    entries.reserve(raw.size() + (size_t)p->ngroups * kWarpsPerCta * 32);
-    size_t pos = 0;
-    for (int g = 0; g < p->ngroups; g++) {
-        size_t gbeg = pos;
-        while (pos < raw.size() && (int)(raw[pos].col / kColsPerGroup) == g) pos++;
-        size_t gend = pos, cnt = gend - gbeg;
-        size_t cut = gbeg;
-        for (int w = 0; w < kWarpsPerCta; w++) {
-            warp_chunk[g * kWarpsPerCta + w] = (int32_t)(entries.size() / 32);
-            // ideal end of this warp's range, moved forward to the next cell boundary
-            size_t want = gbeg + cnt * (w + 1) / kWarpsPerCta;
-            size_t end = std::max(want, cut);
-            if (w == kWarpsPerCta - 1) end = gend;
-            while (end < gend && end > gbeg && raw[end].col == raw[end - 1].col && raw[end].row == raw[end - 1].row) end++;
-            for (size_t s = cut; s < end; s += 32) {
-                size_t e = std::min(end, s + 32);
-                for (size_t k = s; k < s + 32; k++) {
-                    GridEntry ge{0u, 0u};
-                    if (k < e) {
-                        const Raw& r = raw[k];
-                        size_t h = k;   // first lane of this cell inside the chunk
-                        while (h > s && raw[h - 1].col == r.col && raw[h - 1].row == r.row) h--;
-                        bool tail = (k + 1 == e) || raw[k + 1].col != r.col || raw[k + 1].row != r.row;
-                        ge.w0 = r.elem | ((uint32_t)(k - h) << 24) | (tail ? (1u << 29) : 0u) |
-                                (r.conj << 30) | (1u << 31);
-                        ge.w1 = r.ch | (r.row << 12) | ((r.col % kColsPerGroup) << 24);
+    auto emit = [&](GridLists& gl, int kColsPerGroup) -> int {
+        gl.colgrp = kColsPerGroup;
+        gl.cpad = (p->ncol + kColsPerGroup - 1) / kColsPerGroup * kColsPerGroup;
+        gl.ngroups = gl.cpad / kColsPerGroup;
+        std::vector<GridEntry> entries;
+        std::vector<int32_t> warp_chunk(gl.ngroups * kWarpsPerCta + 1, 0);
+        entries.reserve(raw.size() + (size_t)gl.ngroups * kWarpsPerCta * 32);
+        size_t pos = 0;
+        for (int g = 0; g < gl.ngroups; g++) {
+            size_t gbeg = pos;
+            while (pos < raw.size() && (int)(raw[pos].col / kColsPerGroup) == g) pos++;
+            size_t gend = pos, cnt = gend - gbeg;
+            size_t cut = gbeg;
+            for (int w = 0; w < kWarpsPerCta; w++) {
+                warp_chunk[g * kWarpsPerCta + w] = (int32_t)(entries.size() / 32);
+                // ideal end of this warp's range, moved forward to the next cell boundary
+                size_t want = gbeg + cnt * (w + 1) / kWarpsPerCta;
+                size_t end = std::max(want, cut);
+                if (w == kWarpsPerCta - 1) end = gend;
+                while (end < gend && end > gbeg && raw[end].col == raw[end - 1].col && raw[end].row == raw[end - 1].row) end++;
+                for (size_t s = cut; s < end; s += 32) {
+                    size_t e = std::min(end, s + 32);
+                    for (size_t k = s; k < s + 32; k++) {
+                        GridEntry ge{0u, 0u};
+                        if (k < e) {
+                            const Raw& r = raw[k];
+                            size_t h = k;   // first lane of this cell inside the chunk
+                            while (h > s && raw[h - 1].col == r.col && raw[h - 1].row == r.row) h--;
+                            bool tail = (k + 1 == e) || raw[k + 1].col != r.col || raw[k + 1].row != r.row;
+                            ge.w0 = r.elem | ((uint32_t)(k - h) << 24) | (tail ? (1u << 29) : 0u) |
+                                    (r.conj << 30) | (1u << 31);
+                            ge.w1 = r.ch | (r.row << 12) | ((r.col % kColsPerGroup) << 24);
+                        }
+                        entries.push_back(ge);
                     }
-                    entries.push_back(ge);
                 }
+                cut = end;
             }
-            cut = end;
         }
-    }
-    warp_chunk[p->ngroups * kWarpsPerCta] = (int32_t)(entries.size() / 32);
-    p->n_chunks = (int64_t)entries.size() / 32;
-    int rc;
-    if ((rc = upload(&p->d.entries, entries.data(), entries.size())) != RF_OK) return rc;
-    if ((rc = upload(&p->d.warp_chunk, warp_chunk.data(), warp_chunk.size())) != RF_OK) return rc;
-    return RF_OK;
+        warp_chunk[gl.ngroups * kWarpsPerCta] = (int32_t)(entries.size() / 32);
+        gl.n_chunks = (int64_t)entries.size() / 32;
+        int rc;
+        if ((rc = upload(&gl.entries, entries.data(), entries.size())) != RF_OK) return rc;
+        return upload(&gl.warp_chunk, warp_chunk.data(), warp_chunk.size());
+    };
+    int rc = emit(p->d.gen, cols_per_group(N));
+    if (rc == RF_OK && p->tree_tb > 0) rc = emit(p->d.tree, tree_cols_per_group(N, p->tree_tb));
+    return rc;
+}
+
+// Columns per pass-1 CTA of the tree path: TB x NCOL column tiles of N points must fit ~70 KB
+// of shared memory (139 KB for 4096 x 2).
+int tree_cols_per_group(int npix, int tb) {
+    int ncol = (16 * 512) / (npix * tb);
+    if (npix == 4096 && tb == 2) ncol = 2;
+    return ncol < 1 ? 1 : ncol;
 }
 
 // Loop + segment semantics (readings A6, A16): all j with
 // (j+1)*dt <= min(nint - maxdelay(dm), span).
+void configure_tree(rf_plan* p) {
+    // which dt values ride the image-domain boxcar tree (B3)
+    p->tree_tb = 0;
+    for (int l = 0; l < 4; l++) p->tree_dt_idx[l] = -1;
+    if (p->use_tree && p->npix >= 256) {
+        const int tb_max = p->npix <= 1024 ? 8 : 4;
+        for (int k = 0; k < p->ndt; k++) {
+            const int dt = p->dts[k];
+            for (int l = 0; l < 4; l++)
+                if (dt == (1 << l) && dt <= tb_max && p->tree_dt_idx[l] < 0) {
+                    p->tree_dt_idx[l] = k;
+                    p->tree_tb = std::max(p->tree_tb, dt);
+                }
+        }
+        if (p->tree_tb == 1) p->tree_tb = 2;      // the pair transform needs two integrations
+    }
+    p->tpitch = p->tree_tb ? ((p->nint + p->tree_tb + 15) / 16) * 16 : 0;
+}
+
 int build_image_list(rf_plan* p) {
     std::vector<ImgDesc> imgs;
+    std::vector<BlockDesc> blocks;
     p->h_num_t.assign((size_t)p->ndm * p->ndt, 0);
     p->vis_gridded = 0;
+    p->n_images = 0;
     for (int d = 0; d < p->ndm; d++) {
         int nsearch = p->nint - p->h_maxdelay[d];
         if (p->span > 0) nsearch = std::min(nsearch, p->span);
+        bool any_tree = false;
         for (int k = 0; k < p->ndt; k++) {
             int dt = p->dts[k];
             int nj = nsearch > 0 ? nsearch / dt : 0;
             p->h_num_t[(size_t)d * p->ndt + k] = nj;
-            for (int j = 0; j < nj; j++) imgs.push_back({d, k, j, dt});
+            p->n_images += nj;
             p->vis_gridded += (int64_t)nj * dt * p->n_kept;
+            bool in_tree = false;
+            for (int l = 0; l < 4; l++) in_tree |= (p->tree_dt_idx[l] == k);
+            if (in_tree) { any_tree |= nj > 0; continue; }
+            for (int j = 0; j < nj; j++) imgs.push_back({d, k, j, dt});
         }
+        if (any_tree)
+            for (int tb = 0; tb * p->tree_tb < nsearch; tb++) blocks.push_back({d, tb, nsearch, 0});
     }
-    p->n_images = (int64_t)imgs.size();
-    return upload(&p->d.images, imgs.data(), imgs.size());
+    p->n_gen_images = (int64_t)imgs.size();
+    p->n_blocks = (int64_t)blocks.size();
+    int rc = upload(&p->d.images, imgs.data(), imgs.size());
+    if (rc == RF_OK) rc = upload(&p->d.blocks, blocks.data(), blocks.size());
+    return rc;
 }
 
 }  // namespace rf

@@ -1,0 +1,436 @@
+// rf_tree_kernels.cuh -- the "boxcar tree" variant of the hot kernels (sm_100a).
+//
+// Gridding and the FFT are linear and the uv cell of a (baseline, channel) does not depend on
+// time, so the image of (dm, dt, j) is the mean of the dt = 1 images j*dt .. j*dt+dt-1 of the same
+// DM (SURVEY.md section 7 "boxcar linearity"; oracle pin P11).  For power-of-two widths the loops
+// over sampling time and integration (Fig. 2) are therefore walked in BLOCKS of TB
+// consecutive native integrations of one DM:
+//
+//   k_stokes_transpose   : vis [t][bl][ch][pol] -> Stokes-I sum visI [bl*nchan+ch][t] (time fastest),
+//                          so a block reads TB*8 contiguous bytes per (baseline, channel).
+//   k_tree_grid_colfft   : gathers the TB dedispersed samples of every entry, grids TB images into
+//                          shared-memory column tiles, Parseval sums of every tree node, column FFTs,
+//                          store of the half plane as H[y][c][q] (q = integration inside the block).
+//   k_tree_rowfft_stats  : per row, TB/2 Hermitian pair transforms; the wider images are running
+//                          sums of the rows in registers; all 2*TB-1 images get peak, histogram,
+//                          median/MAD, S/N and the threshold test.  The image is never stored.
+#pragma once
+#include <cuda_runtime.h>
+#include <math_constants.h>
+
+#include "rf_kernels.cuh"
+
+namespace rf {
+
+struct TreeParams {
+    const float2* visI;             // [nbl*nchan][tpitch]
+    const int32_t* delay;           // [ndm][nchan]
+    const GridEntry* entries;
+    const int32_t* warp_chunk;
+    const BlockDesc* blocks;        // first block of this batch
+    const float2* twiddles;
+    float2* Ht;                     // [n_blk][N][cpad][TB]
+    float* sumsq;                   // [n_blk][2*TB-1][ngroups]
+    int32_t* counters;
+    rf_cand* cand_items;
+    int32_t* cand_count;
+    int32_t cand_capacity;
+    float* image_out;               // debug: image `dbg_img` of block 0
+    rf_cand* stats_out;
+    int32_t dbg_img;                // -1 = off
+    int32_t tpitch, nchan, ncol, cpad, ngroups, nbins, n_blk;
+    int32_t dt_idx[4];              // tree level -> index in dt_list, or -1
+    float norm;                     // 1 / (2 N_w npol)
+    float threshold;
+};
+
+// image index of tree node (level l, i) inside a block: levels are stored one after the other
+__host__ __device__ constexpr int tree_off(int tb, int l) {
+    int off = 0;
+    for (int m = 0; m < l; m++) off += tb >> m;
+    return off;
+}
+
+// ------------------------------------------------------------------------------------------
+// Stokes-I sum and transpose to time-fastest order.  grid (ceil(E/32), ceil(tpitch/32)), block (32, 8).
+// Rows t >= nint of the output (the read-ahead pad of the last block) are zero.
+template <int NPOL>
+__global__ void k_stokes_transpose(const float* __restrict__ vis, float2* __restrict__ visI,
+                                   int nint, int nelem, int tpitch) {
+    __shared__ float2 tile[32][33];
+    const int e0 = blockIdx.x * 32, t0 = blockIdx.y * 32;
+    for (int r = threadIdx.y; r < 32; r += 8) {
+        const int t = t0 + r, e = e0 + threadIdx.x;
+        float2 s = make_float2(0.f, 0.f);
+        if (t < nint && e < nelem) {
+            const float* src = vis + ((size_t)t * nelem + e) * (2 * NPOL);
+            if (NPOL == 1) {
+                s = *reinterpret_cast<const float2*>(src);
+            } else {
+#pragma unroll
+                for (int h = 0; h < NPOL / 2; h++) {
+                    float4 a = __ldg(reinterpret_cast<const float4*>(src) + h);
+                    s.x += a.x + a.z; s.y += a.y + a.w;
+                }
+            }
+        }
+        tile[r][threadIdx.x] = s;
+    }
+    __syncthreads();
+    for (int r = threadIdx.y; r < 32; r += 8) {
+        const int e = e0 + r, t = t0 + threadIdx.x;
+        if (e < nelem && t < tpitch) visI[(size_t)e * tpitch + t] = tile[threadIdx.x][r];
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Tree pass 1.  grid = (n_blk, ngroups); block = 256.  Dynamic smem:
+//   tile [TB*NCOL][PITCH] float2 (column f = q*NCOL + c) | tw | sdelay [nchan] | red [8][2*TB-1]
+template <int N, int TB, int NCOL>
+__global__ void __launch_bounds__(kThreads) k_tree_grid_colfft(const TreeParams p) {
+    using C = FftCfg<N>;
+    constexpr int PITCH = fft_padded_size(N) + 1;
+    constexpr int NF = TB * NCOL;
+    constexpr int NIMG = 2 * TB - 1;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2* tile = reinterpret_cast<float2*>(smem_raw);
+    float2* tw = tile + NF * PITCH;
+    int* sdelay = reinterpret_cast<int*>(tw + C::TW_TOTAL);
+    float* red = reinterpret_cast<float*>(sdelay + p.nchan);
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int slot = blockIdx.x, g = blockIdx.y;
+    const BlockDesc blk = p.blocks[slot];
+    const int t0 = blk.tb * TB;
+
+    for (int i = tid; i < NF * PITCH; i += kThreads) tile[i] = make_float2(0.f, 0.f);
+    for (int i = tid; i < p.nchan; i += kThreads) sdelay[i] = p.delay[(size_t)blk.dm_idx * p.nchan + i];
+    load_twiddles<N>(tw, p.twiddles, tid, kThreads);
+    __syncthreads();
+
+    // ---- gather TB consecutive dedispersed samples per entry, segmented grid add into TB tiles
+    {
+        const int c_beg = p.warp_chunk[g * kWarpsPerCta + warp];
+        const int c_end = p.warp_chunk[g * kWarpsPerCta + warp + 1];
+        for (int ck = c_beg; ck < c_end; ck++) {
+            const GridEntry e = p.entries[(size_t)ck * 32 + lane];
+            const bool valid = (e.w0 >> 31) != 0;
+            float2 v[TB];
+            const float2* src = p.visI + (size_t)(e.w0 & 0xffffffu) * p.tpitch + (t0 + sdelay[e.w1 & 0xfff]);
+#pragma unroll
+            for (int q = 0; q < TB; q++) v[q] = valid ? __ldg(src + q) : make_float2(0.f, 0.f);
+            if (e.w0 & (1u << 30)) {
+#pragma unroll
+                for (int q = 0; q < TB; q++) v[q].y = -v[q].y;
+            }
+            const int dist = (e.w0 >> 24) & 31;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+#pragma unroll
+                for (int q = 0; q < TB; q++) {
+                    const float r2 = __shfl_up_sync(0xffffffffu, v[q].x, d);
+                    const float i2 = __shfl_up_sync(0xffffffffu, v[q].y, d);
+                    if (dist >= d) { v[q].x += r2; v[q].y += i2; }
+                }
+            }
+            if (valid && (e.w0 & (1u << 29))) {
+                const int row = (e.w1 >> 12) & 0xfff, col = (e.w1 >> 24) & 0xf;
+                float2* dst = &tile[col * PITCH + fft_pad(row)];
+#pragma unroll
+                for (int q = 0; q < TB; q++) {
+                    float2 cur = dst[q * NCOL * PITCH];
+                    dst[q * NCOL * PITCH] = make_float2(cur.x + v[q].x, cur.y + v[q].y);
+                }
+            }
+            __syncwarp();
+        }
+    }
+    __syncthreads();
+
+    // ---- Parseval sums of every tree node: sum_cells w |sum_{q in node} G_q|^2
+    {
+        float acc[NIMG];
+#pragma unroll
+        for (int i = 0; i < NIMG; i++) acc[i] = 0.f;
+        for (int idx = tid; idx < NCOL * N; idx += kThreads) {
+            const int c = idx / N, y = idx % N;
+            const int gc = g * NCOL + c;
+            const float wgt = (gc == 0 || gc == N / 2) ? 1.f : 2.f;
+            float2 s[TB];
+#pragma unroll
+            for (int q = 0; q < TB; q++) s[q] = tile[(q * NCOL + c) * PITCH + fft_pad(y)];
+            int off = 0;
+#pragma unroll
+            for (int cnt = TB; cnt >= 1; cnt >>= 1) {
+#pragma unroll
+                for (int i = 0; i < cnt; i++) acc[off + i] += wgt * (s[i].x * s[i].x + s[i].y * s[i].y);
+                off += cnt;
+#pragma unroll
+                for (int i = 0; i < cnt / 2; i++) s[i] = cadd(s[2 * i], s[2 * i + 1]);
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < NIMG; i++) {
+            const float w = warp_sum(acc[i]);
+            if (lane == 0) red[warp * NIMG + i] = w;
+        }
+    }
+    __syncthreads();
+    if (tid < NIMG) {
+        float tot = 0.f;
+#pragma unroll
+        for (int w = 0; w < kWarpsPerCta; w++) tot += red[w * NIMG + tid];
+        p.sumsq[((size_t)slot * NIMG + tid) * p.ngroups + g] = tot * p.norm * p.norm;
+    }
+
+    // ---- column FFTs in place (inverse, along v)
+    {
+        constexpr int G1 = kThreads / C::TPF;
+        const int grp = tid / C::TPF, t = tid % C::TPF;
+        for (int f = grp; f < NF; f += G1) {
+            float2* col = tile + f * PITCH;
+            float2 v[16];
+            fft_reload<N>(v, col, t);
+            fft_inverse<N>(v, col, tw, t, 1 + grp);
+            fft_group_sync<C::TPF>(1 + grp);
+#pragma unroll
+            for (int e = 0; e < 16; e++)
+                col[fft_pad(t + C::TPF * e)] = make_float2(v[e].x * p.norm, v[e].y * p.norm);
+        }
+    }
+    __syncthreads();
+
+    // ---- store H[slot][y][g*NCOL + c][q]: NCOL*TB*8 contiguous bytes per row
+    {
+        constexpr int SEG = NCOL * TB;
+        float2* Hs = p.Ht + ((size_t)slot * N * p.cpad + g * NCOL) * TB;
+        const int i = tid % SEG, c = i / TB, q = i % TB, y0 = tid / SEG;
+        for (int y = y0; y < N; y += kThreads / SEG)
+            Hs[((size_t)y * p.cpad + c) * TB + q] = tile[(q * NCOL + c) * PITCH + fft_pad(y)];
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Tree pass 2.  grid = (n_blk); block = 256; one CTA = all rows of one block.  Dynamic smem:
+//   xbuf [G2][XB] float2 (reused after the row loop for the unpacked histogram + prefix sums)
+//   | tw | hist [NW][nbins] u32, two images per word (16 bits each) | per-image parameters
+template <int TPF>
+struct TreeStatsCtx {
+    uint32_t* hist;
+    const float* sA;        // bin = x * A + B
+    const float* sScale;    // pixel = x * scale
+    const int* sValid;
+    float* sBest;           // [warp][NIMG]
+    int* sBpos;
+    float B;
+    int nbins, nimg;
+};
+
+template <int N>
+__device__ __forceinline__ void tree_row_stats(const float (&x)[16], int img, int y, int t, int lane, int warp,
+                                               const TreeStatsCtx<N / 16>& cx, float* image_out) {
+    constexpr int TPF = N / 16;
+    if (!cx.sValid[img]) return;
+    const float A = cx.sA[img];
+    uint32_t* hw = cx.hist + (img >> 1) * cx.nbins;
+    const uint32_t inc = (img & 1) ? 65536u : 1u;
+    const int nbm1 = cx.nbins - 1;
+    float m = x[0];
+#pragma unroll
+    for (int e = 0; e < 16; e++) {
+        int bin = __float2int_rd(fmaf(x[e], A, cx.B));
+        atomicAdd(hw + min(max(bin, 0), nbm1), inc);
+        m = fmaxf(m, x[e]);
+    }
+    float wm = m;
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) wm = fmaxf(wm, __shfl_xor_sync(0xffffffffu, wm, d));
+    if (wm > cx.sBest[warp * cx.nimg + img]) {          // warp-uniform
+        int xp = 0x7fffffff;
+        if (m == wm) {
+#pragma unroll
+            for (int e = 15; e >= 0; e--) if (x[e] == wm) xp = t + TPF * e;
+        }
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) xp = min(xp, __shfl_xor_sync(0xffffffffu, xp, d));
+        __syncwarp();
+        if (lane == 0) { cx.sBest[warp * cx.nimg + img] = wm; cx.sBpos[warp * cx.nimg + img] = y * N + xp; }
+        __syncwarp();
+    }
+    if (image_out != nullptr) {
+        const float sc = cx.sScale[img];
+#pragma unroll
+        for (int e = 0; e < 16; e++) image_out[(size_t)y * N + t + TPF * e] = x[e] * sc;
+    }
+}
+
+template <int N, int TB>
+__global__ void __launch_bounds__(kThreads, 2) k_tree_rowfft_stats(const TreeParams p) {
+    using C = FftCfg<N>;
+    constexpr int G2 = kThreads / C::TPF;
+    constexpr int XB = fft_padded_size(N);
+    constexpr int NIMG = 2 * TB - 1;
+    constexpr int NW = (NIMG + 1) / 2;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2* xbuf = reinterpret_cast<float2*>(smem_raw);
+    float2* tw = xbuf + G2 * XB;
+    uint32_t* hist = reinterpret_cast<uint32_t*>(tw + C::TW_TOTAL);          // [NW][nbins]
+    float* sA = reinterpret_cast<float*>(hist + (size_t)NW * p.nbins);       // [16]
+    float* sScale = sA + 16;                                                 // [16]
+    float* sSig = sScale + 16;                                               // [16] sigma_rms per image
+    int* sValid = reinterpret_cast<int*>(sSig + 16);                         // [16]
+    float* sBest = reinterpret_cast<float*>(sValid + 16);                    // [8][NIMG]
+    int* sBpos = reinterpret_cast<int*>(sBest + kWarpsPerCta * NIMG);        // [8][NIMG]
+    uint32_t* hun = reinterpret_cast<uint32_t*>(xbuf);                       // after the row loop
+    uint32_t* cum = hun + p.nbins;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int slot = blockIdx.x;
+    const BlockDesc blk = p.blocks[slot];
+
+    for (int i = tid; i < NW * p.nbins; i += kThreads) hist[i] = 0u;
+    load_twiddles<N>(tw, p.twiddles, tid, kThreads);
+    for (int i = tid; i < kWarpsPerCta * NIMG; i += kThreads) { sBest[i] = -CUDART_INF_F; sBpos[i] = 0; }
+    if (tid < NIMG) {
+        int l = 0, off = 0;
+        while (tid >= off + (TB >> l)) { off += TB >> l; l++; }
+        const int i = tid - off, dt = 1 << l;
+        const int j = blk.tb * (TB >> l) + i;
+        float tot = 0.f;
+        for (int gidx = 0; gidx < p.ngroups; gidx++) tot += p.sumsq[((size_t)slot * NIMG + tid) * p.ngroups + gidx];
+        const float sig = sqrtf(tot) / (float)dt;                // rms of the image (Parseval)
+        const bool valid = p.dt_idx[l] >= 0 && (j + 1) * dt <= blk.nsearch && sig > 0.f;
+        sValid[tid] = valid ? 1 : 0;
+        sSig[tid] = sig;
+        sScale[tid] = 1.f / (float)dt;
+        sA[tid] = valid ? (float)p.nbins / (2.f * kHistRange * sig) / (float)dt : 0.f;
+    }
+    __syncthreads();
+
+    TreeStatsCtx<C::TPF> cx{hist, sA, sScale, sValid, sBest, sBpos, 0.5f * (float)p.nbins, p.nbins, NIMG};
+    const float2* Hblk = p.Ht + (size_t)slot * N * p.cpad * TB;
+    const int grp = tid / C::TPF, t = tid % C::TPF;
+    float2* xb = xbuf + grp * XB;
+    const bool dbg = p.image_out != nullptr && slot == 0;
+
+    for (int y = grp; y < N; y += G2) {
+        const float2* row = Hblk + (size_t)y * p.cpad * TB;
+        float s2p[16], s4p[16];
+#pragma unroll 1
+        for (int p2 = 0; p2 < TB / 2; p2++) {
+            float2 v[16];
+#pragma unroll
+            for (int e = 0; e < 16; e++) {
+                const int c = t + C::TPF * e;
+                const int cc = (e < 8) ? c : N - c;
+                float4 h = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (cc < p.ncol) h = *reinterpret_cast<const float4*>(row + (size_t)cc * TB + 2 * p2);
+                if (cc == 0 || cc == N / 2) v[e] = make_float2(h.x, h.z);
+                else if (e < 8) v[e] = make_float2(h.x - h.w, h.y + h.z);
+                else v[e] = make_float2(h.x + h.w, h.z - h.y);
+            }
+            fft_inverse<N>(v, xb, tw, t, 1 + grp);
+            float a[16], s2[16];
+#pragma unroll
+            for (int e = 0; e < 16; e++) a[e] = v[e].x;
+            tree_row_stats<N>(a, 2 * p2, y, t, lane, warp, cx, (dbg && p.dbg_img == 2 * p2) ? p.image_out : nullptr);
+#pragma unroll
+            for (int e = 0; e < 16; e++) { a[e] = v[e].y; s2[e] = v[e].x + v[e].y; }
+            tree_row_stats<N>(a, 2 * p2 + 1, y, t, lane, warp, cx, (dbg && p.dbg_img == 2 * p2 + 1) ? p.image_out : nullptr);
+            {
+                const int img = TB + p2;
+                tree_row_stats<N>(s2, img, y, t, lane, warp, cx, (dbg && p.dbg_img == img) ? p.image_out : nullptr);
+            }
+            if (TB >= 4) {
+                if (p2 & 1) {
+                    float s4[16];
+#pragma unroll
+                    for (int e = 0; e < 16; e++) s4[e] = s2p[e] + s2[e];
+                    const int img = TB + TB / 2 + (p2 >> 1);
+                    tree_row_stats<N>(s4, img, y, t, lane, warp, cx, (dbg && p.dbg_img == img) ? p.image_out : nullptr);
+                    if (TB >= 8) {
+                        if (p2 == 3) {
+#pragma unroll
+                            for (int e = 0; e < 16; e++) s4[e] += s4p[e];
+                            const int img8 = TB + TB / 2 + TB / 4;
+                            tree_row_stats<N>(s4, img8, y, t, lane, warp, cx, (dbg && p.dbg_img == img8) ? p.image_out : nullptr);
+                        } else {
+#pragma unroll
+                            for (int e = 0; e < 16; e++) s4p[e] = s4[e];
+                        }
+                    }
+                } else {
+#pragma unroll
+                    for (int e = 0; e < 16; e++) s2p[e] = s2[e];
+                }
+            }
+        }
+    }
+    __syncthreads();
+
+    // ---- per image: unpack the histogram, prefix sums, median / MAD, S/N, threshold
+    for (int img = 0; img < NIMG; img++) {
+        const bool report_zero = p.stats_out != nullptr && slot == 0 && img == p.dbg_img;
+        if (!sValid[img] && !report_zero) continue;            // block-uniform
+        const uint32_t* hw = hist + (img >> 1) * p.nbins;
+        const int sh = (img & 1) * 16;
+        const int per = p.nbins / kThreads;
+        uint32_t local = 0;
+        for (int i = 0; i < per; i++) {
+            const uint32_t c = (hw[tid * per + i] >> sh) & 0xffffu;
+            hun[tid * per + i] = c;
+            local += c;
+        }
+        uint32_t inc = local;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            uint32_t o = __shfl_up_sync(0xffffffffu, inc, d);
+            if (lane >= d) inc += o;
+        }
+        __shared__ uint32_t wtot[kWarpsPerCta];
+        if (lane == 31) wtot[warp] = inc;
+        __syncthreads();
+        uint32_t base = inc - local, total = 0;
+        for (int w = 0; w < kWarpsPerCta; w++) { if (w < warp) base += wtot[w]; total += wtot[w]; }
+        for (int i = 0; i < per; i++) { cum[tid * per + i] = base; base += hun[tid * per + i]; }
+        __syncthreads();
+        if (warp == 0) {
+            int overflow = 0;
+            float sigma = 0.f;
+            const float sig_rms = sSig[img];
+            if (sValid[img]) {
+                if (total != (uint32_t)N * (uint32_t)N) overflow = 1;   // a 16-bit counter wrapped
+                HistView hv{hun, cum, p.nbins, -kHistRange * sig_rms, (float)p.nbins / (2.f * kHistRange * sig_rms)};
+                sigma = robust_sigma_from_hist(hv, (float)N * (float)N, lane, &overflow);
+            }
+            if (lane == 0) {
+                float bv = -CUDART_INF_F;
+                int bp = 0;
+                for (int w = 0; w < kWarpsPerCta; w++) {
+                    const float ov = sBest[w * NIMG + img];
+                    const int op = sBpos[w * NIMG + img];
+                    if (ov > bv || (ov == bv && op < bp)) { bv = ov; bp = op; }
+                }
+                int l = 0, off = 0;
+                while (img >= off + (TB >> l)) { off += TB >> l; l++; }
+                const float peak = sValid[img] ? bv * sScale[img] : 0.f;
+                const float snr = sigma > 0.f ? peak / sigma : 0.f;
+                const int x = bp % N, yy = bp / N;
+                rf_cand c;
+                c.dm_idx = blk.dm_idx; c.dt_idx = p.dt_idx[l]; c.t_idx = blk.tb * (TB >> l) + (img - off);
+                c.l_pix = x < N / 2 ? x : x - N;
+                c.m_pix = yy < N / 2 ? yy : yy - N;
+                c.peak = peak; c.sigma = sigma; c.snr = snr;
+                if (overflow) atomicAdd(&p.counters[0], 1);
+                if (report_zero) *p.stats_out = c;
+                if (p.cand_count != nullptr && sValid[img] && snr >= p.threshold) {
+                    int idx = atomicAdd(p.cand_count, 1);
+                    if (idx < p.cand_capacity) p.cand_items[idx] = c;
+                }
+            }
+        }
+        __syncthreads();
+    }
+}
+
+}  // namespace rf
