@@ -9,7 +9,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "librealfast_b200.so")
 SOURCES = ["rf_api.cu", "rf_tables.cu", "rf_search.cu"]
-HEADERS = ["rf_internal.h", "rf_fft.cuh", "rf_kernels.cuh", os.path.join("..", "..", "include", "realfast.h")]
+HEADERS = ["rf_internal.h", "rf_fft.cuh", "rf_kernels.cuh", "rf_tree_kernels.cuh",
+           os.path.join("..", "..", "include", "realfast.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
     "-Xcompiler", "-fPIC", "-Xcompiler", "-O2", "-DNDEBUG",

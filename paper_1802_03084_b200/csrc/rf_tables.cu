@@ -206,8 +206,10 @@ void configure_tree(rf_plan* p) {
     // which dt values ride the image-domain boxcar tree (B3)
     p->tree_tb = 0;
     for (int l = 0; l < 4; l++) p->tree_dt_idx[l] = -1;
-    if (p->use_tree && p->npix >= 256) {
-        const int tb_max = p->npix <= 1024 ? 8 : 4;
+    // npix >= 2048: one CTA per block starves the GPU and the shared-memory tiles shrink to 1-2
+    // columns; measured slower than the generic path (hi-res config: 2.7 s vs 1.2 s), so off.
+    if (p->use_tree && p->npix >= 256 && p->npix <= 1024) {
+        const int tb_max = 8;
         for (int k = 0; k < p->ndt; k++) {
             const int dt = p->dts[k];
             for (int l = 0; l < 4; l++)

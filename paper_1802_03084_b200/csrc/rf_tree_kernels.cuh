@@ -273,7 +273,9 @@ __global__ void __launch_bounds__(kThreads, 2) k_tree_rowfft_stats(const TreePar
     constexpr int NW = (NIMG + 1) / 2;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2* xbuf = reinterpret_cast<float2*>(smem_raw);
-    float2* tw = xbuf + G2 * XB;
+    // region 0 holds the FFT exchange buffers, later the unpacked histogram + prefix sums
+    const int region0 = max(G2 * XB, p.nbins);                               // float2 units
+    float2* tw = xbuf + region0;
     uint32_t* hist = reinterpret_cast<uint32_t*>(tw + C::TW_TOTAL);          // [NW][nbins]
     float* sA = reinterpret_cast<float*>(hist + (size_t)NW * p.nbins);       // [16]
     float* sScale = sA + 16;                                                 // [16]

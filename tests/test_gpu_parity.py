@@ -6,6 +6,7 @@ import pytest
 
 import oracle as O
 import workloads as W
+import workloads.generate  # noqa: F401
 
 pytestmark = pytest.mark.gpu
 
@@ -228,4 +229,76 @@ def test_streaming_segments():
                 assert ((d, k, j) in g) == (snr >= cfg.threshold)
             recovered += (d, k, j) in g
     assert recovered >= 1
+    plan.destroy()
+
+
+def test_tree_and_generic_paths_agree():
+    """The two resampling strategies (image-domain boxcar tree vs averaging at the visibility read,
+    DESIGN.md B3) give the same candidates; mixed dt lists route each width to the right path."""
+    torch = _torch()
+    import paper_1802_03084_b200 as R
+    cfg = W.get_config("lband")
+    f, uvw, dms = W.channel_freqs_hz(cfg), W.baseline_uvw_m(cfg), W.dm_list(cfg)[:16:2]
+    cell = W.default_cell_rad(cfg, uvw)
+    nint = 192
+    src = [W.generate.Transient(0.25, 40, -77, float(dms[3]), 3, 50)]
+    vis = W.make_segment(cfg, sources=src)[:nint].copy()
+    dvis = torch.from_numpy(vis).cuda()
+    dts = (1, 2, 3, 4, 8, 16)                     # 3 and 16 are not tree widths
+    plan = R.Plan(f, uvw, cfg.npol, nint, cfg.inttime_s, cfg.npix, cell, dms, dts, 6.0)
+    a, na = plan.search(dvis, capacity=1 << 16)
+    plan.set_mode(False)
+    b, nb = plan.search(dvis, capacity=1 << 16)
+    assert na == len(a) and nb == len(b) and na > 20
+    ka = {(int(c["dm_idx"]), int(c["dt_idx"]), int(c["t_idx"])): c for c in a}
+    kb = {(int(c["dm_idx"]), int(c["dt_idx"]), int(c["t_idx"])): c for c in b}
+    for key in set(ka) ^ set(kb):
+        c = ka.get(key, kb.get(key))
+        assert abs(float(c["snr"]) - 6.0) <= NEAR_THR * 6.0, key
+    both = set(ka) & set(kb)
+    assert {k[1] for k in both} >= {0, 1, 3, 4}
+    for key in both:
+        assert abs(float(ka[key]["snr"]) - float(kb[key]["snr"])) <= SNR_TOL * float(kb[key]["snr"]), key
+        assert (ka[key]["l_pix"], ka[key]["m_pix"]) == (kb[key]["l_pix"], kb[key]["m_pix"])
+    # and against the oracle on a few images of each width
+    delays = O.delay_table(f, dms, cfg.inttime_s)
+    iu, iv, keep = O.cell_table(uvw, f, cfg.npix, cell)
+    plan.set_mode(True)
+    for (d, k, j) in [(3, 0, 51), (3, 1, 25), (3, 2, 16), (3, 3, 12), (3, 4, 6), (3, 5, 3), (0, 4, 23), (7, 3, 0)]:
+        ref = O.search_image(vis, delays, iu, iv, keep, cfg.npix, d, dts[k], j)
+        peak, y, x, sigma, snr = O.image_stats(ref)
+        img, st = plan.debug_image(dvis, d, k, j)
+        assert np.abs(img - ref).max() <= PIX_TOL * np.sqrt((ref ** 2).mean()), (d, k, j)
+        assert abs(float(st["snr"]) - snr) <= SNR_TOL * snr, (d, k, j)
+    plan.destroy()
+
+
+def test_sigma_statistics_many_images():
+    """S/N parity on 150 L-band images (threshold 0 -> every image is emitted): the histogram
+    quantiles of the CUDA path against the oracle's exact median / MAD."""
+    torch = _torch()
+    import paper_1802_03084_b200 as R
+    cfg = W.get_config("lband")
+    f, uvw = W.channel_freqs_hz(cfg), W.baseline_uvw_m(cfg)
+    cell = W.default_cell_rad(cfg, uvw)
+    dms = np.array([0.0, 333.0, 777.0])
+    nint, dts = 600, (1, 2, 4, 8)
+    vis = W.make_segment(cfg)[:nint].copy()
+    plan = R.Plan(f, uvw, cfg.npol, nint, cfg.inttime_s, cfg.npix, cell, dms, dts, 0.0)
+    gpu, n = plan.search(torch.from_numpy(vis).cuda(), capacity=1 << 14)
+    assert n == plan.num_images() == len(gpu)
+    g = {(int(c["dm_idx"]), int(c["dt_idx"]), int(c["t_idx"])): c for c in gpu}
+    delays = O.delay_table(f, dms, cfg.inttime_s)
+    iu, iv, keep = O.cell_table(uvw, f, cfg.npix, cell)
+    rng = np.random.default_rng(3)
+    keys = [list(g)[i] for i in rng.choice(len(g), size=150, replace=False)]
+    worst = 0.0
+    for (d, k, j) in keys:
+        ref = O.search_image(vis, delays, iu, iv, keep, cfg.npix, d, dts[k], j)
+        peak, y, x, sigma, snr = O.image_stats(ref)
+        c = g[(d, k, j)]
+        worst = max(worst, abs(float(c["snr"]) - snr) / snr)
+        assert (int(c["l_pix"]) % cfg.npix, int(c["m_pix"]) % cfg.npix) == (x, y)
+    assert worst <= SNR_TOL, worst
+    print("worst relative S/N deviation over 150 images:", worst)
     plan.destroy()
