@@ -86,7 +86,8 @@ def _setup(cfg, segment=0):
 
 def _alg_bytes(cfg, plan):
     """A_img = 16 N_bl N_chan,w dt + 16 N_pix^2 per image; split per kernel as
-    pass 1 = the visibility read + the hand-off write (8 N^2), pass 2 = the hand-off read (8 N^2)."""
+    pass 1 (+ the Stokes transpose that feeds it) = the visibility read + the hand-off write (8 N^2),
+    pass 2 = the hand-off read (8 N^2)."""
     c = plan.get_counters()
     images = c["images"]
     vis_bytes = 16.0 * c["vis_gridded"]                     # 16 B per (bl, ch) pol pair per native sample
@@ -213,8 +214,6 @@ def run_ours(args, cfg):
     plan.set_profiling(True)
     sampler = ClockSampler(local)
     sampler.start()
-    k_ms = [0.0, 0.0]
-    k_n = [0, 0]
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     e0.record(stream)
@@ -254,10 +253,16 @@ def run_ours(args, cfg):
     if rank == 0:
         peak, peak_src = _peaks()
         dom = 0 if k_ms[0] >= k_ms[1] else 1
-        dom_name = ["k_grid_colfft (dedisperse+grid+column FFT)", "k_rowfft_stats (row FFT+statistics)"][dom]
+        dom_name = ["grid + column FFT kernels (k_tree_grid_colfft / k_grid_colfft)",
+                    "row FFT + statistics kernels (k_tree_rowfft_stats / k_rowfft_stats)"][dom]
         per_launch_ms = k_ms[dom] / max(1, k_n[dom])
         per_launch_bytes = alg["pass1" if dom == 0 else "pass2"] / max(1, k_n[dom])
         achieved = per_launch_bytes / (per_launch_ms * 1e-3) / 1e9
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "r1_traffic_lband.json.txt")
+        if cfg.name == "lband" and not args.batch and os.path.exists(tpath):
+            with open(tpath) as fh:       # one ncu --set full capture of this launch configuration
+                traffic = json.load(fh)["pass1_dram_bytes_per_launch" if dom == 0 else "pass2_dram_bytes_per_launch"]
         path_gbs = alg["total"] / (ms_per_step * 1e-3) / 1e9
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -274,8 +279,10 @@ def run_ours(args, cfg):
                     "d2h_bytes_per_step": int(4 + min(n_e2e, capacity) * 32)},
             "gpu_launches": int(launches) * args.steps,
             "roofline": {"bound": "hbm", "kernel": dom_name, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
-                         "kernel_ms_per_step": {"pass1": k_ms[0], "pass2": k_ms[1]},
+                         "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                         "alg_bytes_per_launch": per_launch_bytes,
+                         "kernel_ms_per_step": {"pass1": k_ms[0], "pass2": k_ms[1], "prep": k_ms[2]},
+                         "kernel_launches_per_step": {"pass1": k_n[0], "pass2": k_n[1], "prep": k_n[2]},
                          "path": {"alg_bytes_per_step": alg["total"], "achieved": path_gbs, "frac": path_gbs / peak}},
         }
         if world == 1 and not args.no_cpu_baseline:
