@@ -126,10 +126,17 @@ template <int TPF> __device__ __forceinline__ void fft_group_sync(int bar_id) {
 // One Stockham stage.  P = product of the previous radices.  FIRST stages have no
 // twiddles.  Non-LAST stages scatter to shared memory; the LAST stage leaves the
 // result in v in natural register layout.
+//
+// Index arithmetic: the padded index fft_pad(i) = i + (i >> 4) of the scatter target
+// base + r*P is LINEAR in r for every stage (P = 1: base is a multiple of 16 and r < 16;
+// P = 16 or 256: r*P is a multiple of 16), so one padded base per butterfly plus a
+// compile-time stride replaces a shift and two adds per access:
+//   fft_pad(base + r*P) = fft_pad(base) + r * (P == 1 ? 1 : P + P/16).
 template <int N, int R, int P, bool LAST>
 __device__ __forceinline__ void fft_stage(float2 (&v)[16], float2* __restrict__ sm,
                                           const float2* __restrict__ tw, int tid) {
     constexpr int TPF = N / 16, M = 16 / R;
+    constexpr int STRIDE = (P == 1) ? 1 : P + P / 16;
 #pragma unroll
     for (int m = 0; m < M; m++) {
         float2 u[R];
@@ -143,18 +150,38 @@ __device__ __forceinline__ void fft_stage(float2 (&v)[16], float2* __restrict__ 
 #pragma unroll
             for (int r = 0; r < R; r++) v[m + r * M] = u[r];
         } else {
-            const int base = (b - k) * R + k;
+            float2* dst = sm + fft_pad((b - k) * R + k);
 #pragma unroll
-            for (int r = 0; r < R; r++) sm[fft_pad(base + r * P)] = u[r];
+            for (int r = 0; r < R; r++) dst[r * STRIDE] = u[r];
         }
     }
 }
 
+// v[e] <-> element tid + TPF*e.  For TPF a multiple of 16 the padded index is linear in e.
 template <int N>
 __device__ __forceinline__ void fft_reload(float2 (&v)[16], const float2* __restrict__ sm, int tid) {
     constexpr int TPF = N / 16;
+    if (TPF % 16 == 0) {
+        const float2* src = sm + fft_pad(tid);
 #pragma unroll
-    for (int e = 0; e < 16; e++) v[e] = sm[fft_pad(tid + TPF * e)];
+        for (int e = 0; e < 16; e++) v[e] = src[e * (TPF + TPF / 16)];
+    } else {
+#pragma unroll
+        for (int e = 0; e < 16; e++) v[e] = sm[fft_pad(tid + TPF * e)];
+    }
+}
+// the matching store (natural register layout -> padded buffer), with an optional scale
+template <int N>
+__device__ __forceinline__ void fft_unload(const float2 (&v)[16], float2* __restrict__ sm, int tid, float scale) {
+    constexpr int TPF = N / 16;
+    if (TPF % 16 == 0) {
+        float2* dst = sm + fft_pad(tid);
+#pragma unroll
+        for (int e = 0; e < 16; e++) dst[e * (TPF + TPF / 16)] = make_float2(v[e].x * scale, v[e].y * scale);
+    } else {
+#pragma unroll
+        for (int e = 0; e < 16; e++) sm[fft_pad(tid + TPF * e)] = make_float2(v[e].x * scale, v[e].y * scale);
+    }
 }
 
 // Inverse FFT of the 16 x TPF values held in registers by the TPF threads of a group.

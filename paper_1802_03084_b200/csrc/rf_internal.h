@@ -25,6 +25,7 @@ void set_error(const char* fmt, ...);
 inline int cols_per_group(int npix) { return npix <= 512 ? 16 : (npix == 1024 ? 8 : 4); }
 constexpr int kWarpsPerCta = 8;     // 256 threads everywhere
 constexpr int kThreads = 32 * kWarpsPerCta;
+constexpr int kTreeUnroll = 8;      // iterations of the tree gather kept in flight per warp
 constexpr float kHistRange = 3.5f;  // histogram covers +-kHistRange * sigma_rms
 
 // One image of the search loop: 16 bytes, device-resident list.
@@ -48,11 +49,14 @@ struct BlockDesc {
     int32_t dm_idx, tb, nsearch, pad;
 };
 
+// Tree-path lists reuse GridEntry with a different meaning of bits 24..29 of w0:
+//   bit 29 = END: last iteration of its cell (all entries of that iteration carry it); bits 24..28 unused;
+//   w1 row/column are those of the CELL in every entry of its iterations.
 // Half-plane gridding lists for one choice of columns-per-CTA.
 struct GridLists {
     GridEntry* entries = nullptr;    // device [n_chunks * 32]
-    int32_t* warp_chunk = nullptr;   // device [ngroups * kWarpsPerCta + 1]
-    int colgrp = 0, cpad = 0, ngroups = 0;
+    int32_t* warp_chunk = nullptr;   // device [ngroups * kWarpsPerCta + 1] chunk (generic) / iteration (tree) ranges
+    int colgrp = 0, cpad = 0, ngroups = 0, lg = 0;   // lg: entries per warp iteration (tree lists)
     int64_t n_chunks = 0;
 };
 

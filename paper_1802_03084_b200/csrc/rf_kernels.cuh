@@ -167,9 +167,7 @@ __global__ void __launch_bounds__(kThreads) k_grid_colfft(const SearchParams p) 
             ss += wgt * s;
             fft_inverse<N>(v, col, tw, t, 1 + grp);
             fft_group_sync<C::TPF>(1 + grp);            // all lanes done reading the exchange data
-#pragma unroll
-            for (int e = 0; e < 16; e++)
-                col[fft_pad(t + C::TPF * e)] = make_float2(v[e].x * scale, v[e].y * scale);
+            fft_unload<N>(v, col, t, scale);
         }
     }
     ss = warp_sum(ss);
@@ -335,7 +333,7 @@ __global__ void __launch_bounds__(kThreads) k_rowfft_stats(const SearchParams p)
     const float lo_a = -kHistRange * sig_a, lo_b = -kHistRange * sig_b;
     const float iw_a = sig_a > 0.f ? (float)p.nbins / (2.f * kHistRange * sig_a) : 0.f;
     const float iw_b = sig_b > 0.f ? (float)p.nbins / (2.f * kHistRange * sig_b) : 0.f;
-    const int nbm1 = p.nbins - 1;
+    const unsigned nbm1 = (unsigned)p.nbins - 1u;
 
     const float2* Ha = p.H + (size_t)slot_a * N * p.cpad;
     const float2* Hb = p.H + (size_t)(has_b ? slot_b : slot_a) * N * p.cpad;
@@ -389,15 +387,15 @@ __global__ void __launch_bounds__(kThreads) k_rowfft_stats(const SearchParams p)
             if (iw_a > 0.f) {
 #pragma unroll
                 for (int e = 0; e < 16; e++) {
-                    int bin = __float2int_rd((v[e].x - lo_a) * iw_a);
-                    atomicAdd(&hist[min(max(bin, 0), nbm1)], 1u);
+                    const unsigned bin = __float2uint_rd((v[e].x - lo_a) * iw_a);   // saturates below 0
+                    atomicAdd(&hist[min(bin, nbm1)], 1u);
                 }
             }
             if (has_b && iw_b > 0.f) {
 #pragma unroll
                 for (int e = 0; e < 16; e++) {
-                    int bin = __float2int_rd((v[e].y - lo_b) * iw_b);
-                    atomicAdd(&hist[p.nbins + min(max(bin, 0), nbm1)], 1u);
+                    const unsigned bin = __float2uint_rd((v[e].y - lo_b) * iw_b);
+                    atomicAdd(&hist[p.nbins + min(bin, nbm1)], 1u);
                 }
             }
         }

@@ -187,8 +187,78 @@ int build_grid_lists(rf_plan* p) {
         if ((rc = upload(&gl.entries, entries.data(), entries.size())) != RF_OK) return rc;
         return upload(&gl.warp_chunk, warp_chunk.data(), warp_chunk.size());
     };
+    // Tree path ("time in lanes"): a warp reads LG = 32/TB entries per iteration, lane = (entry j,
+    // integration q), so the TB consecutive samples of an entry are one coalesced 8*TB-byte read.
+    // Every cell is owned by ONE warp: its entries fill ceil(n/LG) consecutive iterations, the lane
+    // accumulates over the iterations in a register, and the iteration flagged END reduces the LG
+    // lane groups (xor shuffles) and stores the cell -- no read-modify-write, fixed summation order.
+    // Cells are dealt to the 8 warps of the CTA longest-first onto the least-loaded warp; each warp's
+    // stream is padded to a multiple of kTreeUnroll iterations with weight-0 entries.
+    auto emit_tree = [&](GridLists& gl, int kColsPerGroup, int LG) -> int {
+        gl.colgrp = kColsPerGroup;
+        gl.lg = LG;
+        gl.cpad = (p->ncol + kColsPerGroup - 1) / kColsPerGroup * kColsPerGroup;
+        gl.ngroups = gl.cpad / kColsPerGroup;
+        struct Cell { size_t first; int n, iters; };
+        std::vector<GridEntry> entries;
+        std::vector<int32_t> warp_iter(gl.ngroups * kWarpsPerCta + 1, 0);
+        entries.reserve(raw.size() * 5 / 4 + (size_t)gl.ngroups * kWarpsPerCta * kTreeUnroll * LG);
+        std::vector<Cell> cells;
+        size_t pos = 0;
+        for (int g = 0; g < gl.ngroups; g++) {
+            const size_t gbeg = pos;
+            while (pos < raw.size() && (int)(raw[pos].col / kColsPerGroup) == g) pos++;
+            const size_t gend = pos;
+            cells.clear();
+            for (size_t c0 = gbeg; c0 < gend;) {
+                size_t c1 = c0;
+                while (c1 < gend && raw[c1].col == raw[c0].col && raw[c1].row == raw[c0].row) c1++;
+                cells.push_back({c0, (int)(c1 - c0), (int)((c1 - c0 + LG - 1) / LG)});
+                c0 = c1;
+            }
+            std::vector<size_t> order(cells.size());
+            for (size_t i = 0; i < order.size(); i++) order[i] = i;
+            std::stable_sort(order.begin(), order.end(), [&](size_t a, size_t b) { return cells[a].iters > cells[b].iters; });
+            std::vector<size_t> owned[kWarpsPerCta];
+            long long load[kWarpsPerCta] = {0};
+            for (size_t i : order) {
+                int best = 0;
+                for (int w = 1; w < kWarpsPerCta; w++) if (load[w] < load[best]) best = w;
+                owned[best].push_back(i);
+                load[best] += cells[i].iters;
+            }
+            for (int w = 0; w < kWarpsPerCta; w++) {
+                warp_iter[g * kWarpsPerCta + w] = (int32_t)(entries.size() / LG);
+                std::sort(owned[w].begin(), owned[w].end());        // (column, row) order inside the warp
+                size_t iters = 0;
+                for (size_t ci : owned[w]) {
+                    const Cell& c = cells[ci];
+                    const Raw& r0 = raw[c.first];
+                    for (int it = 0; it < c.iters; it++)
+                        for (int j = 0; j < LG; j++) {
+                            const int k = it * LG + j;
+                            const bool valid = k < c.n;
+                            const Raw& r = raw[c.first + (valid ? k : 0)];   // padding repeats a kept sample, weight 0
+                            GridEntry ge;
+                            ge.w0 = r.elem | (it == c.iters - 1 ? (1u << 29) : 0u) | (r.conj << 30) | (valid ? (1u << 31) : 0u);
+                            ge.w1 = r.ch | (r0.row << 12) | ((r0.col % kColsPerGroup) << 24);
+                            entries.push_back(ge);
+                        }
+                    iters += c.iters;
+                }
+                if (gend > gbeg)
+                    for (; iters % kTreeUnroll; iters++)
+                        for (int j = 0; j < LG; j++) entries.push_back(GridEntry{raw[gbeg].elem, raw[gbeg].ch});
+            }
+        }
+        warp_iter[gl.ngroups * kWarpsPerCta] = (int32_t)(entries.size() / LG);
+        gl.n_chunks = (int64_t)(entries.size() / LG);
+        int rc;
+        if ((rc = upload(&gl.entries, entries.data(), entries.size())) != RF_OK) return rc;
+        return upload(&gl.warp_chunk, warp_iter.data(), warp_iter.size());
+    };
     int rc = emit(p->d.gen, cols_per_group(N));
-    if (rc == RF_OK && p->tree_tb > 0) rc = emit(p->d.tree, tree_cols_per_group(N, p->tree_tb));
+    if (rc == RF_OK && p->tree_tb > 0) rc = emit_tree(p->d.tree, tree_cols_per_group(N, p->tree_tb), 32 / p->tree_tb);
     return rc;
 }
 

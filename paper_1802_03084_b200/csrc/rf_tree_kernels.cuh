@@ -29,7 +29,7 @@ struct TreeParams {
     const int32_t* warp_chunk;
     const BlockDesc* blocks;        // first block of this batch
     const float2* twiddles;
-    float2* Ht;                     // [n_blk][N][cpad][TB]
+    float2* Ht;                     // [n_blk][N][TB/2][cpad][2]
     float* sumsq;                   // [n_blk][2*TB-1][ngroups]
     int32_t* counters;
     rf_cand* cand_items;
@@ -92,6 +92,8 @@ __global__ void __launch_bounds__(kThreads) k_tree_grid_colfft(const TreeParams 
     constexpr int PITCH = fft_padded_size(N) + 1;
     constexpr int NF = TB * NCOL;
     constexpr int NIMG = 2 * TB - 1;
+    constexpr int LG = 32 / TB, U = kTreeUnroll;
+    constexpr int LEVELS = (TB == 8) ? 4 : (TB == 4 ? 3 : 2);      // log2(TB) + 1
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2* tile = reinterpret_cast<float2*>(smem_raw);
     float2* tw = tile + NF * PITCH;
@@ -102,78 +104,92 @@ __global__ void __launch_bounds__(kThreads) k_tree_grid_colfft(const TreeParams 
     const int slot = blockIdx.x, g = blockIdx.y;
     const BlockDesc blk = p.blocks[slot];
     const int t0 = blk.tb * TB;
+    const int j = lane / TB, q = lane % TB;
 
+    // ---- prologue: every global load of the set-up is issued before the tile is cleared
+    const int it_beg = p.warp_chunk[g * kWarpsPerCta + warp];
+    const int it_end = p.warp_chunk[g * kWarpsPerCta + warp + 1];
+    const int32_t* drow = p.delay + (size_t)blk.dm_idx * p.nchan;
+    const int d0 = tid < p.nchan ? drow[tid] : 0;
+    const int d1 = tid + kThreads < p.nchan ? drow[tid + kThreads] : 0;
+    const float2 tw0 = p.twiddles[tid < C::TW_TOTAL ? tid : 0];
+    const float2 tw1 = p.twiddles[tid + kThreads < C::TW_TOTAL ? tid + kThreads : 0];
+    GridEntry en[U];                       // entries of the next batch of iterations (prefetched)
+#pragma unroll
+    for (int u = 0; u < U; u++) en[u] = GridEntry{0u, 0u};
+    if (it_beg < it_end) {
+#pragma unroll
+        for (int u = 0; u < U; u++) en[u] = p.entries[(size_t)(it_beg + u) * LG + j];
+    }
     for (int i = tid; i < NF * PITCH; i += kThreads) tile[i] = make_float2(0.f, 0.f);
-    for (int i = tid; i < p.nchan; i += kThreads) sdelay[i] = p.delay[(size_t)blk.dm_idx * p.nchan + i];
-    load_twiddles<N>(tw, p.twiddles, tid, kThreads);
+    if (tid < p.nchan) sdelay[tid] = d0;
+    if (tid + kThreads < p.nchan) sdelay[tid + kThreads] = d1;
+    for (int i = tid + 2 * kThreads; i < p.nchan; i += kThreads) sdelay[i] = drow[i];
+    if (tid < C::TW_TOTAL) tw[tid] = tw0;
+    if (tid + kThreads < C::TW_TOTAL) tw[tid + kThreads] = tw1;
     __syncthreads();
 
-    // ---- gather TB consecutive dedispersed samples per entry, segmented grid add into TB tiles
+    // ---- gather + grid ("time in lanes"): lane = (entry j = lane / TB, integration q = lane % TB).
+    //      One iteration reads LG = 32/TB entries: the TB dedispersed samples of an entry are ONE
+    //      coalesced 8*TB-byte read.  A cell belongs to one warp; the lane accumulates over the cell's
+    //      iterations in a register, the END iteration sums the LG lane groups with xor shuffles and
+    //      group 0 stores the cell into the TB tiles (plain store: nobody else touches that cell).
+    //      Parseval sums of every boxcar-tree node, sum_cells w |sum_{q in node} G_q|^2, are taken
+    //      at the same place from the cell sums (another log2(TB) xor steps over q).
+    float ps[LEVELS];
+#pragma unroll
+    for (int l = 0; l < LEVELS; l++) ps[l] = 0.f;
     {
-        const int c_beg = p.warp_chunk[g * kWarpsPerCta + warp];
-        const int c_end = p.warp_chunk[g * kWarpsPerCta + warp + 1];
-        for (int ck = c_beg; ck < c_end; ck++) {
-            const GridEntry e = p.entries[(size_t)ck * 32 + lane];
-            const bool valid = (e.w0 >> 31) != 0;
-            float2 v[TB];
-            const float2* src = p.visI + (size_t)(e.w0 & 0xffffffu) * p.tpitch + (t0 + sdelay[e.w1 & 0xfff]);
+        const float2* vbase = p.visI + t0 + q;
+        float2 acc = make_float2(0.f, 0.f);
+#ifdef RF_EXP_NOGATHER
+        if (p.nchan < 0)
+#endif
+        for (int it = it_beg; it < it_end; it += U) {
+            GridEntry e[U];
+            float2 x[U];
 #pragma unroll
-            for (int q = 0; q < TB; q++) v[q] = valid ? __ldg(src + q) : make_float2(0.f, 0.f);
-            if (e.w0 & (1u << 30)) {
+            for (int u = 0; u < U; u++) e[u] = en[u];
 #pragma unroll
-                for (int q = 0; q < TB; q++) v[q].y = -v[q].y;
+            for (int u = 0; u < U; u++)
+                x[u] = __ldg(vbase + (size_t)(e[u].w0 & 0xffffffu) * p.tpitch + sdelay[e[u].w1 & 0xfff]);
+            if (it + U < it_end) {
+#pragma unroll
+                for (int u = 0; u < U; u++) en[u] = p.entries[(size_t)(it + U + u) * LG + j];
             }
-            const int dist = (e.w0 >> 24) & 31;
 #pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
+            for (int u = 0; u < U; u++) {
+                const float wr = (e[u].w0 >> 31) ? 1.f : 0.f;                 // padding: weight 0
+                const float wi = (e[u].w0 & (1u << 30)) ? -wr : wr;           // conjugate
+                acc.x = fmaf(wr, x[u].x, acc.x);
+                acc.y = fmaf(wi, x[u].y, acc.y);
+                if (e[u].w0 & (1u << 29)) {                                   // warp-uniform: cell complete
 #pragma unroll
-                for (int q = 0; q < TB; q++) {
-                    const float r2 = __shfl_up_sync(0xffffffffu, v[q].x, d);
-                    const float i2 = __shfl_up_sync(0xffffffffu, v[q].y, d);
-                    if (dist >= d) { v[q].x += r2; v[q].y += i2; }
+                    for (int d = TB; d < 32; d <<= 1) {
+                        acc.x += __shfl_xor_sync(0xffffffffu, acc.x, d);
+                        acc.y += __shfl_xor_sync(0xffffffffu, acc.y, d);
+                    }
+                    const int row = (e[u].w1 >> 12) & 0xfff, col = (e[u].w1 >> 24) & 0xf;
+                    if (j == 0) tile[(q * NCOL + col) * PITCH + fft_pad(row)] = acc;
+                    const int gc = g * NCOL + col;
+                    const float wgt = (gc == 0 || gc == N / 2) ? 1.f : 2.f;
+                    ps[0] = fmaf(wgt, acc.x * acc.x + acc.y * acc.y, ps[0]);
+#pragma unroll
+                    for (int l = 1; l < LEVELS; l++) {
+                        acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 1 << (l - 1));
+                        acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 1 << (l - 1));
+                        ps[l] = fmaf(wgt, acc.x * acc.x + acc.y * acc.y, ps[l]);
+                    }
+                    acc = make_float2(0.f, 0.f);
                 }
             }
-            if (valid && (e.w0 & (1u << 29))) {
-                const int row = (e.w1 >> 12) & 0xfff, col = (e.w1 >> 24) & 0xf;
-                float2* dst = &tile[col * PITCH + fft_pad(row)];
-#pragma unroll
-                for (int q = 0; q < TB; q++) {
-                    float2 cur = dst[q * NCOL * PITCH];
-                    dst[q * NCOL * PITCH] = make_float2(cur.x + v[q].x, cur.y + v[q].y);
-                }
-            }
-            __syncwarp();
         }
     }
-    __syncthreads();
-
-    // ---- Parseval sums of every tree node: sum_cells w |sum_{q in node} G_q|^2
-    {
-        float acc[NIMG];
+    // node (level l, i) is held by the lanes of group 0 with q >> l == i (all of them hold the same sum)
+    if (j == 0) {
 #pragma unroll
-        for (int i = 0; i < NIMG; i++) acc[i] = 0.f;
-        for (int idx = tid; idx < NCOL * N; idx += kThreads) {
-            const int c = idx / N, y = idx % N;
-            const int gc = g * NCOL + c;
-            const float wgt = (gc == 0 || gc == N / 2) ? 1.f : 2.f;
-            float2 s[TB];
-#pragma unroll
-            for (int q = 0; q < TB; q++) s[q] = tile[(q * NCOL + c) * PITCH + fft_pad(y)];
-            int off = 0;
-#pragma unroll
-            for (int cnt = TB; cnt >= 1; cnt >>= 1) {
-#pragma unroll
-                for (int i = 0; i < cnt; i++) acc[off + i] += wgt * (s[i].x * s[i].x + s[i].y * s[i].y);
-                off += cnt;
-#pragma unroll
-                for (int i = 0; i < cnt / 2; i++) s[i] = cadd(s[2 * i], s[2 * i + 1]);
-            }
-        }
-#pragma unroll
-        for (int i = 0; i < NIMG; i++) {
-            const float w = warp_sum(acc[i]);
-            if (lane == 0) red[warp * NIMG + i] = w;
-        }
+        for (int l = 0; l < LEVELS; l++)
+            if ((q & ((1 << l) - 1)) == 0) red[warp * NIMG + tree_off(TB, l) + (q >> l)] = ps[l];
     }
     __syncthreads();
     if (tid < NIMG) {
@@ -193,20 +209,24 @@ __global__ void __launch_bounds__(kThreads) k_tree_grid_colfft(const TreeParams 
             fft_reload<N>(v, col, t);
             fft_inverse<N>(v, col, tw, t, 1 + grp);
             fft_group_sync<C::TPF>(1 + grp);
-#pragma unroll
-            for (int e = 0; e < 16; e++)
-                col[fft_pad(t + C::TPF * e)] = make_float2(v[e].x * p.norm, v[e].y * p.norm);
+            fft_unload<N>(v, col, t, p.norm);
         }
     }
     __syncthreads();
 
-    // ---- store H[slot][y][g*NCOL + c][q]: NCOL*TB*8 contiguous bytes per row
+    // ---- store H[slot][y][pair][g*NCOL + c][q & 1] (pair = q / 2): the two integrations that share
+    //      one Hermitian pair transform are adjacent (one 16-byte store), and one (row, pair) is
+    //      contiguous for pass 2
     {
-        constexpr int SEG = NCOL * TB;
-        float2* Hs = p.Ht + ((size_t)slot * N * p.cpad + g * NCOL) * TB;
-        const int i = tid % SEG, c = i / TB, q = i % TB, y0 = tid / SEG;
-        for (int y = y0; y < N; y += kThreads / SEG)
-            Hs[((size_t)y * p.cpad + c) * TB + q] = tile[(q * NCOL + c) * PITCH + fft_pad(y)];
+        constexpr int SEG = NCOL * TB / 2;
+        float4* Hs = reinterpret_cast<float4*>(p.Ht + (size_t)slot * N * p.cpad * TB);
+        const int i = tid % SEG, pr = i / NCOL, c = i % NCOL, y0 = tid / SEG;
+        const float2* ta = tile + (2 * pr * NCOL + c) * PITCH;
+        const float2* tb = ta + NCOL * PITCH;
+        for (int y = y0; y < N; y += kThreads / SEG) {
+            const float2 a = ta[fft_pad(y)], b = tb[fft_pad(y)];
+            Hs[((size_t)y * (TB / 2) + pr) * p.cpad + g * NCOL + c] = make_float4(a.x, a.y, b.x, b.y);
+        }
     }
 }
 
@@ -234,18 +254,23 @@ __device__ __forceinline__ void tree_row_stats(const float (&x)[16], int img, in
     const float A = cx.sA[img];
     uint32_t* hw = cx.hist + (img >> 1) * cx.nbins;
     const uint32_t inc = (img & 1) ? 65536u : 1u;
-    const int nbm1 = cx.nbins - 1;
+    const unsigned nbm1 = (unsigned)cx.nbins - 1u;
     float m = x[0];
 #pragma unroll
     for (int e = 0; e < 16; e++) {
-        int bin = __float2int_rd(fmaf(x[e], A, cx.B));
-        atomicAdd(hw + min(max(bin, 0), nbm1), inc);
+        // cvt.rmi.u32.f32 saturates: negative (and NaN) -> bin 0; one min clamps the top
+        const unsigned bin = __float2uint_rd(fmaf(x[e], A, cx.B));
+#ifdef RF_EXP_NOHIST
+        if (bin == 12345678u)
+#endif
+        atomicAdd(hw + min(bin, nbm1), inc);
         m = fmaxf(m, x[e]);
     }
-    float wm = m;
+    // running peak of this warp: a new maximum is rare after the first rows, so one vote decides
+    if (__any_sync(0xffffffffu, m > cx.sBest[warp * cx.nimg + img])) {
+        float wm = m;
 #pragma unroll
-    for (int d = 16; d > 0; d >>= 1) wm = fmaxf(wm, __shfl_xor_sync(0xffffffffu, wm, d));
-    if (wm > cx.sBest[warp * cx.nimg + img]) {          // warp-uniform
+        for (int d = 16; d > 0; d >>= 1) wm = fmaxf(wm, __shfl_xor_sync(0xffffffffu, wm, d));
         int xp = 0x7fffffff;
         if (m == wm) {
 #pragma unroll
@@ -326,7 +351,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_tree_rowfft_stats(const TreePar
                 const int c = t + C::TPF * e;
                 const int cc = (e < 8) ? c : N - c;
                 float4 h = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (cc < p.ncol) h = *reinterpret_cast<const float4*>(row + (size_t)cc * TB + 2 * p2);
+                if (cc < p.ncol) h = *reinterpret_cast<const float4*>(row + ((size_t)p2 * p.cpad + cc) * 2);
                 if (cc == 0 || cc == N / 2) v[e] = make_float2(h.x, h.z);
                 else if (e < 8) v[e] = make_float2(h.x - h.w, h.y + h.z);
                 else v[e] = make_float2(h.x + h.w, h.z - h.y);
