@@ -294,10 +294,166 @@ def run_ours(args, cfg):
     plan.destroy()
 
 
+def _stream_host_rows(cfg, nseg, torch):
+    """Pinned host copy of the new integrations of every segment: segment 0 in full, then the
+    cfg.stride_int integrations each later segment adds (rows [overlap, nint) of that segment)."""
+    from concurrent.futures import ThreadPoolExecutor
+    overlap = cfg.nint - cfg.stride_int
+    row_shape = (cfg.nbl, cfg.nchan, cfg.npol)
+    first = torch.empty((cfg.nint,) + row_shape, dtype=torch.complex64).pin_memory()
+    new = torch.empty((max(1, nseg - 1), cfg.stride_int) + row_shape, dtype=torch.complex64).pin_memory()
+    jobs = [(0, lo, min(lo + 64, cfg.nint), first.numpy()[lo:min(lo + 64, cfg.nint)]) for lo in range(0, cfg.nint, 64)]
+    for s in range(1, nseg):
+        for lo in range(overlap, cfg.nint, 80):
+            hi = min(lo + 80, cfg.nint)
+            jobs.append((s, lo, hi, new.numpy()[s - 1, lo - overlap:hi - overlap]))
+    with ThreadPoolExecutor(max(1, min(32, len(os.sched_getaffinity(0))))) as ex:
+        list(ex.map(lambda j: W.make_segment(cfg, j[0], rows=(j[1], j[2]), out=j[3]), jobs))
+    return first, new
+
+
+def run_stream(args, cfg):
+    """BASELINE.json configs[4]: consecutive overlapping segments.  Each segment keeps the last
+    `overlap` integrations of the previous one on the device (device-to-device copy) and uploads only
+    its cfg.stride_int new integrations from pinned host memory on a side stream while the previous
+    segment is searched; uvw (hour angle) changes per segment, so two plans are used alternately and
+    the tables of the next segment are rebuilt on the host while the GPU searches the current one."""
+    import torch
+
+    import paper_1802_03084_b200 as R
+    from workloads.generate import segment_ha_hours
+
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        raise SystemExit("--config stream is a single-GPU measurement (replicas: run one per GPU)")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    nseg_cfg = cfg.n_segments
+    n_warm, n_timed = args.warmup, args.steps
+    n_total = n_warm + n_timed
+    f, dms = W.channel_freqs_hz(cfg), W.dm_list(cfg)
+    geo = []
+    for s in range(nseg_cfg):
+        uvw = W.baseline_uvw_m(cfg, segment_ha_hours(cfg, s))
+        geo.append((uvw, W.default_cell_rad(cfg, uvw)))
+    first, new = _stream_host_rows(cfg, min(n_total, nseg_cfg), torch)
+    overlap = cfg.nint - cfg.stride_int
+
+    main, side = torch.cuda.Stream(dev), torch.cuda.Stream(dev)
+    capacity = 1 << 17
+    plans, bufs, items, counts, h_items, h_counts = [], [], [], [], [], []
+    for b in range(2):
+        pl = R.Plan(f, geo[0][0], cfg.npol, cfg.nint, cfg.inttime_s, cfg.npix, geo[0][1], dms, cfg.dt_list, cfg.threshold)
+        pl.set_search_span(cfg.stride_int)
+        plans.append(pl)
+        bufs.append(torch.empty((cfg.nint, cfg.nbl, cfg.nchan, cfg.npol), dtype=torch.complex64, device=dev))
+        items.append(torch.empty(capacity * 32, dtype=torch.uint8, device=dev))
+        counts.append(torch.zeros(1, dtype=torch.int32, device=dev))
+        h_items.append(torch.empty(capacity * 32, dtype=torch.uint8).pin_memory())
+        h_counts.append(torch.zeros(1, dtype=torch.int32).pin_memory())
+    images = plans[0].num_images()
+    staged = [torch.cuda.Event() for _ in range(2)]
+    searched = [torch.cuda.Event() for _ in range(2)]
+    for e in searched:
+        e.record(main)
+
+    def stage(k):
+        """Enqueue, on the side stream, everything that fills the device buffer of the k-th segment."""
+        b, s = k % 2, k % nseg_cfg
+        side.wait_event(searched[b])                       # the search that last read this buffer
+        with torch.cuda.stream(side):
+            if s == 0:
+                bufs[b].copy_(first, non_blocking=True)
+            else:
+                side.wait_event(staged[1 - b])
+                bufs[b][:overlap].copy_(bufs[1 - b][cfg.stride_int:], non_blocking=True)
+                bufs[b][overlap:].copy_(new[s - 1], non_blocking=True)
+            staged[b].record(side)
+
+    def search(k):
+        b, s = k % 2, k % nseg_cfg
+        searched[b].synchronize()                          # plan b is idle: its tables may be rebuilt
+        if k >= 2:
+            found[0] += min(int(h_counts[b][0]), capacity)   # the host reads the result of segment k - 2
+        plans[b].set_uvw(*geo[s])
+        main.wait_event(staged[b])
+        plans[b].search_raw(bufs[b].data_ptr(), main.cuda_stream, items[b].data_ptr(), capacity, counts[b].data_ptr())
+        with torch.cuda.stream(main):
+            h_counts[b].copy_(counts[b], non_blocking=True)
+            h_items[b].copy_(items[b], non_blocking=True)
+        searched[b].record(main)
+
+    sampler, found = None, [0]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = 0.0
+    stage(0)
+    for k in range(n_total):
+        if k == n_warm:
+            torch.cuda.synchronize(dev)
+            sampler = ClockSampler(0)
+            sampler.start()
+            t0 = time.perf_counter()
+            e0.record(main)
+        search(k)
+        # staged AFTER the table rebuild of search(k): the upload of segment k + 1 waits (on the device)
+        # for search k - 1, and copies queued behind a waiting copy would stall the rebuild's own uploads
+        if k + 1 < n_total:
+            stage(k + 1)
+    e1.record(main)
+    torch.cuda.synchronize(dev)
+    wall_ms = (time.perf_counter() - t0) * 1e3
+    dev_ms = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    n_last = int(h_counts[(n_total - 1) % 2].item())
+
+    # per-kernel times of one more search of the last segment (profiling events on)
+    b = (n_total - 1) % 2
+    plans[b].set_profiling(True)
+    plans[b].search_raw(bufs[b].data_ptr(), main.cuda_stream, items[b].data_ptr(), capacity, counts[b].data_ptr())
+    main.synchronize()
+    k_ms, k_n = plans[b].get_kernel_times()
+    launches = plans[b].get_counters()["kernel_launches"]
+    alg = _alg_bytes(cfg, plans[b])
+    peak, peak_src = _peaks()
+    dom = 0 if k_ms[0] >= k_ms[1] else 1
+    per_launch_bytes = alg["pass1" if dom == 0 else "pass2"] / max(1, k_n[dom])
+    achieved = per_launch_bytes / (k_ms[dom] / max(1, k_n[dom]) * 1e-3) / 1e9
+    ms_per_step = dev_ms / n_timed
+    data_s = cfg.stride_int * cfg.inttime_s
+    new_bytes = cfg.stride_int * cfg.nbl * cfg.nchan * cfg.npol * 8
+    path_gbs = alg["total"] / (ms_per_step * 1e-3) / 1e9
+    line = {
+        "metric": METRIC, "value": images / (ms_per_step * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": n_timed,
+        "warmup": n_warm, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"stream: BASELINE.json configs[4] ({cfg.nant} antennas, {cfg.nchan} ch, segments of "
+                               f"{cfg.nint} x {cfg.inttime_s * 1e3:g} ms with stride {cfg.stride_int}, {cfg.ndm} DM x dt "
+                               f"{list(cfg.dt_list)}, npix {cfg.npix}); a step = one segment, pipelined",
+                   "images_per_step": images, "realtime_factor": data_s / (ms_per_step * 1e-3),
+                   "realtime_factor_wall": data_s * n_timed / (wall_ms * 1e-3),
+                   "data_seconds_per_step": data_s, "candidates_last_segment": n_last, "candidates_read_on_host": found[0],
+                   "gvis_per_s": alg["vis_gridded"] / (ms_per_step * 1e-3) / 1e9,
+                   "l2_policy": "each segment's 1.47 GB buffer is larger than L2 (126 MB); no flush",
+                   "overlap": "H2D of the next segment's new integrations on a side stream; table rebuild on the host",
+                   "parallelism": "single GPU"},
+        "clocks": clocks,
+        "e2e": {"value": images * n_timed / (wall_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(new_bytes),
+                "d2h_bytes_per_step": int(4 + capacity * 32)},
+        "gpu_launches": int(launches) * n_timed,
+        "roofline": {"bound": "hbm", "kernel": ["grid + column FFT kernels", "row FFT + statistics kernels"][dom],
+                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                     "peak_source": peak_src, "alg_bytes_per_launch": per_launch_bytes,
+                     "kernel_ms_per_step": {"pass1": k_ms[0], "pass2": k_ms[1], "prep": k_ms[2]},
+                     "path": {"alg_bytes_per_step": alg["total"], "achieved": path_gbs, "frac": path_gbs / peak}},
+    }
+    print(json.dumps(line), flush=True)
+    for pl in plans:
+        pl.destroy()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=None, help="timed steps (default 5; 32 segments for --config stream)")
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="lband", choices=sorted(W.CONFIGS))
@@ -306,8 +462,12 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     cfg = W.get_config(args.config)
+    if args.steps is None:
+        args.steps = cfg.n_segments if cfg.n_segments > 1 else 5
     if args.impl == "reference":
         run_reference(args, cfg)
+    elif cfg.n_segments > 1:
+        run_stream(args, cfg)
     else:
         run_ours(args, cfg)
 

@@ -34,7 +34,8 @@ int rebuild_geometry(rf_plan* p) {
 void free_tables(rf_plan* p) {
     rf::DeviceTables& d = p->d;
     cudaFree(d.delay); cudaFree(d.cell); cudaFree(d.keep); cudaFree(d.gen.entries); cudaFree(d.gen.warp_chunk);
-    cudaFree(d.tree.entries); cudaFree(d.tree.warp_chunk); cudaFree(d.blocks); cudaFree(d.images); cudaFree(d.freqs); cudaFree(d.uvw); cudaFree(d.dms); cudaFree(d.twiddles);
+    cudaFree(d.tree.entries); cudaFree(d.tree.warp_chunk); cudaFree(d.blocks); cudaFree(d.images); cudaFree(d.freqs); cudaFree(d.uvw); cudaFree(d.dms); cudaFree(d.weights); cudaFree(d.twiddles);
+    p->dev_cap.clear();
     d = rf::DeviceTables{};
 }
 
@@ -73,6 +74,11 @@ int rf_plan_create(rf_plan** out, const double* freqs_hz, int nchan, const doubl
     p->weights.assign(nchan, 1.0f);
     p->nbins = 2048;
     rf::configure_tree(p);
+    if (cudaStreamCreateWithFlags(&p->tab_stream, cudaStreamNonBlocking) != cudaSuccess) {
+        set_error("cudaStreamCreate failed: %s", cudaGetErrorString(cudaGetLastError()));
+        delete p;
+        return RF_ERR_CUDA;
+    }
     int rc = rf::build_delay_table(p);
     if (rc == RF_OK) rc = rebuild_geometry(p);
     if (rc != RF_OK) { rf_plan_destroy(p); return rc; }
@@ -85,6 +91,7 @@ int rf_plan_destroy(rf_plan* p) {
     for (cudaEvent_t e : p->events) cudaEventDestroy(e);
     cudaFree(p->stage_vis); cudaFree(p->stage_cand); cudaFree(p->stage_count);
     if (p->own_stream) cudaStreamDestroy(p->own_stream);
+    if (p->tab_stream) cudaStreamDestroy(p->tab_stream);
     rf::free_workspace(p);
     free_tables(p);
     delete p;

@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <map>
 #include <string>
 #include <vector>
 
@@ -73,6 +74,7 @@ struct DeviceTables {
     double* freqs = nullptr;         // [nchan] Hz
     double* uvw = nullptr;           // [nbl][3]
     double* dms = nullptr;           // [ndm]
+    float* weights = nullptr;        // [nchan]
     float2* twiddles = nullptr;      // [16 + 256] FFT stage twiddles
 };
 
@@ -138,6 +140,8 @@ struct rf_plan {
     std::vector<int> event_kind;
     int n_events_used = 0;
     rf::DeviceTables d;
+    std::map<void*, size_t> dev_cap;   // capacity in bytes of each table pointer (rf_tables.cu)
+    cudaStream_t tab_stream = nullptr; // plan-time kernels and table copies (non-blocking)
     rf::Workspace ws;
 };
 

@@ -52,15 +52,30 @@ __global__ void k_cell_table(const double* __restrict__ uvw, const double* __res
     keep[i] = ok ? 1 : 0;
 }
 
-template <class T> int upload(T** dst, const T* src, size_t n) {
-    if (*dst) { cudaFree(*dst); *dst = nullptr; }
+// Device buffers are kept between rebuilds (capacity per pointer variable) and all plan-time
+// work runs on the plan's own non-blocking stream, so rf_plan_set_uvw neither frees memory nor
+// touches the legacy default stream: a rebuild does not synchronise with searches of OTHER plans
+// that are in flight (streaming, config 5: two plans used alternately).
+template <class T> int reserve(rf_plan* p, T** dst, size_t n) {
+    size_t& cap = p->dev_cap[(void*)dst];
+    const size_t bytes = n * sizeof(T);
+    if (*dst && bytes <= cap) return RF_OK;
+    if (*dst) { cudaFree(*dst); *dst = nullptr; cap = 0; }
     if (n == 0) return RF_OK;
-    if (cudaMalloc((void**)dst, n * sizeof(T)) != cudaSuccess) {
+    const size_t want = bytes + bytes / 4 + 256;
+    if (cudaMalloc((void**)dst, want) != cudaSuccess) {
         cudaGetLastError();
-        set_error("device allocation of %zu bytes failed", n * sizeof(T));
+        set_error("device allocation of %zu bytes failed", want);
         return RF_ERR_NOMEM;
     }
-    RF_CUDA_CHECK(cudaMemcpy(*dst, src, n * sizeof(T), cudaMemcpyHostToDevice));
+    cap = want;
+    return RF_OK;
+}
+template <class T> int upload(rf_plan* p, T** dst, const T* src, size_t n) {
+    int rc = reserve(p, dst, n);
+    if (rc != RF_OK || n == 0) return rc;
+    // pageable source: returns once the data is staged, so `src` may be freed by the caller
+    RF_CUDA_CHECK(cudaMemcpyAsync(*dst, src, n * sizeof(T), cudaMemcpyHostToDevice, p->tab_stream));
     return RF_OK;
 }
 
@@ -68,17 +83,17 @@ template <class T> int upload(T** dst, const T* src, size_t n) {
 
 int build_delay_table(rf_plan* p) {
     int rc;
-    if ((rc = upload(&p->d.freqs, p->freqs.data(), p->freqs.size())) != RF_OK) return rc;
-    if ((rc = upload(&p->d.dms, p->dms.data(), p->dms.size())) != RF_OK) return rc;
+    if ((rc = upload(p, &p->d.freqs, p->freqs.data(), p->freqs.size())) != RF_OK) return rc;
+    if ((rc = upload(p, &p->d.dms, p->dms.data(), p->dms.size())) != RF_OK) return rc;
     size_t n = (size_t)p->ndm * p->nchan;
-    if (p->d.delay) { cudaFree(p->d.delay); p->d.delay = nullptr; }
-    RF_CUDA_CHECK(cudaMalloc((void**)&p->d.delay, n * sizeof(int32_t)));
+    if ((rc = reserve(p, &p->d.delay, n)) != RF_OK) return rc;
     double fmax = *std::max_element(p->freqs.begin(), p->freqs.end()) / 1e9;
-    k_delay_table<<<(unsigned)((n + 255) / 256), 256>>>(p->d.freqs, p->d.dms, p->nchan, p->ndm, fmax,
+    k_delay_table<<<(unsigned)((n + 255) / 256), 256, 0, p->tab_stream>>>(p->d.freqs, p->d.dms, p->nchan, p->ndm, fmax,
                                                         p->inttime, p->d.delay);
     RF_CUDA_CHECK(cudaGetLastError());
     p->h_delay.resize(n);
-    RF_CUDA_CHECK(cudaMemcpy(p->h_delay.data(), p->d.delay, n * sizeof(int32_t), cudaMemcpyDeviceToHost));
+    RF_CUDA_CHECK(cudaMemcpyAsync(p->h_delay.data(), p->d.delay, n * sizeof(int32_t), cudaMemcpyDeviceToHost, p->tab_stream));
+    RF_CUDA_CHECK(cudaStreamSynchronize(p->tab_stream));
     p->h_maxdelay.assign(p->ndm, 0);
     for (int d = 0; d < p->ndm; d++)
         for (int c = 0; c < p->nchan; c++)
@@ -88,23 +103,20 @@ int build_delay_table(rf_plan* p) {
 
 int build_cell_table(rf_plan* p) {
     int rc;
-    if ((rc = upload(&p->d.uvw, p->uvw.data(), p->uvw.size())) != RF_OK) return rc;
-    float* d_w = nullptr;
-    if ((rc = upload(&d_w, p->weights.data(), p->weights.size())) != RF_OK) return rc;
+    if ((rc = upload(p, &p->d.uvw, p->uvw.data(), p->uvw.size())) != RF_OK) return rc;
+    if ((rc = upload(p, &p->d.weights, p->weights.data(), p->weights.size())) != RF_OK) return rc;
     size_t n = (size_t)p->nbl * p->nchan;
-    if (p->d.cell) { cudaFree(p->d.cell); p->d.cell = nullptr; }
-    if (p->d.keep) { cudaFree(p->d.keep); p->d.keep = nullptr; }
-    RF_CUDA_CHECK(cudaMalloc((void**)&p->d.cell, 2 * n * sizeof(int32_t)));
-    RF_CUDA_CHECK(cudaMalloc((void**)&p->d.keep, n));
+    if ((rc = reserve(p, &p->d.cell, 2 * n)) != RF_OK) return rc;
+    if ((rc = reserve(p, &p->d.keep, n)) != RF_OK) return rc;
     double du = 1.0 / (p->npix * p->cell);
-    k_cell_table<<<(unsigned)((n + 255) / 256), 256>>>(p->d.uvw, p->d.freqs, d_w, p->nbl, p->nchan,
+    k_cell_table<<<(unsigned)((n + 255) / 256), 256, 0, p->tab_stream>>>(p->d.uvw, p->d.freqs, p->d.weights, p->nbl, p->nchan,
                                                        p->npix, du, p->d.cell, p->d.keep);
     RF_CUDA_CHECK(cudaGetLastError());
     p->h_cell.resize(2 * n);
     p->h_keep.resize(n);
-    RF_CUDA_CHECK(cudaMemcpy(p->h_cell.data(), p->d.cell, 2 * n * sizeof(int32_t), cudaMemcpyDeviceToHost));
-    RF_CUDA_CHECK(cudaMemcpy(p->h_keep.data(), p->d.keep, n, cudaMemcpyDeviceToHost));
-    cudaFree(d_w);
+    RF_CUDA_CHECK(cudaMemcpyAsync(p->h_cell.data(), p->d.cell, 2 * n * sizeof(int32_t), cudaMemcpyDeviceToHost, p->tab_stream));
+    RF_CUDA_CHECK(cudaMemcpyAsync(p->h_keep.data(), p->d.keep, n, cudaMemcpyDeviceToHost, p->tab_stream));
+    RF_CUDA_CHECK(cudaStreamSynchronize(p->tab_stream));
     p->n_kept = 0;
     for (size_t i = 0; i < n; i++) p->n_kept += p->h_keep[i];
     p->n_dropped = (int)n - p->n_kept;
@@ -184,8 +196,8 @@ int build_grid_lists(rf_plan* p) {
         warp_chunk[gl.ngroups * kWarpsPerCta] = (int32_t)(entries.size() / 32);
         gl.n_chunks = (int64_t)entries.size() / 32;
         int rc;
-        if ((rc = upload(&gl.entries, entries.data(), entries.size())) != RF_OK) return rc;
-        return upload(&gl.warp_chunk, warp_chunk.data(), warp_chunk.size());
+        if ((rc = upload(p, &gl.entries, entries.data(), entries.size())) != RF_OK) return rc;
+        return upload(p, &gl.warp_chunk, warp_chunk.data(), warp_chunk.size());
     };
     // Tree path ("time in lanes"): a warp reads LG = 32/TB entries per iteration, lane = (entry j,
     // integration q), so the TB consecutive samples of an entry are one coalesced 8*TB-byte read.
@@ -254,11 +266,12 @@ int build_grid_lists(rf_plan* p) {
         warp_iter[gl.ngroups * kWarpsPerCta] = (int32_t)(entries.size() / LG);
         gl.n_chunks = (int64_t)(entries.size() / LG);
         int rc;
-        if ((rc = upload(&gl.entries, entries.data(), entries.size())) != RF_OK) return rc;
-        return upload(&gl.warp_chunk, warp_iter.data(), warp_iter.size());
+        if ((rc = upload(p, &gl.entries, entries.data(), entries.size())) != RF_OK) return rc;
+        return upload(p, &gl.warp_chunk, warp_iter.data(), warp_iter.size());
     };
     int rc = emit(p->d.gen, cols_per_group(N));
     if (rc == RF_OK && p->tree_tb > 0) rc = emit_tree(p->d.tree, tree_cols_per_group(N, p->tree_tb), 32 / p->tree_tb);
+    if (rc == RF_OK) RF_CUDA_CHECK(cudaStreamSynchronize(p->tab_stream));
     return rc;
 }
 
@@ -319,8 +332,9 @@ int build_image_list(rf_plan* p) {
     }
     p->n_gen_images = (int64_t)imgs.size();
     p->n_blocks = (int64_t)blocks.size();
-    int rc = upload(&p->d.images, imgs.data(), imgs.size());
-    if (rc == RF_OK) rc = upload(&p->d.blocks, blocks.data(), blocks.size());
+    int rc = upload(p, &p->d.images, imgs.data(), imgs.size());
+    if (rc == RF_OK) rc = upload(p, &p->d.blocks, blocks.data(), blocks.size());
+    if (rc == RF_OK) RF_CUDA_CHECK(cudaStreamSynchronize(p->tab_stream));
     return rc;
 }
 

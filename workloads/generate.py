@@ -18,7 +18,7 @@ Everything here is INPUT construction.  The recipe:
 from __future__ import annotations
 
 from dataclasses import dataclass
-from typing import List, Sequence
+from typing import List, Sequence, Tuple
 
 import numpy as np
 
@@ -137,9 +137,10 @@ def transients(cfg: Config) -> List[Transient]:
     return out
 
 
-def noise_rows(cfg: Config, t_abs: Sequence[int]) -> np.ndarray:
+def noise_rows(cfg: Config, t_abs: Sequence[int], out: np.ndarray | None = None) -> np.ndarray:
     """complex64 [len(t_abs)][nbl][nchan][npol]; row t depends on (seed, t) only."""
-    out = np.empty((len(t_abs), cfg.nbl, cfg.nchan, cfg.npol), dtype=np.complex64)
+    if out is None:
+        out = np.empty((len(t_abs), cfg.nbl, cfg.nchan, cfg.npol), dtype=np.complex64)
     flat = out.view(np.float32).reshape(len(t_abs), -1)
     for k, t in enumerate(t_abs):
         rng = np.random.Generator(
@@ -151,18 +152,25 @@ def noise_rows(cfg: Config, t_abs: Sequence[int]) -> np.ndarray:
 def make_segment(cfg: Config, segment: int = 0, *, noise: bool = True,
                  inject: bool = True, uvw_m: np.ndarray | None = None,
                  cell_rad: float | None = None,
-                 sources: Sequence[Transient] | None = None) -> np.ndarray:
+                 sources: Sequence[Transient] | None = None,
+                 rows: Tuple[int, int] | None = None, out: np.ndarray | None = None) -> np.ndarray:
     """Visibilities of one segment: complex64 [nint][nbl][nchan][npol].
 
     Segment ``s`` of a streaming config covers absolute integrations
     [s*stride, s*stride + nint).  ``sources`` overrides the seeded transients.
+    ``rows = (lo, hi)`` returns only the segment-relative integrations [lo, hi)
+    (the same values ``make_segment(...)[lo:hi]`` would hold); ``out`` receives them in place.
     """
+    lo, hi = (0, cfg.nint) if rows is None else rows
     t_first = segment * cfg.stride_int
-    t_abs = np.arange(t_first, t_first + cfg.nint)
+    t_abs = np.arange(t_first + lo, t_first + hi)
+    shape = (hi - lo, cfg.nbl, cfg.nchan, cfg.npol)
+    vis = np.empty(shape, dtype=np.complex64) if out is None else out
+    assert vis.shape == shape and vis.dtype == np.complex64
     if noise:
-        vis = noise_rows(cfg, t_abs)
+        noise_rows(cfg, t_abs, out=vis)
     else:
-        vis = np.zeros((cfg.nint, cfg.nbl, cfg.nchan, cfg.npol), dtype=np.complex64)
+        vis[...] = 0
     if not inject:
         return vis
     uvw = baseline_uvw_m(cfg, segment_ha_hours(cfg, segment)) if uvw_m is None else uvw_m
@@ -177,9 +185,9 @@ def make_segment(cfg: Config, segment: int = 0, *, noise: bool = True,
         for q in range(src.width):
             t_ch = src.t0 + q + sweep - t_first           # per channel, segment-relative
             for t in np.unique(t_ch):
-                if 0 <= t < cfg.nint:
+                if lo <= t < hi:
                     ch = np.nonzero(t_ch == t)[0]
-                    vis[t][:, ch, :] += sig[:, ch, None]
+                    vis[t - lo][:, ch, :] += sig[:, ch, None]
     return vis
 
 
