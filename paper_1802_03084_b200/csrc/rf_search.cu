@@ -107,11 +107,12 @@ template <int N, int TB> size_t smem_tree1(int nchan, int ncol) {
     return (size_t)TB * ncol * (fft_padded_size(N) + 1) * sizeof(float2) + FftCfg<N>::TW_TOTAL * sizeof(float2) +
            (size_t)nchan * sizeof(int) + (size_t)kWarpsPerCta * (2 * TB - 1) * sizeof(float);
 }
-template <int N, int TB> size_t smem_tree2(int nbins) {
-    const size_t xb = (size_t)(kThreads / FftCfg<N>::TPF) * fft_padded_size(N) * sizeof(float2);
+template <int N, int TB> size_t smem_tree2(int nbins, int cpad) {
+    const size_t g2 = kThreads2 / FftCfg<N>::TPF;
+    const size_t xb = g2 * fft_padded_size(N) * sizeof(float2);
     const size_t fin = (size_t)2 * nbins * sizeof(uint32_t);
-    return std::max(xb, fin) + FftCfg<N>::TW_TOTAL * sizeof(float2) + (size_t)TB * nbins * sizeof(uint32_t) +
-           64 * 4 + (size_t)2 * kWarpsPerCta * (2 * TB - 1) * 4;
+    return std::max(xb, fin) + FftCfg<N>::TW_TOTAL * sizeof(float2) + g2 * cpad * sizeof(float4) +
+           (size_t)((2 * TB) / 2) * nbins * sizeof(uint32_t) + 64 * 4 + (size_t)2 * kWarps2 * (2 * TB - 1) * 4;
 }
 
 template <int N, int TB, int NCOL>
@@ -132,13 +133,13 @@ int launch_tree(rf_plan* p, const TreeParams& tp, cudaStream_t st) {
     }
     {
         auto kern = k_tree_rowfft_stats<N, TB>;
-        const size_t smem = smem_tree2<N, TB>(tp.nbins);
+        const size_t smem = smem_tree2<N, TB>(tp.nbins, tp.cpad);
         static size_t configured = 0;
         if (smem > configured) {
             RF_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             configured = smem;
         }
-        kern<<<dim3(tp.n_blk), kThreads, smem, st>>>(tp);
+        kern<<<dim3(tp.n_blk), kThreads2, smem, st>>>(tp);
         RF_CUDA_CHECK(cudaGetLastError());
         if ((rc = mark(p, st, 1)) != RF_OK) return rc;
     }
@@ -209,8 +210,13 @@ int ensure_tree_workspace(rf_plan* p) {
     const size_t h_per_blk = (size_t)p->npix * p->d.tree.cpad * p->tree_tb;   // float2 elements
     int blk_batch = p->user_batch > 0 ? std::max(1, p->user_batch / p->tree_tb) : 0;
     if (blk_batch <= 0) {
-        const size_t budget = (size_t)3 << 30;
+        // pass 2 runs one CTA per block and per SM: whole waves of blocks per launch
+        const size_t budget = (size_t)4 << 30;
         blk_batch = (int)std::min<size_t>(4096, std::max<size_t>(1, budget / (h_per_blk * sizeof(float2))));
+        int dev = 0, sms = 148;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (blk_batch > sms) blk_batch -= blk_batch % sms;
     }
     if (!w.Ht || w.blk_batch != blk_batch || w.ht_elems != h_per_blk * blk_batch) {
         cudaFree(w.Ht); cudaFree(w.sumsq_t); w.Ht = nullptr; w.sumsq_t = nullptr;

@@ -266,7 +266,8 @@ __device__ __forceinline__ void tree_row_stats(const float (&x)[16], int img, in
         atomicAdd(hw + min(bin, nbm1), inc);
         m = fmaxf(m, x[e]);
     }
-    // running peak of this warp: a new maximum is rare after the first rows, so one vote decides
+    // running peak of this warp: a new maximum is rare after the first rows, so one vote decides.
+    // Positions are full row-major indices (a warp may hold two rows when N < 512).
     if (__any_sync(0xffffffffu, m > cx.sBest[warp * cx.nimg + img])) {
         float wm = m;
 #pragma unroll
@@ -274,12 +275,12 @@ __device__ __forceinline__ void tree_row_stats(const float (&x)[16], int img, in
         int xp = 0x7fffffff;
         if (m == wm) {
 #pragma unroll
-            for (int e = 15; e >= 0; e--) if (x[e] == wm) xp = t + TPF * e;
+            for (int e = 15; e >= 0; e--) if (x[e] == wm) xp = y * N + t + TPF * e;
         }
 #pragma unroll
         for (int d = 16; d > 0; d >>= 1) xp = min(xp, __shfl_xor_sync(0xffffffffu, xp, d));
         __syncwarp();
-        if (lane == 0) { cx.sBest[warp * cx.nimg + img] = wm; cx.sBpos[warp * cx.nimg + img] = y * N + xp; }
+        if (lane == 0) { cx.sBest[warp * cx.nimg + img] = wm; cx.sBpos[warp * cx.nimg + img] = xp; }
         __syncwarp();
     }
     if (image_out != nullptr) {
@@ -289,10 +290,21 @@ __device__ __forceinline__ void tree_row_stats(const float (&x)[16], int img, in
     }
 }
 
+// 16-byte asynchronous global -> shared copy (LDGSTS): no register staging, no scoreboard wait
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+constexpr int kThreads2 = 512;          // tree pass 2: one CTA of 16 warps per SM
+constexpr int kWarps2 = kThreads2 / 32;
+
 template <int N, int TB>
-__global__ void __launch_bounds__(kThreads, 2) k_tree_rowfft_stats(const TreeParams p) {
+__global__ void __launch_bounds__(kThreads2, 1) k_tree_rowfft_stats(const TreeParams p) {
     using C = FftCfg<N>;
-    constexpr int G2 = kThreads / C::TPF;
+    constexpr int G2 = kThreads2 / C::TPF;
     constexpr int XB = fft_padded_size(N);
     constexpr int NIMG = 2 * TB - 1;
     constexpr int NW = (NIMG + 1) / 2;
@@ -301,23 +313,35 @@ __global__ void __launch_bounds__(kThreads, 2) k_tree_rowfft_stats(const TreePar
     // region 0 holds the FFT exchange buffers, later the unpacked histogram + prefix sums
     const int region0 = max(G2 * XB, p.nbins);                               // float2 units
     float2* tw = xbuf + region0;
-    uint32_t* hist = reinterpret_cast<uint32_t*>(tw + C::TW_TOTAL);          // [NW][nbins]
+    float4* stg = reinterpret_cast<float4*>(tw + C::TW_TOTAL);               // [G2][cpad] staged (row, pair)
+    uint32_t* hist = reinterpret_cast<uint32_t*>(stg + (size_t)G2 * p.cpad); // [NW][nbins]
     float* sA = reinterpret_cast<float*>(hist + (size_t)NW * p.nbins);       // [16]
     float* sScale = sA + 16;                                                 // [16]
     float* sSig = sScale + 16;                                               // [16] sigma_rms per image
     int* sValid = reinterpret_cast<int*>(sSig + 16);                         // [16]
-    float* sBest = reinterpret_cast<float*>(sValid + 16);                    // [8][NIMG]
-    int* sBpos = reinterpret_cast<int*>(sBest + kWarpsPerCta * NIMG);        // [8][NIMG]
+    float* sBest = reinterpret_cast<float*>(sValid + 16);                    // [16 warps][NIMG]
+    int* sBpos = reinterpret_cast<int*>(sBest + kWarps2 * NIMG);             // [16 warps][NIMG]
     uint32_t* hun = reinterpret_cast<uint32_t*>(xbuf);                       // after the row loop
     uint32_t* cum = hun + p.nbins;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int slot = blockIdx.x;
     const BlockDesc blk = p.blocks[slot];
+    const float2* Hblk = p.Ht + (size_t)slot * N * p.cpad * TB;
+    const int grp = tid / C::TPF, t = tid % C::TPF;
+    float4* sg = stg + (size_t)grp * p.cpad;
 
-    for (int i = tid; i < NW * p.nbins; i += kThreads) hist[i] = 0u;
-    load_twiddles<N>(tw, p.twiddles, tid, kThreads);
-    for (int i = tid; i < kWarpsPerCta * NIMG; i += kThreads) { sBest[i] = -CUDART_INF_F; sBpos[i] = 0; }
+    // stage (row y, pair p2): ncol contiguous 16-byte (H_a, H_b) entries, copied asynchronously
+    auto stage = [&](int y, int p2) {
+        const float4* src = reinterpret_cast<const float4*>(Hblk + ((size_t)y * (TB / 2) + p2) * p.cpad * 2);
+        for (int c = t; c < p.ncol; c += C::TPF) cp_async16(sg + c, src + c);
+        cp_async_commit();
+    };
+    stage(grp, 0);
+
+    for (int i = tid; i < NW * p.nbins; i += kThreads2) hist[i] = 0u;
+    load_twiddles<N>(tw, p.twiddles, tid, kThreads2);
+    for (int i = tid; i < kWarps2 * NIMG; i += kThreads2) { sBest[i] = -CUDART_INF_F; sBpos[i] = 0; }
     if (tid < NIMG) {
         int l = 0, off = 0;
         while (tid >= off + (TB >> l)) { off += TB >> l; l++; }
@@ -335,26 +359,31 @@ __global__ void __launch_bounds__(kThreads, 2) k_tree_rowfft_stats(const TreePar
     __syncthreads();
 
     TreeStatsCtx<C::TPF> cx{hist, sA, sScale, sValid, sBest, sBpos, 0.5f * (float)p.nbins, p.nbins, NIMG};
-    const float2* Hblk = p.Ht + (size_t)slot * N * p.cpad * TB;
-    const int grp = tid / C::TPF, t = tid % C::TPF;
     float2* xb = xbuf + grp * XB;
     const bool dbg = p.image_out != nullptr && slot == 0;
 
     for (int y = grp; y < N; y += G2) {
-        const float2* row = Hblk + (size_t)y * p.cpad * TB;
         float s2p[16], s4p[16];
 #pragma unroll 1
         for (int p2 = 0; p2 < TB / 2; p2++) {
             float2 v[16];
+            cp_async_wait_all();
+            fft_group_sync<C::TPF>(1 + grp);                     // every lane's copies have landed
 #pragma unroll
             for (int e = 0; e < 16; e++) {
                 const int c = t + C::TPF * e;
                 const int cc = (e < 8) ? c : N - c;
                 float4 h = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (cc < p.ncol) h = *reinterpret_cast<const float4*>(row + ((size_t)p2 * p.cpad + cc) * 2);
+                if (cc < p.ncol) h = sg[cc];
                 if (cc == 0 || cc == N / 2) v[e] = make_float2(h.x, h.z);
                 else if (e < 8) v[e] = make_float2(h.x - h.w, h.y + h.z);
                 else v[e] = make_float2(h.x + h.w, h.z - h.y);
+            }
+            fft_group_sync<C::TPF>(1 + grp);                     // staging buffer consumed
+            {   // prefetch the next (row, pair) of this group while this one is transformed
+                const int np2 = (p2 + 1 == TB / 2) ? 0 : p2 + 1;
+                const int ny = (p2 + 1 == TB / 2) ? y + G2 : y;
+                if (ny < N) stage(ny, np2);
             }
             fft_inverse<N>(v, xb, tw, t, 1 + grp);
             float a[16], s2[16];
@@ -401,7 +430,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_tree_rowfft_stats(const TreePar
         if (!sValid[img] && !report_zero) continue;            // block-uniform
         const uint32_t* hw = hist + (img >> 1) * p.nbins;
         const int sh = (img & 1) * 16;
-        const int per = p.nbins / kThreads;
+        const int per = p.nbins / kThreads2;
         uint32_t local = 0;
         for (int i = 0; i < per; i++) {
             const uint32_t c = (hw[tid * per + i] >> sh) & 0xffffu;
@@ -414,11 +443,11 @@ __global__ void __launch_bounds__(kThreads, 2) k_tree_rowfft_stats(const TreePar
             uint32_t o = __shfl_up_sync(0xffffffffu, inc, d);
             if (lane >= d) inc += o;
         }
-        __shared__ uint32_t wtot[kWarpsPerCta];
+        __shared__ uint32_t wtot[kWarps2];
         if (lane == 31) wtot[warp] = inc;
         __syncthreads();
         uint32_t base = inc - local, total = 0;
-        for (int w = 0; w < kWarpsPerCta; w++) { if (w < warp) base += wtot[w]; total += wtot[w]; }
+        for (int w = 0; w < kWarps2; w++) { if (w < warp) base += wtot[w]; total += wtot[w]; }
         for (int i = 0; i < per; i++) { cum[tid * per + i] = base; base += hun[tid * per + i]; }
         __syncthreads();
         if (warp == 0) {
@@ -433,7 +462,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_tree_rowfft_stats(const TreePar
             if (lane == 0) {
                 float bv = -CUDART_INF_F;
                 int bp = 0;
-                for (int w = 0; w < kWarpsPerCta; w++) {
+                for (int w = 0; w < kWarps2; w++) {
                     const float ov = sBest[w * NIMG + img];
                     const int op = sBpos[w * NIMG + img];
                     if (ov > bv || (ov == bv && op < bp)) { bv = ov; bp = op; }
