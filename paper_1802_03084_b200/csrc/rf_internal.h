@@ -26,6 +26,7 @@ void set_error(const char* fmt, ...);
 inline int cols_per_group(int npix) { return npix <= 512 ? 16 : (npix == 1024 ? 8 : 4); }
 constexpr int kWarpsPerCta = 8;     // 256 threads everywhere
 constexpr int kThreads = 32 * kWarpsPerCta;
+constexpr int kDmGroup = 8;         // DM trials interleaved in time by the tree path's block order
 constexpr int kTreeUnroll = 8;      // iterations of the tree gather kept in flight per warp
 constexpr float kHistRange = 3.5f;  // histogram covers +-kHistRange * sigma_rms
 

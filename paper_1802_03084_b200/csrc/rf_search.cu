@@ -127,7 +127,7 @@ int launch_tree(rf_plan* p, const TreeParams& tp, cudaStream_t st) {
             configured = smem;
         }
         if ((rc = mark(p, st, -1)) != RF_OK) return rc;
-        kern<<<dim3(tp.n_blk, tp.ngroups), kThreads, smem, st>>>(tp);
+        kern<<<dim3(tp.ngroups, tp.n_blk), kThreads, smem, st>>>(tp);
         RF_CUDA_CHECK(cudaGetLastError());
         if ((rc = mark(p, st, 0)) != RF_OK) return rc;
     }

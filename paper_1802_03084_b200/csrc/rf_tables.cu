@@ -6,6 +6,7 @@
 // (c) PAPER.md:72, 84: FFT imaging without a gridding kernel -> nearest cell (reading A8).
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 
 #include "rf_internal.h"
@@ -312,10 +313,12 @@ int build_image_list(rf_plan* p) {
     p->h_num_t.assign((size_t)p->ndm * p->ndt, 0);
     p->vis_gridded = 0;
     p->n_images = 0;
+    std::vector<int> nsearch_of(p->ndm, 0);
+    std::vector<char> in_tree_dm(p->ndm, 0);
     for (int d = 0; d < p->ndm; d++) {
         int nsearch = p->nint - p->h_maxdelay[d];
         if (p->span > 0) nsearch = std::min(nsearch, p->span);
-        bool any_tree = false;
+        nsearch_of[d] = nsearch;
         for (int k = 0; k < p->ndt; k++) {
             int dt = p->dts[k];
             int nj = nsearch > 0 ? nsearch / dt : 0;
@@ -324,11 +327,31 @@ int build_image_list(rf_plan* p) {
             p->vis_gridded += (int64_t)nj * dt * p->n_kept;
             bool in_tree = false;
             for (int l = 0; l < 4; l++) in_tree |= (p->tree_dt_idx[l] == k);
-            if (in_tree) { any_tree |= nj > 0; continue; }
+            if (in_tree) { in_tree_dm[d] |= nj > 0; continue; }
             for (int j = 0; j < nj; j++) imgs.push_back({d, k, j, dt});
         }
-        if (any_tree)
-            for (int tb = 0; tb * p->tree_tb < nsearch; tb++) blocks.push_back({d, tb, nsearch, 0});
+    }
+    // Block order of the tree path: DM trials sorted by their sweep and taken in groups of
+    // kDmGroup neighbours; inside a group time runs in the OUTER loop.  Consecutive blocks then
+    // read nearly the same window of every (baseline, channel) row (neighbouring DMs differ by a
+    // few integrations of delay), so the gather is served from L2 instead of re-reading the whole
+    // Stokes-I array from HBM once per DM trial.
+    if (p->tree_tb > 0) {
+        std::vector<int> order(p->ndm);
+        for (int d = 0; d < p->ndm; d++) order[d] = d;
+        std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return p->h_maxdelay[a] < p->h_maxdelay[b]; });
+        int dm_group = kDmGroup;
+        if (const char* e = getenv("RF_DMGROUP")) dm_group = std::max(1, atoi(e));
+        for (int g0 = 0; g0 < p->ndm; g0 += dm_group) {
+            const int g1 = std::min(p->ndm, g0 + dm_group);
+            int max_search = 0;
+            for (int i = g0; i < g1; i++) if (in_tree_dm[order[i]]) max_search = std::max(max_search, nsearch_of[order[i]]);
+            for (int tb = 0; tb * p->tree_tb < max_search; tb++)
+                for (int i = g0; i < g1; i++) {
+                    const int d = order[i];
+                    if (in_tree_dm[d] && tb * p->tree_tb < nsearch_of[d]) blocks.push_back({d, tb, nsearch_of[d], 0});
+                }
+        }
     }
     p->n_gen_images = (int64_t)imgs.size();
     p->n_blocks = (int64_t)blocks.size();

@@ -84,7 +84,8 @@ __global__ void k_stokes_transpose(const float* __restrict__ vis, float2* __rest
 }
 
 // ------------------------------------------------------------------------------------------
-// Tree pass 1.  grid = (n_blk, ngroups); block = 256.  Dynamic smem:
+// Tree pass 1.  grid = (ngroups, n_blk) -- column groups of one block run together, so their 32-byte
+// pieces of one H line meet in L2 before the line is written back; block = 256.  Dynamic smem:
 //   tile [TB*NCOL][PITCH] float2 (column f = q*NCOL + c) | tw | sdelay [nchan] | red [8][2*TB-1]
 template <int N, int TB, int NCOL>
 __global__ void __launch_bounds__(kThreads) k_tree_grid_colfft(const TreeParams p) {
@@ -101,7 +102,7 @@ __global__ void __launch_bounds__(kThreads) k_tree_grid_colfft(const TreeParams 
     float* red = reinterpret_cast<float*>(sdelay + p.nchan);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int slot = blockIdx.x, g = blockIdx.y;
+    const int slot = blockIdx.y, g = blockIdx.x;
     const BlockDesc blk = p.blocks[slot];
     const int t0 = blk.tb * TB;
     const int j = lane / TB, q = lane % TB;
@@ -203,6 +204,9 @@ __global__ void __launch_bounds__(kThreads) k_tree_grid_colfft(const TreeParams 
     {
         constexpr int G1 = kThreads / C::TPF;
         const int grp = tid / C::TPF, t = tid % C::TPF;
+#ifdef RF_EXP_NOFFT
+        if (p.nchan < 0)
+#endif
         for (int f = grp; f < NF; f += G1) {
             float2* col = tile + f * PITCH;
             float2 v[16];
@@ -223,6 +227,9 @@ __global__ void __launch_bounds__(kThreads) k_tree_grid_colfft(const TreeParams 
         const int i = tid % SEG, pr = i / NCOL, c = i % NCOL, y0 = tid / SEG;
         const float2* ta = tile + (2 * pr * NCOL + c) * PITCH;
         const float2* tb = ta + NCOL * PITCH;
+#ifdef RF_EXP_NOSTORE
+        if (p.nchan < 0)
+#endif
         for (int y = y0; y < N; y += kThreads / SEG) {
             const float2 a = ta[fft_pad(y)], b = tb[fft_pad(y)];
             Hs[((size_t)y * (TB / 2) + pr) * p.cpad + g * NCOL + c] = make_float4(a.x, a.y, b.x, b.y);
