@@ -85,15 +85,41 @@ def _setup(cfg, segment=0):
 
 
 def _alg_bytes(cfg, plan):
-    """A_img = 16 N_bl N_chan,w dt + 16 N_pix^2 per image; split per kernel as
-    pass 1 (+ the Stokes transpose that feeds it) = the visibility read + the hand-off write (8 N^2),
-    pass 2 = the hand-off read (8 N^2)."""
+    """A_img = 16 N_bl N_chan,w dt + 16 N_pix^2 per image, split per kernel kind
+    (rf_plan_get_kernel_times): the visibility read belongs to the kernel that gathers (kind 3 for the
+    widths on the boxcar tree, kind 0 for the per-image path), the hand-off write (8 N^2) to the column
+    FFT (kind 0), the hand-off read (8 N^2) to the row FFT + statistics (kind 1)."""
     c = plan.get_counters()
     images = c["images"]
+    tree = [k for k, dt in enumerate(cfg.dt_list) if dt in (1, 2, 4, 8) and 256 <= cfg.npix <= 1024]
+    vis_tree = sum(16.0 * plan.num_t(d, k) * cfg.dt_list[k] * c["n_kept"] for d in range(cfg.ndm) for k in tree)
     vis_bytes = 16.0 * c["vis_gridded"]                     # 16 B per (bl, ch) pol pair per native sample
     hand = 8.0 * cfg.npix * cfg.npix * images
-    return {"total": vis_bytes + 2 * hand, "pass1": vis_bytes + hand, "pass2": hand, "images": images,
-            "vis_gridded": c["vis_gridded"]}
+    return {"total": vis_bytes + 2 * hand, "kind": [vis_bytes - vis_tree + hand, hand, 0.0, vis_tree],
+            "images": images, "vis_gridded": c["vis_gridded"]}
+
+
+KIND_NAMES = ["column FFT kernels (k_tree_colfft; k_grid_colfft on the per-image path)",
+              "row FFT + statistics kernels (k_tree_rowfft_stats / k_rowfft_stats)",
+              "Stokes-I transpose (k_stokes_transpose)",
+              "gather + grid kernel (k_tree_gather)"]
+
+
+def _roofline(alg, k_ms, k_n, ms_per_step, traffic=None):
+    peak, peak_src = _peaks()
+    dom = max((0, 1, 3), key=lambda k: k_ms[k])
+    per_launch_bytes = alg["kind"][dom] / max(1, k_n[dom])
+    achieved = per_launch_bytes / (k_ms[dom] / max(1, k_n[dom]) * 1e-3) / 1e9
+    path_gbs = alg["total"] / (ms_per_step * 1e-3) / 1e9
+    names = ["pass1", "pass2", "prep", "gather"]
+    return {"bound": "hbm", "kernel": KIND_NAMES[dom], "achieved": achieved, "peak": peak, "unit": "GB/s",
+            "frac": achieved / peak, "traffic": traffic[dom] if traffic else None, "peak_source": peak_src,
+            "alg_bytes_per_launch": per_launch_bytes,
+            "kernel_ms_per_step": {n: k_ms[i] for i, n in enumerate(names)},
+            "kernel_launches_per_step": {n: k_n[i] for i, n in enumerate(names)},
+            "kernel_alg_gbs": {n: (alg["kind"][i] / (k_ms[i] * 1e-3) / 1e9 if k_ms[i] > 0 else 0.0)
+                               for i, n in enumerate(names)},
+            "path": {"alg_bytes_per_step": alg["total"], "achieved": path_gbs, "frac": path_gbs / peak}}
 
 
 def _oracle_worker(args):
@@ -251,19 +277,13 @@ def run_ours(args, cfg):
     e2e_value = world * images / (e2e_ms / args.steps * 1e-3)
 
     if rank == 0:
-        peak, peak_src = _peaks()
-        dom = 0 if k_ms[0] >= k_ms[1] else 1
-        dom_name = ["grid + column FFT kernels (k_tree_grid_colfft / k_grid_colfft)",
-                    "row FFT + statistics kernels (k_tree_rowfft_stats / k_rowfft_stats)"][dom]
-        per_launch_ms = k_ms[dom] / max(1, k_n[dom])
-        per_launch_bytes = alg["pass1" if dom == 0 else "pass2"] / max(1, k_n[dom])
-        achieved = per_launch_bytes / (per_launch_ms * 1e-3) / 1e9
         traffic = None
         tpath = os.path.join(ROOT, "profiles", "r1_traffic_lband.json.txt")
         if cfg.name == "lband" and not args.batch and os.path.exists(tpath):
             with open(tpath) as fh:       # one ncu --set full capture of this launch configuration
-                traffic = json.load(fh)["pass1_dram_bytes_per_launch" if dom == 0 else "pass2_dram_bytes_per_launch"]
-        path_gbs = alg["total"] / (ms_per_step * 1e-3) / 1e9
+                tj = json.load(fh)
+            traffic = {0: tj.get("pass1_dram_bytes_per_launch"), 1: tj.get("pass2_dram_bytes_per_launch"),
+                       3: tj.get("gather_dram_bytes_per_launch")}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -278,12 +298,7 @@ def run_ours(args, cfg):
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(vis.nbytes),
                     "d2h_bytes_per_step": int(4 + min(n_e2e, capacity) * 32)},
             "gpu_launches": int(launches) * args.steps,
-            "roofline": {"bound": "hbm", "kernel": dom_name, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
-                         "alg_bytes_per_launch": per_launch_bytes,
-                         "kernel_ms_per_step": {"pass1": k_ms[0], "pass2": k_ms[1], "prep": k_ms[2]},
-                         "kernel_launches_per_step": {"pass1": k_n[0], "pass2": k_n[1], "prep": k_n[2]},
-                         "path": {"alg_bytes_per_step": alg["total"], "achieved": path_gbs, "frac": path_gbs / peak}},
+            "roofline": _roofline(alg, k_ms, k_n, ms_per_step, traffic),
         }
         if world == 1 and not args.no_cpu_baseline:
             v, cores, sample = oracle_throughput(cfg, vis, args.ref_images)
@@ -413,14 +428,9 @@ def run_stream(args, cfg):
     k_ms, k_n = plans[b].get_kernel_times()
     launches = plans[b].get_counters()["kernel_launches"]
     alg = _alg_bytes(cfg, plans[b])
-    peak, peak_src = _peaks()
-    dom = 0 if k_ms[0] >= k_ms[1] else 1
-    per_launch_bytes = alg["pass1" if dom == 0 else "pass2"] / max(1, k_n[dom])
-    achieved = per_launch_bytes / (k_ms[dom] / max(1, k_n[dom]) * 1e-3) / 1e9
     ms_per_step = dev_ms / n_timed
     data_s = cfg.stride_int * cfg.inttime_s
     new_bytes = cfg.stride_int * cfg.nbl * cfg.nchan * cfg.npol * 8
-    path_gbs = alg["total"] / (ms_per_step * 1e-3) / 1e9
     line = {
         "metric": METRIC, "value": images / (ms_per_step * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": n_timed,
         "warmup": n_warm, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -439,11 +449,7 @@ def run_stream(args, cfg):
         "e2e": {"value": images * n_timed / (wall_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(new_bytes),
                 "d2h_bytes_per_step": int(4 + capacity * 32)},
         "gpu_launches": int(launches) * n_timed,
-        "roofline": {"bound": "hbm", "kernel": ["grid + column FFT kernels", "row FFT + statistics kernels"][dom],
-                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
-                     "peak_source": peak_src, "alg_bytes_per_launch": per_launch_bytes,
-                     "kernel_ms_per_step": {"pass1": k_ms[0], "pass2": k_ms[1], "prep": k_ms[2]},
-                     "path": {"alg_bytes_per_step": alg["total"], "achieved": path_gbs, "frac": path_gbs / peak}},
+        "roofline": _roofline(alg, k_ms, k_n, ms_per_step),
     }
     print(json.dumps(line), flush=True)
     for pl in plans:

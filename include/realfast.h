@@ -142,8 +142,9 @@ int rf_search_host(rf_plan* plan, const void* vis_host, rf_cand* cand_host, int3
 /* Per-kernel timing for roofline accounting: when enabled, rf_search brackets every kernel
  * launch with CUDA events on its stream.  After the caller has synchronised, get_kernel_times
  * returns, for the last rf_search, the summed durations (ms) and launch counts per kernel
- * kind: index 0 = grid + column FFT (pass 1, either variant), 1 = row FFT + statistics
- * (pass 2, either variant), 2 = Stokes-I transpose (prep of the boxcar tree), 3 = unused. */
+ * kind: index 0 = grid + column FFT (per-image path) or column FFT alone (boxcar-tree path),
+ * 1 = row FFT + statistics (either path), 2 = Stokes-I transpose (prep of the boxcar tree),
+ * 3 = gather + grid into the compact cell list (boxcar-tree path). */
 int rf_plan_set_profiling(rf_plan* plan, int enable);
 int rf_plan_get_kernel_times(rf_plan* plan, float ms[4], int32_t launches[4]);
 

@@ -34,7 +34,7 @@ int rebuild_geometry(rf_plan* p) {
 void free_tables(rf_plan* p) {
     rf::DeviceTables& d = p->d;
     cudaFree(d.delay); cudaFree(d.cell); cudaFree(d.keep); cudaFree(d.gen.entries); cudaFree(d.gen.warp_chunk);
-    cudaFree(d.tree.entries); cudaFree(d.tree.warp_chunk); cudaFree(d.blocks); cudaFree(d.images); cudaFree(d.freqs); cudaFree(d.uvw); cudaFree(d.dms); cudaFree(d.weights); cudaFree(d.twiddles);
+    cudaFree(d.tree.entries); cudaFree(d.tree.cells); cudaFree(d.tree.stream_iter); cudaFree(d.tree.stream_cell); cudaFree(d.tree.group_cell); cudaFree(d.blocks); cudaFree(d.images); cudaFree(d.freqs); cudaFree(d.uvw); cudaFree(d.dms); cudaFree(d.weights); cudaFree(d.twiddles);
     p->dev_cap.clear();
     d = rf::DeviceTables{};
 }
@@ -54,6 +54,7 @@ int rf_plan_create(rf_plan** out, const double* freqs_hz, int nchan, const doubl
     if (nchan <= 0 || nbl <= 0 || nint <= 0 || ndm <= 0 || ndt <= 0) { set_error("counts must be positive"); return RF_ERR_ARG; }
     if (nchan > 4096) { set_error("nchan %d > 4096", nchan); return RF_ERR_ARG; }
     if ((long long)nbl * nchan >= (1ll << 24)) { set_error("nbl*nchan must be < 2^24"); return RF_ERR_ARG; }
+    if (nbl >= (1 << 16)) { set_error("nbl must be < 2^16"); return RF_ERR_ARG; }
     if (npol != 1 && npol != 2 && npol != 4) { set_error("npol must be 1, 2 or 4"); return RF_ERR_ARG; }
     if (npix < 64 || npix > 4096 || (npix & (npix - 1))) { set_error("npix must be a power of two in 64..4096"); return RF_ERR_ARG; }
     if (!finite_pos(inttime_s) || !finite_pos(cell_rad)) { set_error("inttime and cell must be finite and positive"); return RF_ERR_ARG; }

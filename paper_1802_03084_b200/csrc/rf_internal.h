@@ -28,6 +28,7 @@ constexpr int kWarpsPerCta = 8;     // 256 threads everywhere
 constexpr int kThreads = 32 * kWarpsPerCta;
 constexpr int kDmGroup = 8;         // DM trials interleaved in time by the tree path's block order
 constexpr int kTreeUnroll = 8;      // iterations of the tree gather kept in flight per warp
+constexpr int kStreamIters = 64;    // target length of one warp stream of the tree gather
 constexpr float kHistRange = 3.5f;  // histogram covers +-kHistRange * sigma_rms
 
 // One image of the search loop: 16 bytes, device-resident list.
@@ -51,15 +52,30 @@ struct BlockDesc {
     int32_t dm_idx, tb, nsearch, pad;
 };
 
-// Tree-path lists reuse GridEntry with a different meaning of bits 24..29 of w0:
-//   bit 29 = END: last iteration of its cell (all entries of that iteration carry it); bits 24..28 unused;
-//   w1 row/column are those of the CELL in every entry of its iterations.
+// Tree-path gather entry (4 bytes): one (baseline, channel) sample of one half-plane cell.
+//   bits 0..11 channel; bits 12..27 baseline; bit 28 EDGE: the cell lies on column 0 or N/2 (Parseval
+//   weight 1 instead of 2); bit 29 END: last iteration of its cell (every entry of that iteration
+//   carries it); bit 30 conjugate; bit 31 valid (0 = padding, weight 0).
+// Tree-path cell (4 bytes): bits 0..11 grid row; bits 12..15 column inside its column group;
+//   bit 16: the cell lies on column 0 or N/2 (Parseval weight 1 instead of 2).
 // Half-plane gridding lists for one choice of columns-per-CTA.
 struct GridLists {
     GridEntry* entries = nullptr;    // device [n_chunks * 32]
-    int32_t* warp_chunk = nullptr;   // device [ngroups * kWarpsPerCta + 1] chunk (generic) / iteration (tree) ranges
-    int colgrp = 0, cpad = 0, ngroups = 0, lg = 0;   // lg: entries per warp iteration (tree lists)
+    int32_t* warp_chunk = nullptr;   // device [ngroups * kWarpsPerCta + 1]
+    int colgrp = 0, cpad = 0, ngroups = 0;
     int64_t n_chunks = 0;
+};
+
+// Work lists of the boxcar-tree path (built by build_grid_lists, see rf_tables.cu).
+struct TreeLists {
+    uint32_t* entries = nullptr;     // device [n_iters * lg]
+    int32_t* stream_iter = nullptr;  // device [n_streams + 1] first iteration of each warp stream
+    int32_t* stream_cell = nullptr;  // device [n_streams + 1] first cell of each warp stream
+    uint32_t* cells = nullptr;       // device [n_cells] sorted by (column, row)
+    int32_t* group_cell = nullptr;   // device [ngroups + 1] first cell of each column group
+    int colgrp = 0, cpad = 0, ngroups = 0, lg = 0;
+    int n_cells = 0, n_streams = 0, n_parts = 0;   // n_parts = gather CTAs per block
+    int64_t n_iters = 0;
 };
 
 struct DeviceTables {
@@ -68,7 +84,8 @@ struct DeviceTables {
     int32_t* cell = nullptr;         // [nbl][nchan][2]
     uint8_t* keep = nullptr;         // [nbl][nchan]
     // gridding lists: generic path (colgrp = cols_per_group) and boxcar-tree path
-    GridLists gen, tree;
+    GridLists gen;
+    TreeLists tree;
     ImgDesc* images = nullptr;       // [n_gen_images] images searched by the generic path
     BlockDesc* blocks = nullptr;     // [n_blocks] blocks searched by the tree path
     // plan inputs on device
@@ -93,10 +110,11 @@ struct Workspace {
     // boxcar-tree path
     float2* visI = nullptr;          // [nbl*nchan][tpitch] Stokes-I (pol sum), time fastest
     float2* Ht = nullptr;            // [blk_batch][npix][cpad_tree][TB]
-    float* sumsq_t = nullptr;        // [blk_batch][2*TB-1][ngroups_tree]
+    float* sumsq_t = nullptr;        // [blk_batch][2*TB-1][n_parts] Parseval partials of the gather CTAs
+    float2* cellsum = nullptr;       // [blk_batch][n_cells][TB] gridded cell sums (compact grid)
     BlockDesc* dbg_block = nullptr;
     int blk_batch = 0;
-    size_t visI_elems = 0, ht_elems = 0;
+    size_t visI_elems = 0, ht_elems = 0, cs_elems = 0, ss_elems = 0;
 };
 
 }  // namespace rf

@@ -103,9 +103,8 @@ int launch_batch(rf_plan* p, const SearchParams& sp, cudaStream_t st) {
 // ---------------------------------------------------------------- boxcar-tree path
 template <int N> int tree_nbins(int tb) { return N <= 1024 ? 2048 : (N == 2048 ? 4096 : (tb == 2 ? 8192 : 4096)); }
 
-template <int N, int TB> size_t smem_tree1(int nchan, int ncol) {
-    return (size_t)TB * ncol * (fft_padded_size(N) + 1) * sizeof(float2) + FftCfg<N>::TW_TOTAL * sizeof(float2) +
-           (size_t)nchan * sizeof(int) + (size_t)kWarpsPerCta * (2 * TB - 1) * sizeof(float);
+template <int N, int TB> size_t smem_tree1(int ncol) {
+    return (size_t)TB * ncol * (fft_padded_size(N) + 1) * sizeof(float2) + FftCfg<N>::TW_TOTAL * sizeof(float2);
 }
 template <int N, int TB> size_t smem_tree2(int nbins, int cpad) {
     const size_t g2 = kThreads2 / FftCfg<N>::TPF;
@@ -115,18 +114,27 @@ template <int N, int TB> size_t smem_tree2(int nbins, int cpad) {
            (size_t)((2 * TB) / 2) * nbins * sizeof(uint32_t) + 64 * 4 + (size_t)2 * kWarps2 * (2 * TB - 1) * 4;
 }
 
+// event kinds: 0 = grid + column FFT (generic pass 1 / tree column FFT), 1 = row FFT + statistics,
+// 2 = Stokes-I transpose, 3 = tree gather
 template <int N, int TB, int NCOL>
 int launch_tree(rf_plan* p, const TreeParams& tp, cudaStream_t st) {
     int rc;
     {
-        auto kern = k_tree_grid_colfft<N, TB, NCOL>;
-        const size_t smem = smem_tree1<N, TB>(p->nchan, NCOL);
+        auto kern = k_tree_gather<TB>;
+        const size_t smem = (size_t)p->nchan * sizeof(int) + (size_t)kWarpsPerCta * (2 * TB - 1) * sizeof(float);
+        if ((rc = mark(p, st, -1)) != RF_OK) return rc;
+        kern<<<dim3(tp.n_parts, tp.n_blk), kThreads, smem, st>>>(tp);
+        RF_CUDA_CHECK(cudaGetLastError());
+        if ((rc = mark(p, st, 3)) != RF_OK) return rc;
+    }
+    {
+        auto kern = k_tree_colfft<N, TB, NCOL>;
+        const size_t smem = smem_tree1<N, TB>(NCOL);
         static size_t configured = 0;
         if (smem > configured) {
             RF_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             configured = smem;
         }
-        if ((rc = mark(p, st, -1)) != RF_OK) return rc;
         kern<<<dim3(tp.ngroups, tp.n_blk), kThreads, smem, st>>>(tp);
         RF_CUDA_CHECK(cudaGetLastError());
         if ((rc = mark(p, st, 0)) != RF_OK) return rc;
@@ -181,7 +189,14 @@ TreeParams tree_params(rf_plan* p) {
     tp.visI = p->ws.visI;
     tp.delay = p->d.delay;
     tp.entries = p->d.tree.entries;
-    tp.warp_chunk = p->d.tree.warp_chunk;
+    tp.stream_iter = p->d.tree.stream_iter;
+    tp.stream_cell = p->d.tree.stream_cell;
+    tp.cells = p->d.tree.cells;
+    tp.group_cell = p->d.tree.group_cell;
+    tp.cellsum = p->ws.cellsum;
+    tp.n_cells = p->d.tree.n_cells;
+    tp.n_streams = p->d.tree.n_streams;
+    tp.n_parts = p->d.tree.n_parts;
     tp.twiddles = p->d.twiddles;
     tp.Ht = p->ws.Ht;
     tp.sumsq = p->ws.sumsq_t;
@@ -219,11 +234,23 @@ int ensure_tree_workspace(rf_plan* p) {
         if (blk_batch > sms) blk_batch -= blk_batch % sms;
     }
     if (!w.Ht || w.blk_batch != blk_batch || w.ht_elems != h_per_blk * blk_batch) {
-        cudaFree(w.Ht); cudaFree(w.sumsq_t); w.Ht = nullptr; w.sumsq_t = nullptr;
+        cudaFree(w.Ht); w.Ht = nullptr;
         RF_CUDA_CHECK(cudaMalloc((void**)&w.Ht, h_per_blk * blk_batch * sizeof(float2)));
-        RF_CUDA_CHECK(cudaMalloc((void**)&w.sumsq_t, (size_t)blk_batch * (2 * p->tree_tb - 1) * p->d.tree.ngroups * sizeof(float)));
         w.blk_batch = blk_batch;
         w.ht_elems = h_per_blk * blk_batch;
+    }
+    // compact grid and Parseval partials follow the gridding lists (uvw / flags may change them)
+    const size_t cs_elems = (size_t)blk_batch * std::max(1, p->d.tree.n_cells) * p->tree_tb;
+    if (!w.cellsum || w.cs_elems < cs_elems) {
+        cudaFree(w.cellsum); w.cellsum = nullptr;
+        RF_CUDA_CHECK(cudaMalloc((void**)&w.cellsum, (cs_elems + cs_elems / 8) * sizeof(float2)));
+        w.cs_elems = cs_elems + cs_elems / 8;
+    }
+    const size_t ss_elems = (size_t)blk_batch * (2 * p->tree_tb - 1) * std::max(1, p->d.tree.n_parts);
+    if (!w.sumsq_t || w.ss_elems < ss_elems) {
+        cudaFree(w.sumsq_t); w.sumsq_t = nullptr;
+        RF_CUDA_CHECK(cudaMalloc((void**)&w.sumsq_t, (ss_elems + ss_elems / 8) * sizeof(float)));
+        w.ss_elems = ss_elems + ss_elems / 8;
     }
     if (!w.dbg_block) RF_CUDA_CHECK(cudaMalloc((void**)&w.dbg_block, sizeof(BlockDesc)));
     return RF_OK;
@@ -261,7 +288,7 @@ void free_workspace(rf_plan* p) {
     Workspace& w = p->ws;
     cudaFree(w.H); cudaFree(w.sumsq); cudaFree(w.hist); cudaFree(w.peak_val); cudaFree(w.peak_pos);
     cudaFree(w.ticket); cudaFree(w.counters); cudaFree(w.dbg_desc);
-    cudaFree(w.visI); cudaFree(w.Ht); cudaFree(w.sumsq_t); cudaFree(w.dbg_block);
+    cudaFree(w.visI); cudaFree(w.Ht); cudaFree(w.sumsq_t); cudaFree(w.cellsum); cudaFree(w.dbg_block);
     w = Workspace{};
 }
 
@@ -332,7 +359,7 @@ int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out
             tp.blocks = p->d.blocks + base;
             tp.n_blk = (int)std::min<int64_t>(p->ws.blk_batch, p->n_blocks - base);
             if ((rc = launch_tree_batch(p, tp, st)) != RF_OK) return rc;
-            p->last_launches += 2;
+            p->last_launches += 3;
         }
     }
     // ---- every other width: one gridding + transform per image

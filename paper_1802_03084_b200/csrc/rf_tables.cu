@@ -202,73 +202,69 @@ int build_grid_lists(rf_plan* p) {
     };
     // Tree path ("time in lanes"): a warp reads LG = 32/TB entries per iteration, lane = (entry j,
     // integration q), so the TB consecutive samples of an entry are one coalesced 8*TB-byte read.
-    // Every cell is owned by ONE warp: its entries fill ceil(n/LG) consecutive iterations, the lane
-    // accumulates over the iterations in a register, and the iteration flagged END reduces the LG
-    // lane groups (xor shuffles) and stores the cell -- no read-modify-write, fixed summation order.
-    // Cells are dealt to the 8 warps of the CTA longest-first onto the least-loaded warp; each warp's
-    // stream is padded to a multiple of kTreeUnroll iterations with weight-0 entries.
-    auto emit_tree = [&](GridLists& gl, int kColsPerGroup, int LG) -> int {
-        gl.colgrp = kColsPerGroup;
-        gl.lg = LG;
-        gl.cpad = (p->ncol + kColsPerGroup - 1) / kColsPerGroup * kColsPerGroup;
-        gl.ngroups = gl.cpad / kColsPerGroup;
-        struct Cell { size_t first; int n, iters; };
-        std::vector<GridEntry> entries;
-        std::vector<int32_t> warp_iter(gl.ngroups * kWarpsPerCta + 1, 0);
-        entries.reserve(raw.size() * 5 / 4 + (size_t)gl.ngroups * kWarpsPerCta * kTreeUnroll * LG);
-        std::vector<Cell> cells;
-        size_t pos = 0;
-        for (int g = 0; g < gl.ngroups; g++) {
-            const size_t gbeg = pos;
-            while (pos < raw.size() && (int)(raw[pos].col / kColsPerGroup) == g) pos++;
-            const size_t gend = pos;
-            cells.clear();
-            for (size_t c0 = gbeg; c0 < gend;) {
-                size_t c1 = c0;
-                while (c1 < gend && raw[c1].col == raw[c0].col && raw[c1].row == raw[c0].row) c1++;
-                cells.push_back({c0, (int)(c1 - c0), (int)((c1 - c0 + LG - 1) / LG)});
-                c0 = c1;
+    // Cells are numbered in (column, row) order.  The gather kernel walks them in WARP STREAMS:
+    // runs of consecutive cells of about kStreamIters iterations, cut at cell boundaries and padded
+    // to a multiple of kTreeUnroll iterations with weight-0 entries.  A cell of n entries fills
+    // ceil(n/LG) consecutive iterations of its stream; the lane accumulates over them in a register,
+    // the iteration flagged END sums the LG lane groups and writes the cell sum to the compact grid
+    // cellsum[block][cell][q] -- one owner per cell, fixed summation order, no atomics.  The column-FFT
+    // kernel of column group g then scatters cells group_cell[g] .. group_cell[g+1] into its tiles.
+    auto emit_tree = [&](TreeLists& tl, int kColsPerGroup, int LG) -> int {
+        tl.colgrp = kColsPerGroup;
+        tl.lg = LG;
+        tl.cpad = (p->ncol + kColsPerGroup - 1) / kColsPerGroup * kColsPerGroup;
+        tl.ngroups = tl.cpad / kColsPerGroup;
+        std::vector<uint32_t> entries, cells;
+        std::vector<int32_t> stream_iter, stream_cell, group_cell(tl.ngroups + 1, 0);
+        entries.reserve(raw.size() * 5 / 4 + 1024);
+        int64_t iters = 0, stream_start = 0;
+        auto pad_entry = [&]() -> uint32_t { return raw.empty() ? 0u : (raw[0].ch | ((raw[0].elem / (uint32_t)p->nchan) << 12)); };   // a kept sample, weight 0
+        auto close_stream = [&]() {
+            for (; (iters - stream_start) % kTreeUnroll; iters++)
+                for (int j = 0; j < LG; j++) entries.push_back(pad_entry());
+            stream_start = iters;
+        };
+        stream_iter.push_back(0);
+        stream_cell.push_back(0);
+        int next_group = 0;
+        for (size_t c0 = 0; c0 < raw.size();) {
+            size_t c1 = c0;
+            while (c1 < raw.size() && raw[c1].col == raw[c0].col && raw[c1].row == raw[c0].row) c1++;
+            const int n = (int)(c1 - c0), cit = (n + LG - 1) / LG;
+            const int g = (int)(raw[c0].col / kColsPerGroup);
+            while (next_group <= g) group_cell[next_group++] = (int32_t)cells.size();
+            if (iters - stream_start > 0 && iters - stream_start + cit > kStreamIters) {
+                close_stream();
+                stream_iter.push_back((int32_t)iters);
+                stream_cell.push_back((int32_t)cells.size());
             }
-            std::vector<size_t> order(cells.size());
-            for (size_t i = 0; i < order.size(); i++) order[i] = i;
-            std::stable_sort(order.begin(), order.end(), [&](size_t a, size_t b) { return cells[a].iters > cells[b].iters; });
-            std::vector<size_t> owned[kWarpsPerCta];
-            long long load[kWarpsPerCta] = {0};
-            for (size_t i : order) {
-                int best = 0;
-                for (int w = 1; w < kWarpsPerCta; w++) if (load[w] < load[best]) best = w;
-                owned[best].push_back(i);
-                load[best] += cells[i].iters;
-            }
-            for (int w = 0; w < kWarpsPerCta; w++) {
-                warp_iter[g * kWarpsPerCta + w] = (int32_t)(entries.size() / LG);
-                std::sort(owned[w].begin(), owned[w].end());        // (column, row) order inside the warp
-                size_t iters = 0;
-                for (size_t ci : owned[w]) {
-                    const Cell& c = cells[ci];
-                    const Raw& r0 = raw[c.first];
-                    for (int it = 0; it < c.iters; it++)
-                        for (int j = 0; j < LG; j++) {
-                            const int k = it * LG + j;
-                            const bool valid = k < c.n;
-                            const Raw& r = raw[c.first + (valid ? k : 0)];   // padding repeats a kept sample, weight 0
-                            GridEntry ge;
-                            ge.w0 = r.elem | (it == c.iters - 1 ? (1u << 29) : 0u) | (r.conj << 30) | (valid ? (1u << 31) : 0u);
-                            ge.w1 = r.ch | (r0.row << 12) | ((r0.col % kColsPerGroup) << 24);
-                            entries.push_back(ge);
-                        }
-                    iters += c.iters;
+            const bool edge = raw[c0].col == 0 || (int)raw[c0].col == N / 2;
+            cells.push_back(raw[c0].row | ((raw[c0].col % kColsPerGroup) << 12) | (edge ? (1u << 16) : 0u));
+            for (int it = 0; it < cit; it++)
+                for (int j = 0; j < LG; j++) {
+                    const int k = it * LG + j;
+                    const bool valid = k < n;
+                    const Raw& r = raw[c0 + (valid ? k : 0)];        // padding repeats a kept sample, weight 0
+                    entries.push_back(r.ch | ((r.elem / (uint32_t)p->nchan) << 12) | (edge ? (1u << 28) : 0u) |
+                                      (it == cit - 1 ? (1u << 29) : 0u) | (r.conj << 30) | (valid ? (1u << 31) : 0u));
                 }
-                if (gend > gbeg)
-                    for (; iters % kTreeUnroll; iters++)
-                        for (int j = 0; j < LG; j++) entries.push_back(GridEntry{raw[gbeg].elem, raw[gbeg].ch});
-            }
+            iters += cit;
+            c0 = c1;
         }
-        warp_iter[gl.ngroups * kWarpsPerCta] = (int32_t)(entries.size() / LG);
-        gl.n_chunks = (int64_t)(entries.size() / LG);
+        while (next_group <= tl.ngroups) group_cell[next_group++] = (int32_t)cells.size();
+        close_stream();
+        stream_iter.push_back((int32_t)iters);
+        stream_cell.push_back((int32_t)cells.size());
+        tl.n_iters = iters;
+        tl.n_cells = (int)cells.size();
+        tl.n_streams = (int)stream_iter.size() - 1;
+        tl.n_parts = (tl.n_streams + kWarpsPerCta - 1) / kWarpsPerCta;
         int rc;
-        if ((rc = upload(p, &gl.entries, entries.data(), entries.size())) != RF_OK) return rc;
-        return upload(p, &gl.warp_chunk, warp_iter.data(), warp_iter.size());
+        if ((rc = upload(p, &tl.entries, entries.data(), entries.size())) != RF_OK) return rc;
+        if ((rc = upload(p, &tl.cells, cells.data(), cells.size())) != RF_OK) return rc;
+        if ((rc = upload(p, &tl.stream_iter, stream_iter.data(), stream_iter.size())) != RF_OK) return rc;
+        if ((rc = upload(p, &tl.stream_cell, stream_cell.data(), stream_cell.size())) != RF_OK) return rc;
+        return upload(p, &tl.group_cell, group_cell.data(), group_cell.size());
     };
     int rc = emit(p->d.gen, cols_per_group(N));
     if (rc == RF_OK && p->tree_tb > 0) rc = emit_tree(p->d.tree, tree_cols_per_group(N, p->tree_tb), 32 / p->tree_tb);

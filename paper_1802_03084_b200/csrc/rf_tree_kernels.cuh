@@ -8,9 +8,10 @@
 //
 //   k_stokes_transpose   : vis [t][bl][ch][pol] -> Stokes-I sum visI [bl*nchan+ch][t] (time fastest),
 //                          so a block reads TB*8 contiguous bytes per (baseline, channel).
-//   k_tree_grid_colfft   : gathers the TB dedispersed samples of every entry, grids TB images into
-//                          shared-memory column tiles, Parseval sums of every tree node, column FFTs,
-//                          store of the half plane as H[y][c][q] (q = integration inside the block).
+//   k_tree_gather        : gathers the TB dedispersed samples of every entry and sums them per uv cell
+//                          (compact grid of the occupied half-plane cells), Parseval sums of every tree node.
+//   k_tree_colfft        : scatters the cells of its uv columns into shared-memory tiles, column FFTs,
+//                          store of the half plane as H[y][pair][c][q & 1] (q = integration in the block).
 //   k_tree_rowfft_stats  : per row, TB/2 Hermitian pair transforms; the wider images are running
 //                          sums of the rows in registers; all 2*TB-1 images get peak, histogram,
 //                          median/MAD, S/N and the threshold test.  The image is never stored.
@@ -25,12 +26,16 @@ namespace rf {
 struct TreeParams {
     const float2* visI;             // [nbl*nchan][tpitch]
     const int32_t* delay;           // [ndm][nchan]
-    const GridEntry* entries;
-    const int32_t* warp_chunk;
+    const uint32_t* entries;        // gather entries, [n_iters][LG]
+    const int32_t* stream_iter;     // [n_streams + 1]
+    const int32_t* stream_cell;     // [n_streams + 1]
+    const uint32_t* cells;          // [n_cells]
+    const int32_t* group_cell;      // [ngroups + 1]
     const BlockDesc* blocks;        // first block of this batch
     const float2* twiddles;
+    float2* cellsum;                // [n_blk][n_cells][TB] compact grid (unscaled sums)
     float2* Ht;                     // [n_blk][N][TB/2][cpad][2]
-    float* sumsq;                   // [n_blk][2*TB-1][ngroups]
+    float* sumsq;                   // [n_blk][2*TB-1][n_parts]
     int32_t* counters;
     rf_cand* cand_items;
     int32_t* cand_count;
@@ -38,7 +43,7 @@ struct TreeParams {
     float* image_out;               // debug: image `dbg_img` of block 0
     rf_cand* stats_out;
     int32_t dbg_img;                // -1 = off
-    int32_t tpitch, nchan, ncol, cpad, ngroups, nbins, n_blk;
+    int32_t tpitch, nchan, ncol, cpad, ngroups, nbins, n_blk, n_cells, n_streams, n_parts;
     int32_t dt_idx[4];              // tree level -> index in dt_list, or -1
     float norm;                     // 1 / (2 N_w npol)
     float threshold;
@@ -84,105 +89,89 @@ __global__ void k_stokes_transpose(const float* __restrict__ vis, float2* __rest
 }
 
 // ------------------------------------------------------------------------------------------
-// Tree pass 1.  grid = (ngroups, n_blk) -- column groups of one block run together, so their 32-byte
-// pieces of one H line meet in L2 before the line is written back; block = 256.  Dynamic smem:
-//   tile [TB*NCOL][PITCH] float2 (column f = q*NCOL + c) | tw | sdelay [nchan] | red [8][2*TB-1]
-template <int N, int TB, int NCOL>
-__global__ void __launch_bounds__(kThreads) k_tree_grid_colfft(const TreeParams p) {
-    using C = FftCfg<N>;
-    constexpr int PITCH = fft_padded_size(N) + 1;
-    constexpr int NF = TB * NCOL;
+// Tree pass 0: gather + grid.  grid = (n_parts, n_blk); block = 256 = 8 warp streams.  Dynamic smem:
+//   sdelay [nchan] int | red [8][2*TB-1] float.
+// "Time in lanes": lane = (entry j = lane / TB, integration q = lane % TB).  One iteration reads
+// LG = 32/TB entries; the TB dedispersed samples of an entry are ONE coalesced 8*TB-byte read of
+// visI[bl*nchan + ch][t0 + delay[ch] + q].  The lane accumulates over the iterations of a cell in a
+// register; the END iteration sums the LG lane groups with xor shuffles and group 0 writes the cell
+// sum (TB contiguous complex values) to the compact grid.  Parseval sums of every boxcar-tree node,
+// sum_cells w |sum_{q in node} G_q|^2, are taken at the same place (another log2(TB) xor steps over
+// q), so sigma_rms of every image of the block is known before any pixel exists.
+// No tile, no barriers inside the loop, few registers: latency is hidden by occupancy.
+template <int TB>
+__global__ void __launch_bounds__(kThreads) k_tree_gather(const TreeParams p) {
     constexpr int NIMG = 2 * TB - 1;
     constexpr int LG = 32 / TB, U = kTreeUnroll;
     constexpr int LEVELS = (TB == 8) ? 4 : (TB == 4 ? 3 : 2);      // log2(TB) + 1
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    float2* tile = reinterpret_cast<float2*>(smem_raw);
-    float2* tw = tile + NF * PITCH;
-    int* sdelay = reinterpret_cast<int*>(tw + C::TW_TOTAL);
+    int* sdelay = reinterpret_cast<int*>(smem_raw);
     float* red = reinterpret_cast<float*>(sdelay + p.nchan);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int slot = blockIdx.y, g = blockIdx.x;
+    const int part = blockIdx.x, slot = blockIdx.y;
     const BlockDesc blk = p.blocks[slot];
-    const int t0 = blk.tb * TB;
     const int j = lane / TB, q = lane % TB;
-
-    // ---- prologue: every global load of the set-up is issued before the tile is cleared
-    const int it_beg = p.warp_chunk[g * kWarpsPerCta + warp];
-    const int it_end = p.warp_chunk[g * kWarpsPerCta + warp + 1];
+    const int s = part * kWarpsPerCta + warp;
+    const bool has = s < p.n_streams;
+    const int it_beg = has ? p.stream_iter[s] : 0;
+    const int it_end = has ? p.stream_iter[s + 1] : 0;
+    int cell = has ? p.stream_cell[s] : 0;
     const int32_t* drow = p.delay + (size_t)blk.dm_idx * p.nchan;
-    const int d0 = tid < p.nchan ? drow[tid] : 0;
-    const int d1 = tid + kThreads < p.nchan ? drow[tid + kThreads] : 0;
-    const float2 tw0 = p.twiddles[tid < C::TW_TOTAL ? tid : 0];
-    const float2 tw1 = p.twiddles[tid + kThreads < C::TW_TOTAL ? tid + kThreads : 0];
-    GridEntry en[U];                       // entries of the next batch of iterations (prefetched)
+    uint32_t en[U];                        // entries of the next batch of iterations (prefetched)
 #pragma unroll
-    for (int u = 0; u < U; u++) en[u] = GridEntry{0u, 0u};
+    for (int u = 0; u < U; u++) en[u] = 0u;
     if (it_beg < it_end) {
 #pragma unroll
         for (int u = 0; u < U; u++) en[u] = p.entries[(size_t)(it_beg + u) * LG + j];
     }
-    for (int i = tid; i < NF * PITCH; i += kThreads) tile[i] = make_float2(0.f, 0.f);
-    if (tid < p.nchan) sdelay[tid] = d0;
-    if (tid + kThreads < p.nchan) sdelay[tid + kThreads] = d1;
-    for (int i = tid + 2 * kThreads; i < p.nchan; i += kThreads) sdelay[i] = drow[i];
-    if (tid < C::TW_TOTAL) tw[tid] = tw0;
-    if (tid + kThreads < C::TW_TOTAL) tw[tid + kThreads] = tw1;
+    for (int i = tid; i < p.nchan; i += kThreads) sdelay[i] = drow[i];
     __syncthreads();
 
-    // ---- gather + grid ("time in lanes"): lane = (entry j = lane / TB, integration q = lane % TB).
-    //      One iteration reads LG = 32/TB entries: the TB dedispersed samples of an entry are ONE
-    //      coalesced 8*TB-byte read.  A cell belongs to one warp; the lane accumulates over the cell's
-    //      iterations in a register, the END iteration sums the LG lane groups with xor shuffles and
-    //      group 0 stores the cell into the TB tiles (plain store: nobody else touches that cell).
-    //      Parseval sums of every boxcar-tree node, sum_cells w |sum_{q in node} G_q|^2, are taken
-    //      at the same place from the cell sums (another log2(TB) xor steps over q).
     float ps[LEVELS];
 #pragma unroll
     for (int l = 0; l < LEVELS; l++) ps[l] = 0.f;
-    {
-        const float2* vbase = p.visI + t0 + q;
-        float2 acc = make_float2(0.f, 0.f);
+    const float2* vbase = p.visI + blk.tb * TB + q;
+    float2* cs = p.cellsum + (size_t)slot * p.n_cells * TB + q;
+    float2 acc = make_float2(0.f, 0.f);
 #ifdef RF_EXP_NOGATHER
-        if (p.nchan < 0)
+    if (p.nchan < 0)
 #endif
-        for (int it = it_beg; it < it_end; it += U) {
-            GridEntry e[U];
-            float2 x[U];
+    for (int it = it_beg; it < it_end; it += U) {
+        uint32_t e[U];
+        float2 x[U];
 #pragma unroll
-            for (int u = 0; u < U; u++) e[u] = en[u];
+        for (int u = 0; u < U; u++) e[u] = en[u];
 #pragma unroll
-            for (int u = 0; u < U; u++)
-                x[u] = __ldg(vbase + (size_t)(e[u].w0 & 0xffffffu) * p.tpitch + sdelay[e[u].w1 & 0xfff]);
-            if (it + U < it_end) {
+        for (int u = 0; u < U; u++)
+            x[u] = __ldg(vbase + (size_t)(((e[u] >> 12) & 0xffffu) * p.nchan + (e[u] & 0xfffu)) * p.tpitch + sdelay[e[u] & 0xfffu]);
+        if (it + U < it_end) {
 #pragma unroll
-                for (int u = 0; u < U; u++) en[u] = p.entries[(size_t)(it + U + u) * LG + j];
-            }
+            for (int u = 0; u < U; u++) en[u] = p.entries[(size_t)(it + U + u) * LG + j];
+        }
 #pragma unroll
-            for (int u = 0; u < U; u++) {
-                const float wr = (e[u].w0 >> 31) ? 1.f : 0.f;                 // padding: weight 0
-                const float wi = (e[u].w0 & (1u << 30)) ? -wr : wr;           // conjugate
-                acc.x = fmaf(wr, x[u].x, acc.x);
-                acc.y = fmaf(wi, x[u].y, acc.y);
-                if (e[u].w0 & (1u << 29)) {                                   // warp-uniform: cell complete
+        for (int u = 0; u < U; u++) {
+            const float wr = (e[u] >> 31) ? 1.f : 0.f;                    // padding: weight 0
+            const float wi = (e[u] & (1u << 30)) ? -wr : wr;              // conjugate
+            acc.x = fmaf(wr, x[u].x, acc.x);
+            acc.y = fmaf(wi, x[u].y, acc.y);
+            if (e[u] & (1u << 29)) {                                      // warp-uniform: cell complete
 #pragma unroll
-                    for (int d = TB; d < 32; d <<= 1) {
-                        acc.x += __shfl_xor_sync(0xffffffffu, acc.x, d);
-                        acc.y += __shfl_xor_sync(0xffffffffu, acc.y, d);
-                    }
-                    const int row = (e[u].w1 >> 12) & 0xfff, col = (e[u].w1 >> 24) & 0xf;
-                    if (j == 0) tile[(q * NCOL + col) * PITCH + fft_pad(row)] = acc;
-                    const int gc = g * NCOL + col;
-                    const float wgt = (gc == 0 || gc == N / 2) ? 1.f : 2.f;
-                    ps[0] = fmaf(wgt, acc.x * acc.x + acc.y * acc.y, ps[0]);
-#pragma unroll
-                    for (int l = 1; l < LEVELS; l++) {
-                        acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 1 << (l - 1));
-                        acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 1 << (l - 1));
-                        ps[l] = fmaf(wgt, acc.x * acc.x + acc.y * acc.y, ps[l]);
-                    }
-                    acc = make_float2(0.f, 0.f);
+                for (int d = TB; d < 32; d <<= 1) {
+                    acc.x += __shfl_xor_sync(0xffffffffu, acc.x, d);
+                    acc.y += __shfl_xor_sync(0xffffffffu, acc.y, d);
                 }
+                if (j == 0) cs[(size_t)cell * TB] = acc;
+                cell++;
+                const float wgt = (e[u] & (1u << 28)) ? 1.f : 2.f;
+                ps[0] = fmaf(wgt, acc.x * acc.x + acc.y * acc.y, ps[0]);
+#pragma unroll
+                for (int l = 1; l < LEVELS; l++) {
+                    acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 1 << (l - 1));
+                    acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 1 << (l - 1));
+                    ps[l] = fmaf(wgt, acc.x * acc.x + acc.y * acc.y, ps[l]);
+                }
+                acc = make_float2(0.f, 0.f);
             }
         }
     }
@@ -197,8 +186,60 @@ __global__ void __launch_bounds__(kThreads) k_tree_grid_colfft(const TreeParams 
         float tot = 0.f;
 #pragma unroll
         for (int w = 0; w < kWarpsPerCta; w++) tot += red[w * NIMG + tid];
-        p.sumsq[((size_t)slot * NIMG + tid) * p.ngroups + g] = tot * p.norm * p.norm;
+        p.sumsq[((size_t)slot * NIMG + tid) * p.n_parts + part] = tot * p.norm * p.norm;
     }
+}
+
+// ------------------------------------------------------------------------------------------
+// Tree pass 1: column FFTs.  grid = (ngroups, n_blk) -- the column groups of one block run together,
+// so their 32-byte pieces of one H line meet in L2 before the line is written back; block = 256.
+// Dynamic smem:  tile [TB*NCOL][PITCH] float2 (column f = q*NCOL + c) | tw
+// The CTA scatters the cells of its NCOL uv columns from the compact grid into zeroed tiles,
+// transforms the TB*NCOL columns in place (inverse, along v) and stores the half plane.
+template <int N, int TB, int NCOL>
+__global__ void __launch_bounds__(kThreads) k_tree_colfft(const TreeParams p) {
+    using C = FftCfg<N>;
+    constexpr int PITCH = fft_padded_size(N) + 1;
+    constexpr int NF = TB * NCOL;
+    constexpr int KPRE = 3;                // compact-grid values per thread loaded ahead of the tile clear
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2* tile = reinterpret_cast<float2*>(smem_raw);
+    float2* tw = tile + NF * PITCH;
+
+    const int tid = threadIdx.x;
+    const int g = blockIdx.x, slot = blockIdx.y;
+    const int c_beg = p.group_cell[g], c_end = p.group_cell[g + 1];
+    const int nval = (c_end - c_beg) * TB;
+    const float2* cs = p.cellsum + ((size_t)slot * p.n_cells + c_beg) * TB;
+    const uint32_t* cm = p.cells + c_beg;
+
+    // ---- prologue: every global load of the set-up is issued before the tile is cleared
+    const float2 tw0 = p.twiddles[tid < C::TW_TOTAL ? tid : 0];
+    const float2 tw1 = p.twiddles[tid + kThreads < C::TW_TOTAL ? tid + kThreads : 0];
+    float2 pv[KPRE];
+    uint32_t pm[KPRE];
+#pragma unroll
+    for (int k = 0; k < KPRE; k++) {
+        const int i = tid + k * kThreads;
+        pv[k] = make_float2(0.f, 0.f);
+        pm[k] = 0u;
+        if (i < nval) { pv[k] = cs[i]; pm[k] = cm[i / TB]; }
+    }
+    for (int i = tid; i < NF * PITCH; i += kThreads) tile[i] = make_float2(0.f, 0.f);
+    if (tid < C::TW_TOTAL) tw[tid] = tw0;
+    if (tid + kThreads < C::TW_TOTAL) tw[tid + kThreads] = tw1;
+    __syncthreads();
+    // ---- scatter the cells of these columns: value i = (cell i / TB, integration i % TB)
+#pragma unroll
+    for (int k = 0; k < KPRE; k++) {
+        const int i = tid + k * kThreads;
+        if (i < nval) tile[((i % TB) * NCOL + ((pm[k] >> 12) & 0xf)) * PITCH + fft_pad(pm[k] & 0xfff)] = pv[k];
+    }
+    for (int i = tid + KPRE * kThreads; i < nval; i += kThreads) {
+        const uint32_t m = cm[i / TB];
+        tile[((i % TB) * NCOL + ((m >> 12) & 0xf)) * PITCH + fft_pad(m & 0xfff)] = cs[i];
+    }
+    __syncthreads();
 
     // ---- column FFTs in place (inverse, along v)
     {
@@ -355,7 +396,7 @@ __global__ void __launch_bounds__(kThreads2, 1) k_tree_rowfft_stats(const TreePa
         const int i = tid - off, dt = 1 << l;
         const int j = blk.tb * (TB >> l) + i;
         float tot = 0.f;
-        for (int gidx = 0; gidx < p.ngroups; gidx++) tot += p.sumsq[((size_t)slot * NIMG + tid) * p.ngroups + gidx];
+        for (int part = 0; part < p.n_parts; part++) tot += p.sumsq[((size_t)slot * NIMG + tid) * p.n_parts + part];
         const float sig = sqrtf(tot) / (float)dt;                // rms of the image (Parseval)
         const bool valid = p.dt_idx[l] >= 0 && (j + 1) * dt <= blk.nsearch && sig > 0.f;
         sValid[tid] = valid ? 1 : 0;
