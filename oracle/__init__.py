@@ -8,6 +8,7 @@ from .realfast_oracle import (  # noqa: F401
     K_DM,
     C_LIGHT,
     Candidate,
+    mean_subtract,
     delay_table,
     cell_table,
     dedisperse_resample,

@@ -4,6 +4,7 @@ Slow, unblocked, unfused: each function is the definition written out, in the
 order the paper gives it (PAPER.md = /root/reference/PAPER.md; readings A1-A20
 are DESIGN.md "Readings", taken from SURVEY.md section 8(c)).
 
+    O0  mean-visibility subtraction (prep)
     O1  delay table            PAPER.md:45 (footnote 1: tau = 4.15 ms DM / nu^2)
     O2  uv cell table          PAPER.md:72, 84 (FFT imaging, no gridding kernel)
     O3  dedisperse + resample  PAPER.md:63, 104 (loops over DM and sampling time), 118
@@ -48,6 +49,19 @@ class Candidate:
     @property
     def key(self) -> Tuple[int, int, int]:
         return (self.dm_idx, self.dt_idx, self.t_idx)
+
+
+# --------------------------------------------------------------------------- O0
+def mean_subtract(vis: np.ndarray) -> np.ndarray:
+    """complex128 [nint][nbl][nchan][npol]: vis minus its mean over the integrations of the segment,
+    separately for every (baseline, channel, polarisation).
+
+    "subtracting the mean visibility in time on timescales less [than] the VLA fringe rate" (PAPER.md:84-86);
+    the segment IS that timescale ("the largest size for which mean visibility subtraction is accurate",
+    PAPER.md:108).  Reading A21: one plain arithmetic mean over all nint integrations of the
+    segment; flagged channels are simply never gridded afterwards (A17), no weights enter the mean."""
+    v = np.asarray(vis).astype(np.complex128)
+    return v - v.mean(axis=0, keepdims=True)
 
 
 # --------------------------------------------------------------------------- O1

@@ -153,13 +153,16 @@ def make_segment(cfg: Config, segment: int = 0, *, noise: bool = True,
                  inject: bool = True, uvw_m: np.ndarray | None = None,
                  cell_rad: float | None = None,
                  sources: Sequence[Transient] | None = None,
-                 rows: Tuple[int, int] | None = None, out: np.ndarray | None = None) -> np.ndarray:
+                 rows: Tuple[int, int] | None = None, out: np.ndarray | None = None,
+                 persistent: Sequence[Tuple[float, int, int]] = ()) -> np.ndarray:
     """Visibilities of one segment: complex64 [nint][nbl][nchan][npol].
 
     Segment ``s`` of a streaming config covers absolute integrations
     [s*stride, s*stride + nint).  ``sources`` overrides the seeded transients.
     ``rows = (lo, hi)`` returns only the segment-relative integrations [lo, hi)
     (the same values ``make_segment(...)[lo:hi]`` would hold); ``out`` receives them in place.
+    ``persistent`` = (amplitude, l_pix, m_pix) of constant point sources present in every
+    integration (what the mean-visibility subtraction of PAPER.md:84-86 removes).
     """
     lo, hi = (0, cfg.nint) if rows is None else rows
     t_first = segment * cfg.stride_int
@@ -178,6 +181,9 @@ def make_segment(cfg: Config, segment: int = 0, *, noise: bool = True,
     f = channel_freqs_hz(cfg)
     ul = uvw[:, 0:1] * f[None, :] / C_M_S          # [nbl][nchan]
     vl = uvw[:, 1:2] * f[None, :] / C_M_S
+    for (amp, l_pix, m_pix) in persistent:
+        sig = (amp * np.exp(-2j * np.pi * (ul * l_pix + vl * m_pix) * cell)).astype(np.complex64)
+        vis += sig[None, :, :, None]
     for src in (transients(cfg) if sources is None else sources):
         phase = np.exp(-2j * np.pi * (ul * src.l_pix + vl * src.m_pix) * cell)
         sig = (src.amp * phase).astype(np.complex64)
