@@ -219,6 +219,8 @@ def run_ours(args, cfg):
         plan.set_chan_weights(W.chan_weights(cfg))
     if args.batch:
         plan.set_batch(args.batch)
+    if args.meansub:
+        plan.set_meansub(True)
     capacity = 1 << 17
     stream = torch.cuda.current_stream(dev)
     items = torch.empty(capacity * 32, dtype=torch.uint8, device=dev)
@@ -293,7 +295,8 @@ def run_ours(args, cfg):
                                    f"{list(cfg.dt_list)}, npix {cfg.npix})",
                        "images_per_step": images, "gvis_per_s": world * alg["vis_gridded"] / (ms_per_step * 1e-3) / 1e9,
                        "l2_policy": f"input segment {vis.nbytes / 1e9:.2f} GB is larger than L2 (126 MB); no flush",
-                       "candidates": n_cands, "parallelism": f"replicas x{world}" if world > 1 else "single GPU"},
+                       "candidates": n_cands, "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
+                       "prep": "mean-visibility subtraction fused into the readers" if args.meansub else "none"},
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(vis.nbytes),
                     "d2h_bytes_per_step": int(4 + min(n_e2e, capacity) * 32)},
@@ -466,6 +469,7 @@ def main():
     ap.add_argument("--batch", type=int, default=0, help="images per batch (0 = library default)")
     ap.add_argument("--ref-images", type=int, default=512, help="oracle sample size per timing")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--meansub", action="store_true", help="also run the prep stage (mean-visibility subtraction, 8f-1)")
     args = ap.parse_args()
     cfg = W.get_config(args.config)
     if args.steps is None:

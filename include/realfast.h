@@ -155,6 +155,18 @@ int rf_plan_get_kernel_times(rf_plan* plan, float ms[4], int32_t launches[4]);
  * transform per (dm, dt, j).  Rebuilds the work lists.                             */
 int rf_plan_set_mode(rf_plan* plan, int use_tree);
 
+/* Prep stage: mean-visibility subtraction.  "subtracting the mean visibility in
+ * time on timescales less [than] the VLA fringe rate ... removes constant sources";
+ * the segment is that timescale.  Reading A21: one arithmetic mean over all nint
+ * integrations of the segment per (baseline, channel, polarisation), float64 accumulation.
+ *   rf_plan_set_meansub(plan, 1): every later rf_search / rf_debug_image searches
+ *     vis - mean_t(vis) WITHOUT modifying vis (one extra streaming read of the segment; the mean is
+ *     subtracted inside the readers).  Default off.
+ *   rf_prep_meansub: subtracts the mean IN PLACE in the caller's DEVICE buffer
+ *     (complex64 [nint][nbl][nchan][npol], 16-byte aligned), enqueued on cuda_stream, no sync.   */
+int rf_plan_set_meansub(rf_plan* plan, int enable);
+int rf_prep_meansub(rf_plan* plan, void* vis_dev, void* cuda_stream);
+
 /* Thread-local description of the last error returned on this thread. */
 const char* rf_last_error(void);
 

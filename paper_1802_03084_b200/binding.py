@@ -21,6 +21,7 @@ EXPORTS = [
     "rf_plan_set_search_span", "rf_plan_get_tables", "rf_plan_num_images", "rf_plan_num_t",
     "rf_debug_image", "rf_plan_get_counters", "rf_plan_set_batch", "rf_last_error",
     "rf_search_host", "rf_plan_set_profiling", "rf_plan_get_kernel_times", "rf_plan_set_mode",
+    "rf_plan_set_meansub", "rf_prep_meansub",
 ]
 
 # numpy view of rf_cand (32 bytes)
@@ -76,6 +77,8 @@ def load_library() -> C.CDLL:
     lib.rf_plan_set_profiling.argtypes = [vp, C.c_int]
     lib.rf_plan_set_mode.argtypes = [vp, C.c_int]
     lib.rf_plan_get_kernel_times.argtypes = [vp, C.POINTER(C.c_float), ip]
+    lib.rf_plan_set_meansub.argtypes = [vp, C.c_int]
+    lib.rf_prep_meansub.argtypes = [vp, vp, vp]
     for name in EXPORTS:
         if name not in ("rf_plan_num_images", "rf_last_error"):
             getattr(lib, name).restype = C.c_int
@@ -211,6 +214,18 @@ class Plan:
     def set_mode(self, use_tree: bool) -> None:
         """rf_plan_set_mode: image-domain boxcar tree (default) or per-image resampling at the read."""
         _check(self._lib.rf_plan_set_mode(self._h, int(use_tree)))
+
+    def set_meansub(self, enable: bool) -> None:
+        """rf_plan_set_meansub: search vis - mean_t(vis) without modifying vis."""
+        _check(self._lib.rf_plan_set_meansub(self._h, int(enable)))
+
+    def prep_meansub(self, vis, stream=None) -> None:
+        """rf_prep_meansub: subtract the time mean in place in a torch complex64 CUDA tensor."""
+        import torch
+        assert vis.is_cuda and vis.dtype == torch.complex64 and vis.is_contiguous()
+        assert tuple(vis.shape) == (self.nint, self.nbl, self.nchan, self.npol), tuple(vis.shape)
+        st = torch.cuda.current_stream(vis.device) if stream is None else stream
+        _check(self._lib.rf_prep_meansub(self._h, vis.data_ptr(), st.cuda_stream))
 
     def debug_image(self, vis, dm_idx: int, dt_idx: int, t_idx: int, stream=None):
         """Returns (image float32 [npix][npix] numpy, stats record) of one (dm, dt, t)."""

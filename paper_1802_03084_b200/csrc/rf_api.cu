@@ -162,6 +162,18 @@ int rf_plan_set_mode(rf_plan* p, int use_tree) {
     return rebuild_geometry(p);
 }
 
+int rf_plan_set_meansub(rf_plan* p, int enable) {
+    if (!p) { set_error("null plan"); return RF_ERR_ARG; }
+    p->meansub = enable != 0;
+    return RF_OK;
+}
+
+int rf_prep_meansub(rf_plan* p, void* vis_dev, void* cuda_stream) {
+    if (!p || !vis_dev) { set_error("null pointer argument"); return RF_ERR_ARG; }
+    if (reinterpret_cast<uintptr_t>(vis_dev) & 15) { set_error("vis_dev must be 16-byte aligned"); return RF_ERR_ARG; }
+    return rf::launch_meansub_inplace(p, vis_dev, static_cast<cudaStream_t>(cuda_stream));
+}
+
 int rf_plan_set_chan_weights(rf_plan* p, const float* w) {
     if (!p || !w) { set_error("null pointer argument"); return RF_ERR_ARG; }
     for (int i = 0; i < p->nchan; i++) p->weights[i] = (w[i] != 0.0f) ? 1.0f : 0.0f;

@@ -115,6 +115,10 @@ struct Workspace {
     BlockDesc* dbg_block = nullptr;
     int blk_batch = 0;
     size_t visI_elems = 0, ht_elems = 0, cs_elems = 0, ss_elems = 0;
+    // prep (mean-visibility subtraction)
+    double2* mean_partial = nullptr; // [kMeanChunks][nbl*nchan*npol]
+    float2* mean_p = nullptr;        // [nbl*nchan*npol] time mean per polarisation product
+    float2* mean_i = nullptr;        // [nbl*nchan] sum over pol of mean_p
 };
 
 }  // namespace rf
@@ -125,6 +129,7 @@ struct rf_plan {
     float threshold = 0;
     int span = 0;                    // streaming search span (0 = all valid)
     bool use_tree = true;            // image-domain boxcar tree for power-of-two dt (rf_plan_set_mode)
+    bool meansub = false;            // search vis - mean_t(vis) (rf_plan_set_meansub)
     int user_batch = 0;
     std::vector<double> freqs, uvw, dms;
     std::vector<int32_t> dts;
@@ -172,6 +177,9 @@ int build_grid_lists(rf_plan* p);             // host binning of the cell table 
 int build_image_list(rf_plan* p);             // (dm, dt, j) loop -> d.images (generic) + d.blocks (tree)
 int tree_cols_per_group(int npix, int tb);
 void configure_tree(rf_plan* p);              // which dt values ride the boxcar tree    // columns per pass-1 CTA of the tree path
+// rf_prep.cu
+int launch_time_mean(rf_plan* p, const void* vis, cudaStream_t st);
+int launch_meansub_inplace(rf_plan* p, void* vis, cudaStream_t st);
 // rf_search.cu
 int ensure_workspace(rf_plan* p);
 void free_workspace(rf_plan* p);

@@ -19,6 +19,7 @@ namespace rf {
 
 struct SearchParams {
     const float* vis;               // complex64 [nint][nbl][nchan][npol] as floats
+    const float2* mean_i;           // [nbl*nchan] Stokes-I sum of the time means, or null (no subtraction)
     const int32_t* delay;           // [ndm][nchan]
     const GridEntry* entries;
     const int32_t* warp_chunk;
@@ -85,6 +86,16 @@ __device__ __forceinline__ void gather_grid(const SearchParams& p, float2* __res
                             re[u] += a.x + a.z; im_[u] += a.y + a.w;
                         }
                     }
+                }
+            }
+        }
+        if (p.mean_i != nullptr) {     // mean-visibility subtraction: sum_q (x_q - m) = sum_q x_q - nq m
+#pragma unroll
+            for (int u = 0; u < U; u++) {
+                if (e[u].w0 >> 31) {
+                    const float2 m = __ldg(p.mean_i + (e[u].w0 & 0xffffffu));
+                    re[u] = fmaf(-(float)nq, m.x, re[u]);
+                    im_[u] = fmaf(-(float)nq, m.y, im_[u]);
                 }
             }
         }

@@ -171,14 +171,15 @@ int launch_tree_batch(rf_plan* p, TreeParams& tp, cudaStream_t st) {
 
 int launch_prep(rf_plan* p, const void* vis, cudaStream_t st) {
     const int nelem = p->nbl * p->nchan;
+    const float2* mi = p->meansub ? p->ws.mean_i : nullptr;
     dim3 grid((nelem + 31) / 32, (p->tpitch + 31) / 32), block(32, 8);
     const float* v = reinterpret_cast<const float*>(vis);
     int rc;
     if ((rc = mark(p, st, -1)) != RF_OK) return rc;
     switch (p->npol) {
-        case 1: k_stokes_transpose<1><<<grid, block, 0, st>>>(v, p->ws.visI, p->nint, nelem, p->tpitch); break;
-        case 2: k_stokes_transpose<2><<<grid, block, 0, st>>>(v, p->ws.visI, p->nint, nelem, p->tpitch); break;
-        default: k_stokes_transpose<4><<<grid, block, 0, st>>>(v, p->ws.visI, p->nint, nelem, p->tpitch); break;
+        case 1: k_stokes_transpose<1><<<grid, block, 0, st>>>(v, p->ws.visI, mi, p->nint, nelem, p->tpitch); break;
+        case 2: k_stokes_transpose<2><<<grid, block, 0, st>>>(v, p->ws.visI, mi, p->nint, nelem, p->tpitch); break;
+        default: k_stokes_transpose<4><<<grid, block, 0, st>>>(v, p->ws.visI, mi, p->nint, nelem, p->tpitch); break;
     }
     RF_CUDA_CHECK(cudaGetLastError());
     return mark(p, st, 2);
@@ -259,6 +260,7 @@ int ensure_tree_workspace(rf_plan* p) {
 SearchParams base_params(rf_plan* p, const void* vis) {
     SearchParams sp{};
     sp.vis = reinterpret_cast<const float*>(vis);
+    sp.mean_i = p->meansub ? p->ws.mean_i : nullptr;
     sp.delay = p->d.delay;
     sp.entries = p->d.gen.entries;
     sp.warp_chunk = p->d.gen.warp_chunk;
@@ -289,6 +291,7 @@ void free_workspace(rf_plan* p) {
     cudaFree(w.H); cudaFree(w.sumsq); cudaFree(w.hist); cudaFree(w.peak_val); cudaFree(w.peak_pos);
     cudaFree(w.ticket); cudaFree(w.counters); cudaFree(w.dbg_desc);
     cudaFree(w.visI); cudaFree(w.Ht); cudaFree(w.sumsq_t); cudaFree(w.cellsum); cudaFree(w.dbg_block);
+    cudaFree(w.mean_partial); cudaFree(w.mean_p); cudaFree(w.mean_i);
     w = Workspace{};
 }
 
@@ -347,6 +350,12 @@ int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out
     p->last_launches = 0;
     p->n_events_used = 0;
     if (p->n_kept == 0) return RF_OK;      // nothing gridded: every image is zero, snr := 0
+    if (p->meansub) {                      // prep (8f-1): time means, subtracted on the fly by the readers
+        if ((rc = mark(p, st, -1)) != RF_OK) return rc;
+        if ((rc = launch_time_mean(p, vis, st)) != RF_OK) return rc;
+        if ((rc = mark(p, st, 2)) != RF_OK) return rc;
+        p->last_launches += 2;
+    }
     // ---- power-of-two widths: blocks of TB integrations through the boxcar tree
     if (p->tree_tb > 0 && p->n_blocks > 0) {
         if ((rc = launch_prep(p, vis, st)) != RF_OK) return rc;
@@ -380,6 +389,7 @@ int launch_debug_image(rf_plan* p, const void* vis, int dm_idx, int dt_idx, int 
                        float* image_dev, rf_cand* stats_dev, cudaStream_t st) {
     int rc = ensure_workspace(p);
     if (rc == RF_OK) rc = ensure_tree_workspace(p);
+    if (rc == RF_OK && p->meansub && p->n_kept > 0) rc = launch_time_mean(p, vis, st);
     if (rc != RF_OK) return rc;
     for (int l = 0; l < 4 && p->tree_tb > 0 && p->n_kept > 0; l++) {
         if (p->tree_dt_idx[l] != dt_idx) continue;

@@ -58,10 +58,11 @@ __host__ __device__ constexpr int tree_off(int tb, int l) {
 
 // ------------------------------------------------------------------------------------------
 // Stokes-I sum and transpose to time-fastest order.  grid (ceil(E/32), ceil(tpitch/32)), block (32, 8).
-// Rows t >= nint of the output (the read-ahead pad of the last block) are zero.
+// Rows t >= nint of the output (the read-ahead pad of the last block) are zero.  mean_i (or null):
+// Stokes-I sum of the time means, subtracted on the fly (mean-visibility subtraction).
 template <int NPOL>
 __global__ void k_stokes_transpose(const float* __restrict__ vis, float2* __restrict__ visI,
-                                   int nint, int nelem, int tpitch) {
+                                   const float2* __restrict__ mean_i, int nint, int nelem, int tpitch) {
     __shared__ float2 tile[32][33];
     const int e0 = blockIdx.x * 32, t0 = blockIdx.y * 32;
     for (int r = threadIdx.y; r < 32; r += 8) {
@@ -78,6 +79,7 @@ __global__ void k_stokes_transpose(const float* __restrict__ vis, float2* __rest
                     s.x += a.x + a.z; s.y += a.y + a.w;
                 }
             }
+            if (mean_i != nullptr) { const float2 m = __ldg(mean_i + e); s.x -= m.x; s.y -= m.y; }
         }
         tile[r][threadIdx.x] = s;
     }
