@@ -9,6 +9,7 @@ from .realfast_oracle import (  # noqa: F401
     C_LIGHT,
     Candidate,
     mean_subtract,
+    candidate_spectrum,
     delay_table,
     cell_table,
     dedisperse_resample,

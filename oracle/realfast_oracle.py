@@ -12,6 +12,7 @@ are DESIGN.md "Readings", taken from SURVEY.md section 8(c)).
     O5  2-D FFT Stokes-I image PAPER.md:88, 118
     O6  peak and robust sigma  PAPER.md:86-88 ("thresholding each image")
     O7  threshold              PAPER.md:88 ("S/N greater than a threshold")
+    O8  candidate cut-out: image + phased, dedispersed spectrum
 
 Pins (tests/test_oracle_pins.py): every function below is pinned to something
 other than itself -- closed forms, exact rational arithmetic, a direct DFT,
@@ -175,6 +176,37 @@ def image_stats(img: np.ndarray):
     sigma = MAD_TO_SIGMA * float(np.median(np.abs(flat - med)))
     snr = peak / sigma if sigma > 0.0 else 0.0
     return peak, y, x, sigma, snr
+
+
+# --------------------------------------------------------------------------- O8
+def candidate_spectrum(vis: np.ndarray, delay_dm: np.ndarray, iu: np.ndarray, iv: np.ndarray,
+                       keep: np.ndarray, npix: int, dt: int, j: int, l_pix: int, m_pix: int,
+                       half_window: int) -> np.ndarray:
+    """float64 [2*half_window + 1][nchan]: the dedispersed dynamic spectrum of the array phased towards
+    the candidate pixel -- the "spectrum" half of a candidate visualisation ("candidate
+    visualizations", 124-131 "image and spectrum").
+
+    Reading A22: row r is output integration jj = j - half_window + r of the candidate's
+    (DM, dt) series; spec[r][ch] = (1/n_ch) sum over the kept baselines of channel ch of
+    Re( s[bl][ch] e^{+2 pi i (iu x + iv y)/N} ) with s = dedisperse_resample(vis, delay, dt, jj) (O3),
+    (x, y) = (l_pix mod N, m_pix mod N), n_ch = kept baselines of that channel (0 for a channel without
+    any: flagged).  The phase uses the GRIDDED cell of each sample, so that the image pixel is exactly the
+    weighted channel sum:  image(dm, dt, jj)[y][x] = sum_ch n_ch spec[r][ch] / N_w   (pinned).
+    Rows whose integrations fall outside the segment are zero."""
+    nint, nbl, nchan, npol = vis.shape
+    x, y = l_pix % npix, m_pix % npix
+    out = np.zeros((2 * half_window + 1, nchan), dtype=np.float64)
+    n_ch = keep.sum(axis=0)
+    phase = np.exp(2j * np.pi * ((iu.astype(np.int64) * x + iv.astype(np.int64) * y) % npix) / npix)
+    for r in range(2 * half_window + 1):
+        jj = j - half_window + r
+        if jj < 0 or (jj + 1) * dt + int(np.max(delay_dm)) > nint:
+            continue
+        s = dedisperse_resample(vis, delay_dm, dt, jj)
+        for c in range(nchan):
+            if n_ch[c] > 0:
+                out[r, c] = np.real(s[keep[:, c], c] * phase[keep[:, c], c]).sum() / n_ch[c]
+    return out
 
 
 # --------------------------------------------------------------------------- O3-O7
