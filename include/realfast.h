@@ -167,6 +167,19 @@ int rf_plan_set_mode(rf_plan* plan, int use_tree);
 int rf_plan_set_meansub(rf_plan* plan, int enable);
 int rf_prep_meansub(rf_plan* plan, void* vis_dev, void* cuda_stream);
 
+/* Candidate cut-out, spectrum half ("candidate visualizations"; "image and
+ * spectrum"; the image half is rf_debug_image).  Writes to DEVICE memory the float32
+ * dynamic spectrum [2*half_window + 1][nchan] of the array phased towards pixel (l_pix, m_pix) (signed
+ * offsets as in rf_cand), dedispersed at DM trial dm_idx and averaged over dt = dt_list[dt_idx]:
+ * row r is output integration jj = t_idx - half_window + r,
+ *   spec[r][ch] = (1/n_ch) sum_{kept bl} Re( s[bl][ch] e^{+2 pi i (iu x + iv y)/npix} ),
+ * s = Stokes-I mean of vis[jj*dt + q + delay[dm][ch]][bl][ch][pol] over q < dt and pol, phase at the
+ * GRIDDED cell (reading A22), so sum_ch n_ch spec[r][ch] / N_w is the image pixel.  Rows outside
+ * [0, (nint - maxdelay(dm))/dt) and channels without kept baselines are zero.  Honours
+ * rf_plan_set_meansub.  Enqueues on cuda_stream, never synchronises.                            */
+int rf_cand_spectrum(rf_plan* plan, const void* vis_dev, int dm_idx, int dt_idx, int t_idx,
+                     int l_pix, int m_pix, int half_window, float* spec_dev, void* cuda_stream);
+
 /* Thread-local description of the last error returned on this thread. */
 const char* rf_last_error(void);
 

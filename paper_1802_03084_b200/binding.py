@@ -21,7 +21,7 @@ EXPORTS = [
     "rf_plan_set_search_span", "rf_plan_get_tables", "rf_plan_num_images", "rf_plan_num_t",
     "rf_debug_image", "rf_plan_get_counters", "rf_plan_set_batch", "rf_last_error",
     "rf_search_host", "rf_plan_set_profiling", "rf_plan_get_kernel_times", "rf_plan_set_mode",
-    "rf_plan_set_meansub", "rf_prep_meansub",
+    "rf_plan_set_meansub", "rf_prep_meansub", "rf_cand_spectrum",
 ]
 
 # numpy view of rf_cand (32 bytes)
@@ -79,6 +79,7 @@ def load_library() -> C.CDLL:
     lib.rf_plan_get_kernel_times.argtypes = [vp, C.POINTER(C.c_float), ip]
     lib.rf_plan_set_meansub.argtypes = [vp, C.c_int]
     lib.rf_prep_meansub.argtypes = [vp, vp, vp]
+    lib.rf_cand_spectrum.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, vp, vp]
     for name in EXPORTS:
         if name not in ("rf_plan_num_images", "rf_last_error"):
             getattr(lib, name).restype = C.c_int
@@ -226,6 +227,18 @@ class Plan:
         assert tuple(vis.shape) == (self.nint, self.nbl, self.nchan, self.npol), tuple(vis.shape)
         st = torch.cuda.current_stream(vis.device) if stream is None else stream
         _check(self._lib.rf_prep_meansub(self._h, vis.data_ptr(), st.cuda_stream))
+
+    def cand_spectrum(self, vis, dm_idx: int, dt_idx: int, t_idx: int, l_pix: int, m_pix: int,
+                      half_window: int, stream=None):
+        """rf_cand_spectrum: float32 numpy [2*half_window + 1][nchan] (phased, dedispersed spectrum)."""
+        import torch
+        assert vis.is_cuda and vis.dtype == torch.complex64 and vis.is_contiguous()
+        st = torch.cuda.current_stream(vis.device) if stream is None else stream
+        spec = torch.empty((2 * half_window + 1, self.nchan), dtype=torch.float32, device=vis.device)
+        _check(self._lib.rf_cand_spectrum(self._h, vis.data_ptr(), dm_idx, dt_idx, t_idx, l_pix, m_pix,
+                                          half_window, spec.data_ptr(), st.cuda_stream))
+        st.synchronize()
+        return spec.cpu().numpy()
 
     def debug_image(self, vis, dm_idx: int, dt_idx: int, t_idx: int, stream=None):
         """Returns (image float32 [npix][npix] numpy, stats record) of one (dm, dt, t)."""

@@ -228,6 +228,16 @@ int rf_debug_image(rf_plan* p, const void* vis_dev, int dm_idx, int dt_idx, int 
                                   static_cast<cudaStream_t>(cuda_stream));
 }
 
+int rf_cand_spectrum(rf_plan* p, const void* vis_dev, int dm_idx, int dt_idx, int t_idx, int l_pix, int m_pix,
+                     int half_window, float* spec_dev, void* cuda_stream) {
+    if (!p || !vis_dev || !spec_dev) { set_error("null pointer argument"); return RF_ERR_ARG; }
+    if (dm_idx < 0 || dm_idx >= p->ndm || dt_idx < 0 || dt_idx >= p->ndt) { set_error("trial index out of range"); return RF_ERR_STATE; }
+    if (half_window < 0 || half_window > 32767) { set_error("half_window out of range"); return RF_ERR_ARG; }
+    if (l_pix < -p->npix || l_pix >= p->npix || m_pix < -p->npix || m_pix >= p->npix) { set_error("pixel out of range"); return RF_ERR_ARG; }
+    return rf::launch_cand_spectrum(p, vis_dev, dm_idx, dt_idx, t_idx, l_pix, m_pix, half_window, spec_dev,
+                                    static_cast<cudaStream_t>(cuda_stream));
+}
+
 int rf_plan_get_counters(rf_plan* p, rf_counters* out) {
     if (!p || !out) { set_error("null pointer argument"); return RF_ERR_ARG; }
     int32_t c[4] = {0, 0, 0, 0};
