@@ -10,6 +10,7 @@ from .realfast_oracle import (  # noqa: F401
     Candidate,
     mean_subtract,
     candidate_spectrum,
+    inject_transient,
     delay_table,
     cell_table,
     dedisperse_resample,

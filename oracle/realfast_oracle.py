@@ -13,6 +13,7 @@ are DESIGN.md "Readings", taken from SURVEY.md section 8(c)).
     O6  peak and robust sigma  PAPER.md:86-88 ("thresholding each image")
     O7  threshold              PAPER.md:88 ("S/N greater than a threshold")
     O8  candidate cut-out: image + phased, dedispersed spectrum
+    O9  mock-transient injection
 
 Pins (tests/test_oracle_pins.py): every function below is pinned to something
 other than itself -- closed forms, exact rational arithmetic, a direct DFT,
@@ -206,6 +207,33 @@ def candidate_spectrum(vis: np.ndarray, delay_dm: np.ndarray, iu: np.ndarray, iv
         for c in range(nchan):
             if n_ch[c] > 0:
                 out[r, c] = np.real(s[keep[:, c], c] * phase[keep[:, c], c]).sum() / n_ch[c]
+    return out
+
+
+# --------------------------------------------------------------------------- O9
+def inject_transient(vis: np.ndarray, freqs_hz, uvw_m, inttime_s: float, cell_rad: float, amp: float,
+                     l_pix: float, m_pix: float, dm: float, width: int, t0: int) -> np.ndarray:
+    """complex128 copy of vis with a mock transient added ("randomly insert mock transient sources into
+    data ... inserted after calibration").
+
+    Reading A18: a point source of amplitude `amp` at pixel offset (l, m), i.e. direction cosines
+    (l*cell, m*cell), has visibility amp * e^{-2 pi i (u_lambda l + v_lambda m) cell} (sign convention A12);
+    it is added to every polarisation product at native integrations t0 + q + delay[ch], q < width, where
+    delay[ch] is the O1 delay of DM `dm` (arrival at the top channel at t0); samples that fall outside
+    the segment are dropped."""
+    out = np.asarray(vis).astype(np.complex128)
+    nint = out.shape[0]
+    f = np.asarray(freqs_hz, dtype=np.float64)
+    uvw = np.asarray(uvw_m, dtype=np.float64)
+    delay = delay_table(f, np.array([dm], dtype=np.float64), inttime_s)[0]
+    ul = uvw[:, 0:1] * f[None, :] / C_LIGHT
+    vl = uvw[:, 1:2] * f[None, :] / C_LIGHT
+    sig = amp * np.exp(-2j * np.pi * (ul * l_pix + vl * m_pix) * cell_rad)       # [nbl][nchan]
+    for c in range(f.size):
+        for q in range(width):
+            t = t0 + q + int(delay[c])
+            if 0 <= t < nint:
+                out[t, :, c, :] += sig[:, c, None]
     return out
 
 
