@@ -180,6 +180,16 @@ int rf_prep_meansub(rf_plan* plan, void* vis_dev, void* cuda_stream);
 int rf_cand_spectrum(rf_plan* plan, const void* vis_dev, int dm_idx, int dt_idx, int t_idx,
                      int l_pix, int m_pix, int half_window, float* spec_dev, void* cuda_stream);
 
+/* Mock-transient injection on the device ("The search pipeline will randomly insert
+ * mock transient sources into data as a test of its efficiency and sensitivity"; reading
+ * A18).  Adds, IN PLACE in the caller's DEVICE segment (complex64 [nint][nbl][nchan][npol]), a point
+ * source of amplitude amp at pixel offset (l_pix, m_pix) (fractions allowed; cell and uvw of the plan):
+ *   vis[t0 + q + delay[ch]][bl][ch][pol] += amp e^{-2 pi i (u_lambda l + v_lambda m) cell},  q < width,
+ * delay[ch] = the delay-table expression at DM `dm` (arrival at the top channel at t0).  Samples that
+ * fall outside the segment are dropped.  Enqueues on cuda_stream, never synchronises.          */
+int rf_inject(rf_plan* plan, void* vis_dev, double amp, double l_pix, double m_pix, double dm,
+              int width, int t0, void* cuda_stream);
+
 /* Thread-local description of the last error returned on this thread. */
 const char* rf_last_error(void);
 

@@ -21,7 +21,7 @@ EXPORTS = [
     "rf_plan_set_search_span", "rf_plan_get_tables", "rf_plan_num_images", "rf_plan_num_t",
     "rf_debug_image", "rf_plan_get_counters", "rf_plan_set_batch", "rf_last_error",
     "rf_search_host", "rf_plan_set_profiling", "rf_plan_get_kernel_times", "rf_plan_set_mode",
-    "rf_plan_set_meansub", "rf_prep_meansub", "rf_cand_spectrum",
+    "rf_plan_set_meansub", "rf_prep_meansub", "rf_cand_spectrum", "rf_inject",
 ]
 
 # numpy view of rf_cand (32 bytes)
@@ -79,6 +79,7 @@ def load_library() -> C.CDLL:
     lib.rf_plan_get_kernel_times.argtypes = [vp, C.POINTER(C.c_float), ip]
     lib.rf_plan_set_meansub.argtypes = [vp, C.c_int]
     lib.rf_prep_meansub.argtypes = [vp, vp, vp]
+    lib.rf_inject.argtypes = [vp, vp, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int, C.c_int, vp]
     lib.rf_cand_spectrum.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, vp, vp]
     for name in EXPORTS:
         if name not in ("rf_plan_num_images", "rf_last_error"):
@@ -227,6 +228,14 @@ class Plan:
         assert tuple(vis.shape) == (self.nint, self.nbl, self.nchan, self.npol), tuple(vis.shape)
         st = torch.cuda.current_stream(vis.device) if stream is None else stream
         _check(self._lib.rf_prep_meansub(self._h, vis.data_ptr(), st.cuda_stream))
+
+    def inject(self, vis, amp: float, l_pix: float, m_pix: float, dm: float, width: int, t0: int, stream=None) -> None:
+        """rf_inject: add a mock transient in place to a torch complex64 CUDA segment."""
+        import torch
+        assert vis.is_cuda and vis.dtype == torch.complex64 and vis.is_contiguous()
+        assert tuple(vis.shape) == (self.nint, self.nbl, self.nchan, self.npol), tuple(vis.shape)
+        st = torch.cuda.current_stream(vis.device) if stream is None else stream
+        _check(self._lib.rf_inject(self._h, vis.data_ptr(), amp, l_pix, m_pix, dm, width, t0, st.cuda_stream))
 
     def cand_spectrum(self, vis, dm_idx: int, dt_idx: int, t_idx: int, l_pix: int, m_pix: int,
                       half_window: int, stream=None):

@@ -238,6 +238,16 @@ int rf_cand_spectrum(rf_plan* p, const void* vis_dev, int dm_idx, int dt_idx, in
                                     static_cast<cudaStream_t>(cuda_stream));
 }
 
+int rf_inject(rf_plan* p, void* vis_dev, double amp, double l_pix, double m_pix, double dm, int width, int t0,
+              void* cuda_stream) {
+    if (!p || !vis_dev) { set_error("null pointer argument"); return RF_ERR_ARG; }
+    if (!std::isfinite(amp) || !std::isfinite(l_pix) || !std::isfinite(m_pix) || !std::isfinite(dm) || dm < 0 || width < 0) {
+        set_error("invalid source parameters");
+        return RF_ERR_ARG;
+    }
+    return rf::launch_inject(p, vis_dev, amp, l_pix, m_pix, dm, width, t0, static_cast<cudaStream_t>(cuda_stream));
+}
+
 int rf_plan_get_counters(rf_plan* p, rf_counters* out) {
     if (!p || !out) { set_error("null pointer argument"); return RF_ERR_ARG; }
     int32_t c[4] = {0, 0, 0, 0};

@@ -61,7 +61,52 @@ __global__ void __launch_bounds__(128) k_cand_spectrum(const float* __restrict__
     }
 }
 
+// Mock-transient injection ("randomly insert mock transient sources into data",
+// PAPER.md:135; reading A18): vis[t0 + q + delay[ch]][bl][ch][pol] += A e^{-2 pi i (u l + v m) cell}, q < width,
+// delay = the O1 expression at the injected DM (float64, explicit rounding, same operation order as
+// k_delay_table); the phase is evaluated in float64 (up to ~100 turns), the sum is rounded once to float32.
+// One thread per (baseline, channel); samples outside the segment are dropped.
+__global__ void k_inject(float2* __restrict__ vis, const double* __restrict__ freqs_hz, const double* __restrict__ uvw,
+                         int nint, int nbl, int nchan, int npol, double fmax_ghz, double inttime, double cell,
+                         double amp, double l_pix, double m_pix, double dm, int width, int t0) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nbl * nchan) return;
+    const int ch = i % nchan, bl = i / nchan;
+    const double fh = freqs_hz[ch];
+    const double f = __ddiv_rn(fh, 1e9);
+    const double a = __ddiv_rn(1.0, __dmul_rn(f, f));
+    const double b = __ddiv_rn(1.0, __dmul_rn(fmax_ghz, fmax_ghz));
+    const double x = __ddiv_rn(__dmul_rn(__dmul_rn(4.148808e-3, dm), __dsub_rn(a, b)), inttime);
+    const int delay = (int)floor(__dadd_rn(x, 0.5));
+    const double ul = uvw[3 * bl + 0] * fh / 299792458.0, vl = uvw[3 * bl + 1] * fh / 299792458.0;
+    double sn, cs;
+    sincospi(-2.0 * (ul * l_pix + vl * m_pix) * cell, &sn, &cs);
+    const double re = amp * cs, im = amp * sn;
+    const size_t row = (size_t)nbl * nchan * npol;
+    for (int q = 0; q < width; q++) {
+        const long long t = (long long)t0 + q + delay;
+        if (t < 0 || t >= nint) continue;
+        float2* dst = vis + (size_t)t * row + (size_t)i * npol;
+        for (int pol = 0; pol < npol; pol++) {
+            float2 v = dst[pol];
+            dst[pol] = make_float2((float)((double)v.x + re), (float)((double)v.y + im));
+        }
+    }
+}
+
 }  // namespace
+
+int launch_inject(rf_plan* p, void* vis, double amp, double l_pix, double m_pix, double dm, int width, int t0,
+                  cudaStream_t st) {
+    double fmax = 0.0;
+    for (double f : p->freqs) fmax = f > fmax ? f : fmax;
+    const int n = p->nbl * p->nchan;
+    k_inject<<<(n + 255) / 256, 256, 0, st>>>(reinterpret_cast<float2*>(vis), p->d.freqs, p->d.uvw, p->nint, p->nbl,
+                                              p->nchan, p->npol, fmax / 1e9, p->inttime, p->cell, amp, l_pix, m_pix, dm,
+                                              width, t0);
+    RF_CUDA_CHECK(cudaGetLastError());
+    return RF_OK;
+}
 
 int launch_cand_spectrum(rf_plan* p, const void* vis, int dm_idx, int dt_idx, int t_idx, int l_pix, int m_pix,
                          int half_window, float* spec_dev, cudaStream_t st) {

@@ -183,6 +183,8 @@ int launch_meansub_inplace(rf_plan* p, void* vis, cudaStream_t st);
 // rf_cutout.cu
 int launch_cand_spectrum(rf_plan* p, const void* vis, int dm_idx, int dt_idx, int t_idx, int l_pix, int m_pix,
                          int half_window, float* spec_dev, cudaStream_t st);
+int launch_inject(rf_plan* p, void* vis, double amp, double l_pix, double m_pix, double dm, int width, int t0,
+                  cudaStream_t st);
 // rf_search.cu
 int ensure_workspace(rf_plan* p);
 void free_workspace(rf_plan* p);
