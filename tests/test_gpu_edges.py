@@ -1,0 +1,113 @@
+"""GPU parity on the edges of the hot path: image sizes and polarisation counts the five configs do not
+use, degenerate plans (nothing kept, a DM that sweeps past the segment), unsorted trial lists, candidate
+overflow, ragged time ranges.  Everything is compared with the float64 oracle on the same bytes."""
+import numpy as np
+import pytest
+
+import oracle as O
+import workloads as W
+import workloads.generate  # noqa: F401
+
+pytestmark = pytest.mark.gpu
+
+PIX_TOL, SNR_TOL, NEAR_THR = 1e-4, 1e-3, 2e-3
+
+
+def _rand_vis(shape, seed):
+    rng = np.random.default_rng(seed)
+    return (rng.standard_normal(shape, dtype=np.float32) + 1j * rng.standard_normal(shape, dtype=np.float32)).astype(np.complex64)
+
+
+def _compare_all(plan, dvis, vis, f, uvw, cell, npix, dms, dts, thr, inttime, weights=None, min_match=1):
+    gpu, n = plan.search(dvis, capacity=1 << 15)
+    assert n == len(gpu)
+    ref, stats = O.search(vis, f, uvw, inttime, npix, cell, dms, dts, thr, chan_weights=weights, return_all_stats=True)
+    assert plan.num_images() == len(stats)
+    g = {(int(c["dm_idx"]), int(c["dt_idx"]), int(c["t_idx"])): c for c in gpu}
+    o = {c.key: c for c in ref}
+    for key in set(g) ^ set(o):
+        assert abs(stats[key][4] - thr) <= NEAR_THR * thr, (key, stats[key][4])
+    for key in set(g) & set(o):
+        assert abs(float(g[key]["snr"]) - o[key].snr) <= SNR_TOL * o[key].snr, key
+        assert (int(g[key]["l_pix"]), int(g[key]["m_pix"])) == (o[key].l_pix, o[key].m_pix), key
+    assert len(set(g) & set(o)) >= min_match
+    assert plan.get_counters()["stats_overflow"] == 0
+    return g
+
+
+@pytest.mark.parametrize("npix,npol,dts", [(256, 2, (1, 2, 4, 8)), (128, 1, (1, 2, 5)), (256, 4, (1, 3)), (64, 4, (2, 4))])
+def test_small_sizes_every_image(npix, npol, dts):
+    """Whole candidate lists at threshold 0 (every image is emitted): npix 256 runs the boxcar tree with two
+    rows per warp, 128 / 64 the exact-statistics kernel; npol 1 and 4; widths on and off the tree."""
+    import torch
+    import paper_1802_03084_b200 as R
+    cfg = W.get_config("tiny")
+    f, uvw = W.channel_freqs_hz(cfg), W.baseline_uvw_m(cfg)
+    cell = W.default_cell_rad(cfg, uvw) * 64 / npix * (1.0 if npix <= 128 else 0.8)
+    nint = 43                                               # ragged: not a multiple of any width or block
+    dms = np.array([0.0, 60.0, 25.0])                       # unsorted trials
+    vis = _rand_vis((nint, cfg.nbl, cfg.nchan, npol), 100 + npix + npol)
+    vis = O.inject_transient(vis, f, uvw, cfg.inttime_s, cell, 1.0, 5, -9, 60.0, 2, 12).astype(np.complex64)
+    plan = R.Plan(f, uvw, npol, nint, cfg.inttime_s, npix, cell, dms, dts, 0.0)
+    g = _compare_all(plan, torch.from_numpy(vis).cuda(), vis, f, uvw, cell, npix, dms, dts, 0.0, cfg.inttime_s,
+                     min_match=20)
+    assert len(g) == plan.num_images()
+    # pixel parity of one image per width through the debug hook
+    delays = O.delay_table(f, dms, cfg.inttime_s)
+    iu, iv, keep = O.cell_table(uvw, f, npix, cell)
+    d = torch.from_numpy(vis).cuda()
+    for k, dt in enumerate(dts):
+        ref = O.search_image(vis, delays, iu, iv, keep, npix, 1, dt, 12 // dt)
+        img, _ = plan.debug_image(d, 1, k, 12 // dt)
+        assert np.abs(img - ref).max() <= PIX_TOL * np.sqrt((ref ** 2).mean()), (npix, dt)
+    plan.destroy()
+
+
+def test_degenerate_plans():
+    """Nothing kept (all channels flagged): zero candidates, zero image, no crash.  A DM whose sweep is
+    longer than the segment contributes no images.  Unsorted channel order gives the same tables as the oracle."""
+    import torch
+    import paper_1802_03084_b200 as R
+    cfg = W.get_config("tiny")
+    f, uvw = W.channel_freqs_hz(cfg), W.baseline_uvw_m(cfg)
+    cell = W.default_cell_rad(cfg, uvw)
+    vis = W.make_segment(cfg)
+    d = torch.from_numpy(vis).cuda()
+    dms = np.array([0.0, 50.0, 400.0])                      # DM 400: max delay 89 > 64 integrations
+    plan = R.Plan(f, uvw, cfg.npol, cfg.nint, cfg.inttime_s, cfg.npix, cell, dms, (1,), cfg.threshold)
+    assert plan.num_t(2, 0) == 0 and plan.num_t(0, 0) == 64 and plan.num_t(1, 0) == 64 - 11
+    gpu, n = plan.search(d)
+    assert n > 0 and (gpu["dm_idx"] < 2).all()
+    plan.set_chan_weights(np.zeros(cfg.nchan, dtype=np.float32))
+    gpu, n = plan.search(d)
+    assert n == 0 and plan.get_counters()["n_kept"] == 0
+    img, st = plan.debug_image(d, 0, 0, 5)
+    assert not img.any() and float(st["snr"]) == 0.0
+    plan.destroy()
+    # channels given in reverse order: tables and candidates follow the caller's order
+    perm = np.arange(cfg.nchan)[::-1].copy()
+    plan = R.Plan(f[perm], uvw, cfg.npol, cfg.nint, cfg.inttime_s, cfg.npix, cell, W.dm_list(cfg), (1,), cfg.threshold)
+    delay, cells, keep = plan.get_tables()
+    assert np.array_equal(delay, O.delay_table(f[perm], W.dm_list(cfg), cfg.inttime_s))
+    vis_p = np.ascontiguousarray(vis[:, :, perm, :])
+    a, _ = plan.search(torch.from_numpy(vis_p).cuda())
+    ref = O.search(vis, f, uvw, cfg.inttime_s, cfg.npix, cell, W.dm_list(cfg), (1,), cfg.threshold)
+    ka = {(int(c["dm_idx"]), int(c["t_idx"])) for c in a}
+    kr = {(c.dm_idx, c.t_idx) for c in ref if abs(c.snr - cfg.threshold) > NEAR_THR * cfg.threshold}
+    assert kr <= ka and len(ka) - len(kr) <= 2
+    plan.destroy()
+
+
+def test_candidate_overflow_keeps_counting():
+    import torch
+    import paper_1802_03084_b200 as R
+    cfg = W.get_config("tiny")
+    f, uvw = W.channel_freqs_hz(cfg), W.baseline_uvw_m(cfg)
+    cell = W.default_cell_rad(cfg, uvw)
+    plan = R.Plan(f, uvw, cfg.npol, cfg.nint, cfg.inttime_s, cfg.npix, cell, W.dm_list(cfg), (1,), 0.0)
+    d = torch.from_numpy(W.make_segment(cfg)).cuda()
+    rec, n = plan.search(d, capacity=10)
+    assert n == plan.num_images() == 388 and len(rec) == 10           # count runs past capacity, items are capped
+    keys = {(int(c["dm_idx"]), int(c["t_idx"])) for c in rec}
+    assert len(keys) == 10 and all(float(c["sigma"]) > 0 for c in rec)
+    plan.destroy()
