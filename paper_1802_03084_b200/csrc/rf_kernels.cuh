@@ -20,6 +20,8 @@ namespace rf {
 struct SearchParams {
     const float* vis;               // complex64 [nint][nbl][nchan][npol] as floats
     const float2* mean_i;           // [nbl*nchan] Stokes-I sum of the time means, or null (no subtraction)
+    const float2* visI;             // [nbl*nchan][tpitch] time-fastest Stokes-I sums (mean already removed), or null
+    int32_t tpitch;
     const int32_t* delay;           // [ndm][nchan]
     const GridEntry* entries;
     const int32_t* warp_chunk;
@@ -121,6 +123,46 @@ __device__ __forceinline__ void gather_grid(const SearchParams& p, float2* __res
     }
 }
 
+// The same gather from the time-fastest Stokes-I array of the boxcar-tree path (when the plan has one):
+// the dt samples of an entry are contiguous (8*dt bytes) instead of dt scattered 16-byte pol pairs.
+template <int PITCH>
+__device__ __forceinline__ void gather_grid_visi(const SearchParams& p, float2* __restrict__ tile,
+                                                 const int* __restrict__ sdelay, int t_first,
+                                                 int c_beg, int c_end, int lane, int dt) {
+    for (int ck = c_beg; ck < c_end; ck++) {
+        const GridEntry e = p.entries[(size_t)ck * 32 + lane];
+        const bool valid = (e.w0 >> 31) != 0;
+        const float2* src = p.visI + (size_t)(e.w0 & 0xffffffu) * p.tpitch + (t_first + sdelay[e.w1 & 0xfff]);
+        float re = 0.f, im = 0.f;
+        if (valid) {
+            int q = 0;
+            for (; q + 8 <= dt; q += 8) {
+                float2 a[8];
+#pragma unroll
+                for (int k = 0; k < 8; k++) a[k] = __ldg(src + q + k);
+#pragma unroll
+                for (int k = 0; k < 8; k++) { re += a[k].x; im += a[k].y; }
+            }
+            for (; q < dt; q++) { const float2 a = __ldg(src + q); re += a.x; im += a.y; }
+        }
+        if (e.w0 & (1u << 30)) im = -im;
+        const int dist = (e.w0 >> 24) & 31;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            float r2 = __shfl_up_sync(0xffffffffu, re, d);
+            float i2 = __shfl_up_sync(0xffffffffu, im, d);
+            if (dist >= d) { re += r2; im += i2; }
+        }
+        if (valid && (e.w0 & (1u << 29))) {
+            const int row = (e.w1 >> 12) & 0xfff, col = (e.w1 >> 24) & 0xf;
+            float2* dst = &tile[col * PITCH + fft_pad(row)];
+            float2 cur = *dst;
+            *dst = make_float2(cur.x + re, cur.y + im);
+        }
+        __syncwarp();
+    }
+}
+
 // ------------------------------------------------------------------------------------------
 // Pass 1.  grid = (n_img, ngroups): group-major launch order, so the heavy central column
 // groups start first (measured faster than image-major order); block = 256.  Dynamic smem:
@@ -150,7 +192,8 @@ __global__ void __launch_bounds__(kThreads) k_grid_colfft(const SearchParams p) 
         const int c_beg = p.warp_chunk[g * kWarpsPerCta + warp];
         const int c_end = p.warp_chunk[g * kWarpsPerCta + warp + 1];
         const float* base = p.vis + (long long)im.j * im.dt * p.row_floats;
-        switch (im.dt) {   // compile-time widths keep U x DT independent 16-byte loads in flight per lane
+        if (p.visI != nullptr) gather_grid_visi<PITCH>(p, tile, sdelay, im.j * im.dt, c_beg, c_end, lane, im.dt);
+        else switch (im.dt) {   // compile-time widths keep U x DT independent 16-byte loads in flight per lane
             case 1: gather_grid<NPOL, 1, 8, PITCH>(p, tile, sdelay, base, c_beg, c_end, lane, 1); break;
             case 2: gather_grid<NPOL, 2, 4, PITCH>(p, tile, sdelay, base, c_beg, c_end, lane, 2); break;
             case 4: gather_grid<NPOL, 4, 2, PITCH>(p, tile, sdelay, base, c_beg, c_end, lane, 4); break;

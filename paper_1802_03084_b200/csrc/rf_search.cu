@@ -103,8 +103,8 @@ int launch_batch(rf_plan* p, const SearchParams& sp, cudaStream_t st) {
 // ---------------------------------------------------------------- boxcar-tree path
 template <int N> int tree_nbins(int tb) { return N <= 1024 ? 2048 : (N == 2048 ? 4096 : (tb == 2 ? 8192 : 4096)); }
 
-template <int N, int TB> size_t smem_tree1(int ncol) {
-    return (size_t)TB * ncol * (fft_padded_size(N) + 1) * sizeof(float2) + FftCfg<N>::TW_TOTAL * sizeof(float2);
+template <int N> size_t smem_tree1(int ntiles) {
+    return (size_t)ntiles * (fft_padded_size(N) + 1) * sizeof(float2) + FftCfg<N>::TW_TOTAL * sizeof(float2);
 }
 template <int N, int TB> size_t smem_tree2(int nbins, int cpad) {
     const size_t g2 = kThreads2 / FftCfg<N>::TPF;
@@ -116,7 +116,7 @@ template <int N, int TB> size_t smem_tree2(int nbins, int cpad) {
 
 // event kinds: 0 = grid + column FFT (generic pass 1 / tree column FFT), 1 = row FFT + statistics,
 // 2 = Stokes-I transpose, 3 = tree gather
-template <int N, int TB, int NCOL>
+template <int N, int TB, int NCOL, int QH>
 int launch_tree(rf_plan* p, const TreeParams& tp, cudaStream_t st) {
     int rc;
     {
@@ -128,14 +128,14 @@ int launch_tree(rf_plan* p, const TreeParams& tp, cudaStream_t st) {
         if ((rc = mark(p, st, 3)) != RF_OK) return rc;
     }
     {
-        auto kern = k_tree_colfft<N, TB, NCOL>;
-        const size_t smem = smem_tree1<N, TB>(NCOL);
+        auto kern = k_tree_colfft<N, TB, NCOL, QH>;
+        const size_t smem = smem_tree1<N>(QH * NCOL);
         static size_t configured = 0;
         if (smem > configured) {
             RF_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             configured = smem;
         }
-        kern<<<dim3(tp.ngroups, tp.n_blk), kThreads, smem, st>>>(tp);
+        kern<<<dim3(tp.ngroups, tp.n_blk, TB / QH), kThreads, smem, st>>>(tp);
         RF_CUDA_CHECK(cudaGetLastError());
         if ((rc = mark(p, st, 0)) != RF_OK) return rc;
     }
@@ -157,12 +157,12 @@ int launch_tree(rf_plan* p, const TreeParams& tp, cudaStream_t st) {
 int launch_tree_batch(rf_plan* p, TreeParams& tp, cudaStream_t st) {
     const int key = p->npix * 16 + p->tree_tb;
     switch (key) {
-#define RF_TCASE(N, TB, NCOL) case N * 16 + TB: tp.nbins = tree_nbins<N>(TB); return launch_tree<N, TB, NCOL>(p, tp, st);
-        RF_TCASE(256, 2, 16) RF_TCASE(256, 4, 8) RF_TCASE(256, 8, 4)
-        RF_TCASE(512, 2, 8) RF_TCASE(512, 4, 4) RF_TCASE(512, 8, 2)
-        RF_TCASE(1024, 2, 4) RF_TCASE(1024, 4, 2) RF_TCASE(1024, 8, 1)
-        RF_TCASE(2048, 2, 2) RF_TCASE(2048, 4, 1)
-        RF_TCASE(4096, 2, 2) RF_TCASE(4096, 4, 1)
+#define RF_TCASE(N, TB, NCOL, QH) case N * 16 + TB: tp.nbins = tree_nbins<N>(TB); return launch_tree<N, TB, NCOL, QH>(p, tp, st);
+        RF_TCASE(256, 2, 16, 2) RF_TCASE(256, 4, 8, 4) RF_TCASE(256, 8, 4, 8)
+        RF_TCASE(512, 2, 8, 2) RF_TCASE(512, 4, 4, 4) RF_TCASE(512, 8, 2, 8)
+        RF_TCASE(1024, 2, 4, 2) RF_TCASE(1024, 4, 2, 4) RF_TCASE(1024, 8, 2, 4)
+        RF_TCASE(2048, 2, 2, 2) RF_TCASE(2048, 4, 2, 2)
+        RF_TCASE(4096, 2, 2, 2) RF_TCASE(4096, 4, 2, 2)
 #undef RF_TCASE
     }
     set_error("unsupported tree configuration npix %d tb %d", p->npix, p->tree_tb);
@@ -261,6 +261,8 @@ SearchParams base_params(rf_plan* p, const void* vis) {
     SearchParams sp{};
     sp.vis = reinterpret_cast<const float*>(vis);
     sp.mean_i = p->meansub ? p->ws.mean_i : nullptr;
+    sp.visI = nullptr;     // set by the caller once the Stokes-I transpose of this segment has been enqueued
+    sp.tpitch = p->tpitch;
     sp.delay = p->d.delay;
     sp.entries = p->d.gen.entries;
     sp.warp_chunk = p->d.gen.warp_chunk;
@@ -373,6 +375,7 @@ int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out
     }
     // ---- every other width: one gridding + transform per image
     SearchParams sp = base_params(p, vis);
+    if (p->tree_tb > 0 && p->n_blocks > 0) sp.visI = p->ws.visI;     // transposed above for the tree path
     sp.cand_items = out->items;
     sp.cand_count = out->count;
     sp.cand_capacity = out->capacity;

@@ -275,9 +275,9 @@ int build_grid_lists(rf_plan* p) {
 // Columns per pass-1 CTA of the tree path: TB x NCOL column tiles of N points must fit ~70 KB
 // of shared memory (139 KB for 4096 x 2).
 int tree_cols_per_group(int npix, int tb) {
-    int ncol = (16 * 512) / (npix * tb);
-    if (npix == 4096 && tb == 2) ncol = 2;
-    return ncol < 1 ? 1 : ncol;
+    if (npix <= 512) return (16 * 512) / (npix * tb);     // TB x NCOL = 16 tiles of 512 (32 of 256): 70 KB
+    if (npix == 1024) return tb == 2 ? 4 : 2;             // 8 tiles of 1024; TB > 4 is split over blockIdx.z
+    return 2;                                             // 4 tiles of 2048 (70 KB) / 4096 (139 KB)
 }
 
 // Loop + segment semantics (readings A6, A16): all j with

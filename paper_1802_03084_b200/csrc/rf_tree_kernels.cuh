@@ -196,23 +196,25 @@ __global__ void __launch_bounds__(kThreads) k_tree_gather(const TreeParams p) {
 // Tree pass 1: column FFTs.  grid = (ngroups, n_blk) -- the column groups of one block run together,
 // so their 32-byte pieces of one H line meet in L2 before the line is written back; block = 256.
 // Dynamic smem:  tile [TB*NCOL][PITCH] float2 (column f = q*NCOL + c) | tw
-// The CTA scatters the cells of its NCOL uv columns from the compact grid into zeroed tiles,
-// transforms the TB*NCOL columns in place (inverse, along v) and stores the half plane.
-template <int N, int TB, int NCOL>
+// The CTA scatters the cells of its NCOL uv columns, for QH of the block's TB integrations
+// (blockIdx.z selects which: QH < TB keeps two columns per CTA when N = 1024, i.e. whole 32-byte
+// sectors in the store), from the compact grid into zeroed tiles, transforms the QH*NCOL columns
+// in place (inverse, along v) and stores the half plane.
+template <int N, int TB, int NCOL, int QH>
 __global__ void __launch_bounds__(kThreads) k_tree_colfft(const TreeParams p) {
     using C = FftCfg<N>;
     constexpr int PITCH = fft_padded_size(N) + 1;
-    constexpr int NF = TB * NCOL;
+    constexpr int NF = QH * NCOL;
     constexpr int KPRE = 3;                // compact-grid values per thread loaded ahead of the tile clear
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2* tile = reinterpret_cast<float2*>(smem_raw);
     float2* tw = tile + NF * PITCH;
 
     const int tid = threadIdx.x;
-    const int g = blockIdx.x, slot = blockIdx.y;
+    const int g = blockIdx.x, slot = blockIdx.y, q0 = blockIdx.z * QH;
     const int c_beg = p.group_cell[g], c_end = p.group_cell[g + 1];
-    const int nval = (c_end - c_beg) * TB;
-    const float2* cs = p.cellsum + ((size_t)slot * p.n_cells + c_beg) * TB;
+    const int nval = (c_end - c_beg) * QH;
+    const float2* cs = p.cellsum + ((size_t)slot * p.n_cells + c_beg) * TB + q0;
     const uint32_t* cm = p.cells + c_beg;
 
     // ---- prologue: every global load of the set-up is issued before the tile is cleared
@@ -225,21 +227,21 @@ __global__ void __launch_bounds__(kThreads) k_tree_colfft(const TreeParams p) {
         const int i = tid + k * kThreads;
         pv[k] = make_float2(0.f, 0.f);
         pm[k] = 0u;
-        if (i < nval) { pv[k] = cs[i]; pm[k] = cm[i / TB]; }
+        if (i < nval) { pv[k] = cs[(i / QH) * TB + i % QH]; pm[k] = cm[i / QH]; }
     }
     for (int i = tid; i < NF * PITCH; i += kThreads) tile[i] = make_float2(0.f, 0.f);
     if (tid < C::TW_TOTAL) tw[tid] = tw0;
     if (tid + kThreads < C::TW_TOTAL) tw[tid + kThreads] = tw1;
     __syncthreads();
-    // ---- scatter the cells of these columns: value i = (cell i / TB, integration i % TB)
+    // ---- scatter the cells of these columns: value i = (cell i / QH, integration q0 + i % QH)
 #pragma unroll
     for (int k = 0; k < KPRE; k++) {
         const int i = tid + k * kThreads;
-        if (i < nval) tile[((i % TB) * NCOL + ((pm[k] >> 12) & 0xf)) * PITCH + fft_pad(pm[k] & 0xfff)] = pv[k];
+        if (i < nval) tile[((i % QH) * NCOL + ((pm[k] >> 12) & 0xf)) * PITCH + fft_pad(pm[k] & 0xfff)] = pv[k];
     }
     for (int i = tid + KPRE * kThreads; i < nval; i += kThreads) {
-        const uint32_t m = cm[i / TB];
-        tile[((i % TB) * NCOL + ((m >> 12) & 0xf)) * PITCH + fft_pad(m & 0xfff)] = cs[i];
+        const uint32_t m = cm[i / QH];
+        tile[((i % QH) * NCOL + ((m >> 12) & 0xf)) * PITCH + fft_pad(m & 0xfff)] = cs[(i / QH) * TB + i % QH];
     }
     __syncthreads();
 
@@ -265,7 +267,7 @@ __global__ void __launch_bounds__(kThreads) k_tree_colfft(const TreeParams p) {
     //      one Hermitian pair transform are adjacent (one 16-byte store), and one (row, pair) is
     //      contiguous for pass 2
     {
-        constexpr int SEG = NCOL * TB / 2;
+        constexpr int SEG = NCOL * QH / 2;
         float4* Hs = reinterpret_cast<float4*>(p.Ht + (size_t)slot * N * p.cpad * TB);
         const int i = tid % SEG, pr = i / NCOL, c = i % NCOL, y0 = tid / SEG;
         const float2* ta = tile + (2 * pr * NCOL + c) * PITCH;
@@ -275,7 +277,7 @@ __global__ void __launch_bounds__(kThreads) k_tree_colfft(const TreeParams p) {
 #endif
         for (int y = y0; y < N; y += kThreads / SEG) {
             const float2 a = ta[fft_pad(y)], b = tb[fft_pad(y)];
-            Hs[((size_t)y * (TB / 2) + pr) * p.cpad + g * NCOL + c] = make_float4(a.x, a.y, b.x, b.y);
+            Hs[((size_t)y * (TB / 2) + q0 / 2 + pr) * p.cpad + g * NCOL + c] = make_float4(a.x, a.y, b.x, b.y);
         }
     }
 }
