@@ -11,6 +11,11 @@ from .realfast_oracle import (  # noqa: F401
     mean_subtract,
     candidate_spectrum,
     inject_transient,
+    periodicity_nt,
+    periodicity_spectrum,
+    periodicity_image,
+    periodicity_stats,
+    periodicity_search,
     delay_table,
     cell_table,
     dedisperse_resample,

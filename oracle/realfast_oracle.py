@@ -14,6 +14,7 @@ are DESIGN.md "Readings", taken from SURVEY.md section 8(c)).
     O7  threshold              PAPER.md:88 ("S/N greater than a threshold")
     O8  candidate cut-out: image + phased, dedispersed spectrum
     O9  mock-transient injection
+    O10 periodicity search: Fourier transform in time, image each frequency   PAPER.md:100 (footnote 4), 104
 
 Pins (tests/test_oracle_pins.py): every function below is pinned to something
 other than itself -- closed forms, exact rational arithmetic, a direct DFT,
@@ -235,6 +236,83 @@ def inject_transient(vis: np.ndarray, freqs_hz, uvw_m, inttime_s: float, cell_ra
             if 0 <= t < nint:
                 out[t, :, c, :] += sig[:, c, None]
     return out
+
+
+# --------------------------------------------------------------------------- O10
+LN2 = 0.6931471805599453
+
+
+def periodicity_nt(nint: int, max_delay: int) -> int:
+    """Length of the time transform of one DM trial: the largest power of two <= nint - max_delay
+    (0 when that is below 64)."""
+    n = nint - max_delay
+    if n < 64:
+        return 0
+    return 1 << (int(n).bit_length() - 1)
+
+
+def periodicity_spectrum(vis: np.ndarray, delay_dm: np.ndarray, nt: int) -> np.ndarray:
+    """complex128 [nt][nbl][nchan]: S[k] = (1/nt) sum_t s[t] e^{-2 pi i k t / nt} of the dedispersed
+    Stokes-I series s[t][bl][ch] = mean_pol vis[t + delay[ch]][bl][ch][pol], t < nt ("reading a time
+    segment, transforming it to frequencies with a Fourier transform", PAPER.md:100 footnote 4)."""
+    nint, nbl, nchan, npol = vis.shape
+    s = np.empty((nt, nbl, nchan), dtype=np.complex128)
+    for c in range(nchan):
+        d = int(delay_dm[c])
+        s[:, :, c] = vis[d:d + nt, :, c, :].astype(np.complex128).mean(axis=2)
+    return np.fft.fft(s, axis=0) / nt
+
+
+def periodicity_image(spec_k: np.ndarray, iu: np.ndarray, iv: np.ndarray, keep: np.ndarray, npix: int) -> np.ndarray:
+    """complex128 [npix][npix]: I_k[y][x] = (1/N_w) sum_kept S[k][bl][ch] e^{+2 pi i (iu x + iv y)/N}
+    ("imaging each frequency", footnote 4).  S[k] is not the visibility of a real sky, so there is no
+    Hermitian completion: the image is complex and its POWER |I_k|^2 is searched (reading A23)."""
+    g = np.zeros((npix, npix), dtype=np.complex128)
+    np.add.at(g, (iv[keep].astype(np.int64) % npix, iu[keep].astype(np.int64) % npix), spec_k[keep])
+    return np.fft.ifft2(g) * (npix * npix) / int(keep.sum())
+
+
+def periodicity_stats(power: np.ndarray):
+    """(peak_amp, y, x, sigma, snr) of one power image: peak_amp = sqrt(max P) (first maximum in
+    row-major order), sigma = sqrt(median(P) / ln 2) -- the rms amplitude of a complex Gaussian field
+    whose power has that median (P is exponentially distributed on noise) --, snr = peak_amp / sigma
+    (reading A23; the estimator is this build's choice: parity unpinned by the paper)."""
+    flat = power.reshape(-1)
+    k = int(np.argmax(flat))
+    y, x = divmod(k, power.shape[1])
+    med = float(np.median(flat))
+    sigma = float(np.sqrt(med / LN2))
+    amp = float(np.sqrt(flat[k]))
+    return amp, y, x, sigma, (amp / sigma if sigma > 0.0 else 0.0)
+
+
+def periodicity_search(vis: np.ndarray, freqs_hz, uvw_m, inttime_s: float, npix: int, cell_rad: float,
+                       dm_list, threshold: float, chan_weights: Optional[np.ndarray] = None,
+                       keys: Optional[Iterable[Tuple[int, int]]] = None, return_all_stats: bool = False):
+    """Periodicity search of one segment: for every DM trial and every positive
+    fluctuation frequency k = 1 .. nt/2 image S[k] and threshold the power image.  Candidates carry
+    dt_idx = -1 and t_idx = k; order (dm, k)."""
+    nint = vis.shape[0]
+    delays = delay_table(freqs_hz, dm_list, inttime_s)
+    iu, iv, keep = cell_table(uvw_m, freqs_hz, npix, cell_rad, chan_weights)
+    want = None if keys is None else set(keys)
+    cands: List[Candidate] = []
+    stats = {}
+    for d in range(len(dm_list)):
+        nt = periodicity_nt(nint, int(delays[d].max()))
+        ks = [k for k in range(1, nt // 2 + 1) if want is None or (d, k) in want]
+        if not ks or not keep.any():
+            continue
+        spec = periodicity_spectrum(vis, delays[d], nt)
+        for k in ks:
+            img = periodicity_image(spec[k], iu, iv, keep, npix)
+            amp, y, x, sigma, snr = periodicity_stats(img.real ** 2 + img.imag ** 2)
+            if return_all_stats:
+                stats[(d, k)] = (amp, y, x, sigma, snr)
+            if snr >= threshold:
+                cands.append(Candidate(d, -1, k, x if x < npix // 2 else x - npix, y if y < npix // 2 else y - npix,
+                                       amp, sigma, snr))
+    return (cands, stats) if return_all_stats else cands
 
 
 # --------------------------------------------------------------------------- O3-O7
