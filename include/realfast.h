@@ -190,6 +190,27 @@ int rf_cand_spectrum(rf_plan* plan, const void* vis_dev, int dm_idx, int dt_idx,
 int rf_inject(rf_plan* plan, void* vis_dev, double amp, double l_pix, double m_pix, double dm,
               int width, int t0, void* cuda_stream);
 
+/* Periodicity search ("a periodicity search requires reading a time segment,
+ * transforming it to frequencies with a Fourier transform, and imaging each frequency"
+ * footnote 4; "a modification of the innermost iteration loop"; reading A23).  For every DM
+ * trial: NT = rf_plan_periodic_nt(plan, dm_idx) = the largest power of two <= nint - maxdelay(dm) (0 = the
+ * trial is skipped when that is below 64; capped at 4096);
+ *   S[k][bl][ch] = (1/NT) sum_{t<NT} s[t] e^{-2 pi i k t/NT},  s[t] = Stokes-I mean of vis[t + delay[dm][ch]],
+ * and for every positive fluctuation frequency k = 1..NT/2 the COMPLEX image
+ *   I_k[y][x] = (1/N_w) sum_kept S[k] e^{+2 pi i (iu x + iv y)/npix}    (no Hermitian completion)
+ * is searched in power P = |I_k|^2: peak = sqrt(max P) (first maximum in row-major order), sigma =
+ * sqrt(median(P)/ln 2), snr = peak/sigma.  Candidates with snr >= threshold are appended to cand_out with
+ * dt_idx = -1 and t_idx = k (fluctuation frequency k/(NT inttime) Hz).  Honours rf_plan_set_meansub and
+ * the channel weights; ignores the search span.  Needs a plan on the boxcar-tree kernels (npix 256..1024
+ * and a power-of-two width <= 8 in dt_list), else RF_ERR_STATE.  Enqueues on cuda_stream; one host
+ * synchronisation at entry (block-list upload), none after the first kernel.
+ *   rf_debug_periodic_image: power image [npix][npix] (float32, DEVICE) and/or statistics of one
+ *   (dm_idx, k), through the same kernels.                                                          */
+int rf_search_periodic(rf_plan* plan, const void* vis_dev, void* cuda_stream, rf_cand_out* cand_out);
+int rf_plan_periodic_nt(const rf_plan* plan, int dm_idx);
+int rf_debug_periodic_image(rf_plan* plan, const void* vis_dev, int dm_idx, int k,
+                            float* power_dev, rf_cand* stats_dev, void* cuda_stream);
+
 /* Thread-local description of the last error returned on this thread. */
 const char* rf_last_error(void);
 

@@ -22,6 +22,7 @@ EXPORTS = [
     "rf_debug_image", "rf_plan_get_counters", "rf_plan_set_batch", "rf_last_error",
     "rf_search_host", "rf_plan_set_profiling", "rf_plan_get_kernel_times", "rf_plan_set_mode",
     "rf_plan_set_meansub", "rf_prep_meansub", "rf_cand_spectrum", "rf_inject",
+    "rf_search_periodic", "rf_plan_periodic_nt", "rf_debug_periodic_image",
 ]
 
 # numpy view of rf_cand (32 bytes)
@@ -81,6 +82,9 @@ def load_library() -> C.CDLL:
     lib.rf_prep_meansub.argtypes = [vp, vp, vp]
     lib.rf_inject.argtypes = [vp, vp, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int, C.c_int, vp]
     lib.rf_cand_spectrum.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, vp, vp]
+    lib.rf_search_periodic.argtypes = [vp, vp, vp, C.POINTER(_CandOut)]
+    lib.rf_plan_periodic_nt.argtypes = [vp, C.c_int]
+    lib.rf_debug_periodic_image.argtypes = [vp, vp, C.c_int, C.c_int, vp, vp, vp]
     for name in EXPORTS:
         if name not in ("rf_plan_num_images", "rf_last_error"):
             getattr(lib, name).restype = C.c_int
@@ -258,5 +262,35 @@ class Plan:
         stats = torch.zeros(32, dtype=torch.uint8, device=vis.device)
         _check(self._lib.rf_debug_image(self._h, vis.data_ptr(), dm_idx, dt_idx, t_idx, img.data_ptr(),
                                         stats.data_ptr(), st.cuda_stream))
+        st.synchronize()
+        return img.cpu().numpy(), stats.cpu().numpy().view(CAND_DTYPE)[0].copy()
+
+    def periodic_nt(self, dm_idx: int) -> int:
+        """rf_plan_periodic_nt: length of the time transform of one DM trial (0 = trial skipped)."""
+        return int(self._lib.rf_plan_periodic_nt(self._h, dm_idx))
+
+    def search_periodic(self, vis, capacity: int = 1 << 16, stream=None):
+        """rf_search_periodic: candidates (dt_idx = -1, t_idx = fluctuation-frequency bin k) and their count."""
+        import torch
+        assert vis.is_cuda and vis.dtype == torch.complex64 and vis.is_contiguous()
+        assert tuple(vis.shape) == (self.nint, self.nbl, self.nchan, self.npol), tuple(vis.shape)
+        st = torch.cuda.current_stream(vis.device) if stream is None else stream
+        items = torch.empty(max(1, capacity) * 32, dtype=torch.uint8, device=vis.device)
+        count = torch.zeros(1, dtype=torch.int32, device=vis.device)
+        out = _CandOut(items.data_ptr(), capacity, count.data_ptr())
+        _check(self._lib.rf_search_periodic(self._h, vis.data_ptr(), st.cuda_stream, C.byref(out)))
+        st.synchronize()
+        n = int(count.item())
+        return items[: min(n, capacity) * 32].cpu().numpy().view(CAND_DTYPE).copy(), n
+
+    def debug_periodic_image(self, vis, dm_idx: int, k: int, stream=None):
+        """Returns (power image float32 [npix][npix] numpy, stats record) of one (dm, k)."""
+        import torch
+        assert vis.is_cuda and vis.dtype == torch.complex64 and vis.is_contiguous()
+        st = torch.cuda.current_stream(vis.device) if stream is None else stream
+        img = torch.empty((self.npix, self.npix), dtype=torch.float32, device=vis.device)
+        stats = torch.zeros(32, dtype=torch.uint8, device=vis.device)
+        _check(self._lib.rf_debug_periodic_image(self._h, vis.data_ptr(), dm_idx, k, img.data_ptr(),
+                                                 stats.data_ptr(), st.cuda_stream))
         st.synchronize()
         return img.cpu().numpy(), stats.cpu().numpy().view(CAND_DTYPE)[0].copy()

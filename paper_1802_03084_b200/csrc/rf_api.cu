@@ -248,6 +248,30 @@ int rf_inject(rf_plan* p, void* vis_dev, double amp, double l_pix, double m_pix,
     return rf::launch_inject(p, vis_dev, amp, l_pix, m_pix, dm, width, t0, static_cast<cudaStream_t>(cuda_stream));
 }
 
+int rf_search_periodic(rf_plan* p, const void* vis_dev, void* cuda_stream, rf_cand_out* out) {
+    if (!p || !vis_dev || !out || !out->count || (out->capacity > 0 && !out->items) || out->capacity < 0) {
+        set_error("null pointer argument");
+        return RF_ERR_ARG;
+    }
+    if (reinterpret_cast<uintptr_t>(vis_dev) & 15) { set_error("vis_dev must be 16-byte aligned"); return RF_ERR_ARG; }
+    return rf::launch_search_periodic(p, vis_dev, static_cast<cudaStream_t>(cuda_stream), out, -1, 0, nullptr, nullptr);
+}
+
+int rf_plan_periodic_nt(const rf_plan* p, int dm_idx) {
+    if (!p || dm_idx < 0 || dm_idx >= p->ndm) return RF_ERR_ARG;
+    return rf::periodic_nt(p, dm_idx);
+}
+
+int rf_debug_periodic_image(rf_plan* p, const void* vis_dev, int dm_idx, int k, float* power_dev, rf_cand* stats_dev,
+                            void* cuda_stream) {
+    if (!p || !vis_dev) { set_error("null pointer argument"); return RF_ERR_ARG; }
+    if (dm_idx < 0 || dm_idx >= p->ndm) { set_error("trial index out of range"); return RF_ERR_STATE; }
+    const int nt = rf::periodic_nt(p, dm_idx);
+    if (k < 1 || k > nt / 2) { set_error("fluctuation-frequency bin out of range"); return RF_ERR_STATE; }
+    return rf::launch_search_periodic(p, vis_dev, static_cast<cudaStream_t>(cuda_stream), nullptr, dm_idx, k, power_dev,
+                                      stats_dev);
+}
+
 int rf_plan_get_counters(rf_plan* p, rf_counters* out) {
     if (!p || !out) { set_error("null pointer argument"); return RF_ERR_ARG; }
     int32_t c[4] = {0, 0, 0, 0};

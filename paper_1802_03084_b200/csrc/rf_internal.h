@@ -115,6 +115,14 @@ struct Workspace {
     BlockDesc* dbg_block = nullptr;
     int blk_batch = 0;
     size_t visI_elems = 0, ht_elems = 0, cs_elems = 0, ss_elems = 0;
+    // periodicity search
+    float2* slab = nullptr;          // [n_slabs][nbl*nchan][slab_pitch] time spectra as (S, -i S) pairs
+    size_t slab_elems = 0;
+    int n_slabs = 0, slab_pitch = 0;
+    BlockDesc* pblocks = nullptr;    // block list of the periodicity search
+    size_t pblocks_cap = 0;
+    int32_t* zero_delay = nullptr;   // [nchan] zeros: the slabs are already dedispersed
+    float2* time_tw = nullptr;       // [7][16 + 256] twiddles of the time transforms, NT = 64 << i
     // prep (mean-visibility subtraction)
     double2* mean_partial = nullptr; // [kMeanChunks][nbl*nchan*npol]
     float2* mean_p = nullptr;        // [nbl*nchan*npol] time mean per polarisation product
@@ -191,4 +199,7 @@ void free_workspace(rf_plan* p);
 int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out);
 int launch_debug_image(rf_plan* p, const void* vis, int dm_idx, int dt_idx, int t_idx,
                        float* image_dev, rf_cand* stats_dev, cudaStream_t st);
+int periodic_nt(const rf_plan* p, int dm_idx);   // length of the time transform of one DM trial (0 = none)
+int launch_search_periodic(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out, int dbg_dm, int dbg_k,
+                           float* power_dev, rf_cand* stats_dev);
 }  // namespace rf

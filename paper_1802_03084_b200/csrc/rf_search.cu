@@ -139,6 +139,18 @@ int launch_tree(rf_plan* p, const TreeParams& tp, cudaStream_t st) {
         RF_CUDA_CHECK(cudaGetLastError());
         if ((rc = mark(p, st, 0)) != RF_OK) return rc;
     }
+    if (tp.zero_row >= 0) {    // periodicity search: every pair is one complex image, searched in power
+        auto kern = k_tree_rowfft_power<N, TB>;
+        const size_t smem = smem_tree2<N, TB>(tp.nbins, tp.cpad);
+        static size_t configured = 0;
+        if (smem > configured) {
+            RF_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            configured = smem;
+        }
+        kern<<<dim3(tp.n_blk), kThreads2, smem, st>>>(tp);
+        RF_CUDA_CHECK(cudaGetLastError());
+        return mark(p, st, 1);
+    }
     {
         auto kern = k_tree_rowfft_stats<N, TB>;
         const size_t smem = smem_tree2<N, TB>(tp.nbins, tp.cpad);
@@ -203,6 +215,8 @@ TreeParams tree_params(rf_plan* p) {
     tp.sumsq = p->ws.sumsq_t;
     tp.counters = p->ws.counters;
     tp.dbg_img = -1;
+    tp.zero_row = -1;
+    tp.slab_stride = 0;
     tp.tpitch = p->tpitch;
     tp.nchan = p->nchan;
     tp.ncol = p->ncol;
@@ -294,6 +308,7 @@ void free_workspace(rf_plan* p) {
     cudaFree(w.ticket); cudaFree(w.counters); cudaFree(w.dbg_desc);
     cudaFree(w.visI); cudaFree(w.Ht); cudaFree(w.sumsq_t); cudaFree(w.cellsum); cudaFree(w.dbg_block);
     cudaFree(w.mean_partial); cudaFree(w.mean_p); cudaFree(w.mean_i);
+    cudaFree(w.slab); cudaFree(w.pblocks); cudaFree(w.zero_delay); cudaFree(w.time_tw);
     w = Workspace{};
 }
 
@@ -428,6 +443,174 @@ int launch_debug_image(rf_plan* p, const void* vis, int dm_idx, int dt_idx, int 
         return RF_OK;
     }
     return launch_batch(p, sp, st);
+}
+
+// ---------------------------------------------------------------- periodicity search (8f-3)
+// Per DM trial: time transform of the dedispersed Stokes-I series of every (baseline, channel) into a
+// slab of (S[k], -i S[k]) pairs, then the gather / column-FFT kernels of the boxcar-tree path on the slab
+// (zero delays: it is already dedispersed) and the power variant of the row pass.  DM trials are taken in
+// chunks of n_slabs so that a chunk fills the GPU for several waves.
+int periodic_nt(const rf_plan* p, int dm_idx) {
+    const int n = p->nint - p->h_maxdelay[dm_idx];
+    if (n < 64) return 0;
+    int nt = 64;
+    while (nt * 2 <= n && nt < 4096) nt *= 2;
+    return nt;
+}
+
+namespace {
+
+template <int NT>
+int launch_time_fft(rf_plan* p, const int32_t* delay_dm, const float2* tw, float2* slab, cudaStream_t st) {
+    constexpr int G = kThreads / FftCfg<NT>::TPF;
+    auto kern = k_time_fft<NT>;
+    const size_t smem = ((size_t)G * fft_padded_size(NT) + FftCfg<NT>::TW_TOTAL) * sizeof(float2);
+    static size_t configured = 0;
+    if (smem > configured) {
+        RF_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured = smem;
+    }
+    const int nelem = p->nbl * p->nchan;
+    kern<<<(nelem + G - 1) / G, kThreads, smem, st>>>(p->ws.visI, delay_dm, tw, slab, nelem, p->nchan, p->tpitch,
+                                                       p->ws.slab_pitch);
+    RF_CUDA_CHECK(cudaGetLastError());
+    return RF_OK;
+}
+
+int launch_time_fft_nt(rf_plan* p, int nt, int dm_idx, int slab_idx, cudaStream_t st) {
+    int lg = 0;
+    while ((64 << lg) < nt) lg++;
+    const float2* tw = p->ws.time_tw + (size_t)lg * (16 + 256);
+    const int32_t* dd = p->d.delay + (size_t)dm_idx * p->nchan;
+    float2* slab = p->ws.slab + (size_t)slab_idx * p->nbl * p->nchan * p->ws.slab_pitch;
+    switch (nt) {
+        case 64: return launch_time_fft<64>(p, dd, tw, slab, st);
+        case 128: return launch_time_fft<128>(p, dd, tw, slab, st);
+        case 256: return launch_time_fft<256>(p, dd, tw, slab, st);
+        case 512: return launch_time_fft<512>(p, dd, tw, slab, st);
+        case 1024: return launch_time_fft<1024>(p, dd, tw, slab, st);
+        case 2048: return launch_time_fft<2048>(p, dd, tw, slab, st);
+        case 4096: return launch_time_fft<4096>(p, dd, tw, slab, st);
+    }
+    set_error("unsupported time-transform length %d", nt);
+    return RF_ERR_ARG;
+}
+
+int ensure_periodic_workspace(rf_plan* p, int nt_max, int n_dm_live) {
+    Workspace& w = p->ws;
+    const size_t per_slab = (size_t)p->nbl * p->nchan * nt_max;
+    const size_t budget = (size_t)6 << 30;
+    int n_slabs = (int)std::min<size_t>(8, std::max<size_t>(1, budget / (per_slab * sizeof(float2))));
+    n_slabs = std::max(1, std::min(n_slabs, n_dm_live));
+    if (!w.slab || w.slab_elems < per_slab * n_slabs) {
+        cudaFree(w.slab); w.slab = nullptr;
+        RF_CUDA_CHECK(cudaMalloc((void**)&w.slab, per_slab * n_slabs * sizeof(float2)));
+        w.slab_elems = per_slab * n_slabs;
+    }
+    w.n_slabs = n_slabs;
+    w.slab_pitch = nt_max;
+    if (!w.zero_delay) {
+        RF_CUDA_CHECK(cudaMalloc((void**)&w.zero_delay, (size_t)p->nchan * sizeof(int32_t)));
+        RF_CUDA_CHECK(cudaMemset(w.zero_delay, 0, (size_t)p->nchan * sizeof(int32_t)));
+    }
+    if (!w.time_tw) {
+        std::vector<float2> tw((size_t)7 * (16 + 256));
+        for (int i = 0; i < 7; i++) host_twiddles(64 << i, tw.data() + (size_t)i * (16 + 256));
+        RF_CUDA_CHECK(cudaMalloc((void**)&w.time_tw, tw.size() * sizeof(float2)));
+        RF_CUDA_CHECK(cudaMemcpy(w.time_tw, tw.data(), tw.size() * sizeof(float2), cudaMemcpyHostToDevice));
+    }
+    return RF_OK;
+}
+
+}  // namespace
+
+// dbg_dm >= 0: debug hook -- only image (dbg_dm, dbg_k), power image and statistics written out.
+int launch_search_periodic(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out, int dbg_dm, int dbg_k,
+                           float* power_dev, rf_cand* stats_dev) {
+    if (p->tree_tb == 0) {
+        set_error("the periodicity search runs on the boxcar-tree kernels: the plan needs npix in 256..1024 and "
+                  "a power-of-two width <= 8 in dt_list");
+        return RF_ERR_STATE;
+    }
+    int rc = ensure_workspace(p);
+    if (rc == RF_OK) rc = ensure_tree_workspace(p);
+    if (rc != RF_OK) return rc;
+    const bool dbg = dbg_dm >= 0;
+    const int TB = p->tree_tb, nimg = TB / 2;
+    std::vector<int> dms;                       // DM trials with a time transform, in this call
+    int nt_max = 0;
+    for (int d = 0; d < p->ndm; d++) {
+        if (dbg && d != dbg_dm) continue;
+        const int nt = periodic_nt(p, d);
+        if (nt > 0) { dms.push_back(d); nt_max = std::max(nt_max, nt); }
+    }
+    if (out) RF_CUDA_CHECK(cudaMemsetAsync(out->count, 0, sizeof(int32_t), st));
+    RF_CUDA_CHECK(cudaMemsetAsync(p->ws.counters, 0, 4 * sizeof(int32_t), st));
+    p->last_launches = 0;
+    p->n_events_used = 0;
+    if (dms.empty() || p->n_kept == 0) {
+        if (power_dev) RF_CUDA_CHECK(cudaMemsetAsync(power_dev, 0, (size_t)p->npix * p->npix * sizeof(float), st));
+        if (stats_dev) RF_CUDA_CHECK(cudaMemsetAsync(stats_dev, 0, sizeof(rf_cand), st));
+        return RF_OK;
+    }
+    if ((rc = ensure_periodic_workspace(p, nt_max, (int)dms.size())) != RF_OK) return rc;
+    Workspace& w = p->ws;
+    // block list of the whole call, uploaded before the first kernel (chunk c = DM trials c*n_slabs ...)
+    std::vector<BlockDesc> blocks;
+    std::vector<size_t> chunk_first;
+    for (size_t c0 = 0; c0 < dms.size(); c0 += w.n_slabs) {
+        chunk_first.push_back(blocks.size());
+        const size_t c1 = std::min(dms.size(), c0 + w.n_slabs);
+        for (size_t i = c0; i < c1; i++) {
+            const int nt = periodic_nt(p, dms[i]);
+            for (int tb = 0; tb < nt / TB; tb++) {
+                if (dbg && tb != (dbg_k - 1) / nimg) continue;
+                blocks.push_back({dms[i], tb, nt, (int)(i - c0)});
+            }
+        }
+    }
+    chunk_first.push_back(blocks.size());
+    if (!w.pblocks || w.pblocks_cap < blocks.size()) {
+        cudaFree(w.pblocks); w.pblocks = nullptr;
+        RF_CUDA_CHECK(cudaMalloc((void**)&w.pblocks, blocks.size() * sizeof(BlockDesc)));
+        w.pblocks_cap = blocks.size();
+    }
+    RF_CUDA_CHECK(cudaMemcpyAsync(w.pblocks, blocks.data(), blocks.size() * sizeof(BlockDesc), cudaMemcpyHostToDevice, st));
+    RF_CUDA_CHECK(cudaStreamSynchronize(st));      // `blocks` lives on this stack frame
+    if (p->meansub) {
+        if ((rc = launch_time_mean(p, vis, st)) != RF_OK) return rc;
+        p->last_launches += 2;
+    }
+    if ((rc = launch_prep(p, vis, st)) != RF_OK) return rc;
+    p->last_launches += 1;
+    TreeParams tp = tree_params(p);
+    tp.visI = w.slab;
+    tp.delay = w.zero_delay;
+    tp.zero_row = 0;
+    tp.tpitch = w.slab_pitch;
+    tp.slab_stride = (long long)p->nbl * p->nchan * w.slab_pitch;
+    tp.cand_items = out ? out->items : nullptr;
+    tp.cand_count = out ? out->count : nullptr;
+    tp.cand_capacity = out ? out->capacity : 0;
+    if (dbg) {
+        tp.image_out = power_dev;
+        tp.stats_out = stats_dev;
+        tp.dbg_img = (dbg_k - 1) % nimg;
+    }
+    for (size_t c = 0; c + 1 < chunk_first.size(); c++) {
+        const size_t c0 = c * w.n_slabs, c1 = std::min(dms.size(), c0 + w.n_slabs);
+        for (size_t i = c0; i < c1; i++) {
+            if ((rc = launch_time_fft_nt(p, periodic_nt(p, dms[i]), dms[i], (int)(i - c0), st)) != RF_OK) return rc;
+            p->last_launches += 1;
+        }
+        for (size_t base = chunk_first[c]; base < chunk_first[c + 1]; base += w.blk_batch) {
+            tp.blocks = w.pblocks + base;
+            tp.n_blk = (int)std::min<size_t>(w.blk_batch, chunk_first[c + 1] - base);
+            if ((rc = launch_tree_batch(p, tp, st)) != RF_OK) return rc;
+            p->last_launches += 3;
+        }
+    }
+    return RF_OK;
 }
 
 }  // namespace rf

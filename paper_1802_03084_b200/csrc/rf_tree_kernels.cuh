@@ -44,6 +44,8 @@ struct TreeParams {
     rf_cand* stats_out;
     int32_t dbg_img;                // -1 = off
     int32_t tpitch, nchan, ncol, cpad, ngroups, nbins, n_blk, n_cells, n_streams, n_parts;
+    int32_t zero_row;               // >= 0: periodicity mode, every block uses this (all-zero) delay row
+    long long slab_stride;          // periodicity mode: visI is [slab][nbl*nchan][tpitch], block.pad = slab
     int32_t dt_idx[4];              // tree level -> index in dt_list, or -1
     float norm;                     // 1 / (2 N_w npol)
     float threshold;
@@ -119,7 +121,7 @@ __global__ void __launch_bounds__(kThreads) k_tree_gather(const TreeParams p) {
     const int it_beg = has ? p.stream_iter[s] : 0;
     const int it_end = has ? p.stream_iter[s + 1] : 0;
     int cell = has ? p.stream_cell[s] : 0;
-    const int32_t* drow = p.delay + (size_t)blk.dm_idx * p.nchan;
+    const int32_t* drow = p.delay + (size_t)(p.zero_row >= 0 ? p.zero_row : blk.dm_idx) * p.nchan;
     uint32_t en[U];                        // entries of the next batch of iterations (prefetched)
 #pragma unroll
     for (int u = 0; u < U; u++) en[u] = 0u;
@@ -133,7 +135,7 @@ __global__ void __launch_bounds__(kThreads) k_tree_gather(const TreeParams p) {
     float ps[LEVELS];
 #pragma unroll
     for (int l = 0; l < LEVELS; l++) ps[l] = 0.f;
-    const float2* vbase = p.visI + blk.tb * TB + q;
+    const float2* vbase = p.visI + (size_t)blk.pad * p.slab_stride + blk.tb * TB + q;
     float2* cs = p.cellsum + (size_t)slot * p.n_cells * TB + q;
     float2 acc = make_float2(0.f, 0.f);
 #ifdef RF_EXP_NOGATHER
@@ -535,6 +537,209 @@ __global__ void __launch_bounds__(kThreads2, 1) k_tree_rowfft_stats(const TreePa
                     int idx = atomicAdd(p.cand_count, 1);
                     if (idx < p.cand_capacity) p.cand_items[idx] = c;
                 }
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// ==========================================================================================
+// Periodicity search ("reading a time segment, transforming it to frequencies with a
+// Fourier transform, and imaging each frequency", PAPER.md:100 footnote 4; reading A23).
+//
+// k_time_fft<NT>: for one DM trial, S[k] = (1/NT) sum_t s[t] e^{-2 pi i k t/NT} of the dedispersed Stokes-I
+// series of every (baseline, channel), written for k = 1..NT/2 as the PAIR (S[k], -i S[k]) at
+// "integrations" 2(k-1), 2(k-1)+1 of a visI-shaped slab.  Hermitian imaging of S gives Re I_k and of -i S
+// gives Im I_k (I_k = the complex image of S[k]), so the unchanged gather / column-FFT kernels and the pair
+// transform of the row pass deliver the complex image of every fluctuation frequency.
+// grid = ceil(nelem / G) with G = 256 / (NT/16) transforms per CTA; smem: G exchange buffers | twiddles.
+template <int NT>
+__global__ void __launch_bounds__(kThreads) k_time_fft(const float2* __restrict__ visI, const int32_t* __restrict__ delay_dm,
+                                                       const float2* __restrict__ twiddles, float2* __restrict__ slab,
+                                                       int nelem, int nchan, int tpitch_in, int tpitch_out) {
+    using C = FftCfg<NT>;
+    constexpr int G = kThreads / C::TPF;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2* xbuf = reinterpret_cast<float2*>(smem_raw);
+    float2* tw = xbuf + G * fft_padded_size(NT);
+    const int tid = threadIdx.x, grp = tid / C::TPF, t = tid % C::TPF;
+    load_twiddles<NT>(tw, twiddles, tid, kThreads);
+    __syncthreads();
+    const int e = blockIdx.x * G + grp;
+    const bool live = e < nelem;
+    const int ee = live ? e : nelem - 1;             // idle groups repeat the last element (barriers stay uniform)
+    const float2* src = visI + (size_t)ee * tpitch_in + delay_dm[ee % nchan];
+    float2 v[16];
+#pragma unroll
+    for (int k = 0; k < 16; k++) { const float2 x = __ldg(src + t + C::TPF * k); v[k] = make_float2(x.x, -x.y); }
+    fft_inverse<NT>(v, xbuf + grp * fft_padded_size(NT), tw, t, 1 + grp);     // forward = conj(inverse(conj))
+    if (!live) return;
+    const float sc = 1.f / (float)NT;
+    float4* dst = reinterpret_cast<float4*>(slab + (size_t)e * tpitch_out);
+#pragma unroll
+    for (int k = 0; k < 16; k++) {
+        const int kk = t + C::TPF * k;                // natural order: fluctuation-frequency bin
+        if (kk >= 1 && kk <= NT / 2) {
+            const float re = v[k].x * sc, im = -v[k].y * sc;
+            dst[kk - 1] = make_float4(re, im, im, -re);          // (S, -i S)
+        }
+    }
+}
+
+// Row pass of the periodicity search.  Same structure as k_tree_rowfft_stats (one CTA per block, staged
+// (row, pair) input, pair transform), but each pair IS one image: a = Re I_k, b = Im I_k, searched in power
+// P = a^2 + b^2.  Histogram over [0, kPowerRange * mean P] (mean P from Parseval), median by interpolation,
+// sigma = sqrt(median / ln 2), snr = sqrt(peak) / sigma.  Candidate: dt_idx = -1, t_idx = k.
+constexpr float kPowerRange = 6.f;
+
+template <int N, int TB>
+__global__ void __launch_bounds__(kThreads2, 1) k_tree_rowfft_power(const TreeParams p) {
+    using C = FftCfg<N>;
+    constexpr int G2 = kThreads2 / C::TPF;
+    constexpr int XB = fft_padded_size(N);
+    constexpr int NIMG = TB / 2;                      // one power image per pair
+    constexpr int NNODE = 2 * TB - 1;                 // Parseval nodes written by the gather kernel
+    constexpr int NSL = 2 * NIMG;                     // image i uses statistics slot 2 i: a whole 32-bit counter per bin
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2* xbuf = reinterpret_cast<float2*>(smem_raw);
+    const int region0 = max(G2 * XB, p.nbins);
+    float2* tw = xbuf + region0;
+    float4* stg = reinterpret_cast<float4*>(tw + C::TW_TOTAL);
+    uint32_t* hist = reinterpret_cast<uint32_t*>(stg + (size_t)G2 * p.cpad);   // [NIMG][nbins]
+    float* sA = reinterpret_cast<float*>(hist + (size_t)NIMG * p.nbins);
+    float* sScale = sA + 16;
+    float* sMean = sScale + 16;                       // mean power per image (Parseval)
+    int* sValid = reinterpret_cast<int*>(sMean + 16);
+    float* sBest = reinterpret_cast<float*>(sValid + 16);
+    int* sBpos = reinterpret_cast<int*>(sBest + kWarps2 * NSL);
+    uint32_t* hun = reinterpret_cast<uint32_t*>(xbuf);
+    uint32_t* cum = hun + p.nbins;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int slot = blockIdx.x;
+    const BlockDesc blk = p.blocks[slot];
+    const float2* Hblk = p.Ht + (size_t)slot * N * p.cpad * TB;
+    const int grp = tid / C::TPF, t = tid % C::TPF;
+    float4* sg = stg + (size_t)grp * p.cpad;
+    auto stage = [&](int y, int p2) {
+        const float4* src = reinterpret_cast<const float4*>(Hblk + ((size_t)y * (TB / 2) + p2) * p.cpad * 2);
+        for (int c = t; c < p.ncol; c += C::TPF) cp_async16(sg + c, src + c);
+        cp_async_commit();
+    };
+    stage(grp, 0);
+    for (int i = tid; i < NIMG * p.nbins; i += kThreads2) hist[i] = 0u;
+    load_twiddles<N>(tw, p.twiddles, tid, kThreads2);
+    for (int i = tid; i < kWarps2 * NSL; i += kThreads2) { sBest[i] = -CUDART_INF_F; sBpos[i] = 0; }
+    if (tid < 16) { sValid[tid] = 0; sA[tid] = 0.f; sScale[tid] = 1.f; sMean[tid] = 0.f; }
+    __syncthreads();
+    if (tid < NIMG) {
+        float tot = 0.f;                               // mean P = mean(a^2) + mean(b^2): level-0 nodes 2i, 2i+1
+        for (int h = 0; h < 2; h++)
+            for (int part = 0; part < p.n_parts; part++) tot += p.sumsq[((size_t)slot * NNODE + 2 * tid + h) * p.n_parts + part];
+        const int k = 1 + blk.tb * NIMG + tid;         // fluctuation-frequency bin of this image
+        const bool valid = k <= blk.nsearch / 2 && tot > 0.f;      // nsearch = NT of this DM
+        sValid[2 * tid] = valid ? 1 : 0;
+        sMean[2 * tid] = tot;
+        sA[2 * tid] = valid ? (float)p.nbins / (kPowerRange * tot) : 0.f;
+    }
+    __syncthreads();
+
+    TreeStatsCtx<C::TPF> cx{hist, sA, sScale, sValid, sBest, sBpos, 0.f, p.nbins, NSL};
+    float2* xb = xbuf + grp * XB;
+    const bool dbg = p.image_out != nullptr && slot == 0;
+    for (int y = grp; y < N; y += G2) {
+#pragma unroll 1
+        for (int p2 = 0; p2 < TB / 2; p2++) {
+            float2 v[16];
+            cp_async_wait_all();
+            fft_group_sync<C::TPF>(1 + grp);
+#pragma unroll
+            for (int e = 0; e < 16; e++) {
+                const int c = t + C::TPF * e;
+                const int cc = (e < 8) ? c : N - c;
+                float4 h = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (cc < p.ncol) h = sg[cc];
+                if (cc == 0 || cc == N / 2) v[e] = make_float2(h.x, h.z);
+                else if (e < 8) v[e] = make_float2(h.x - h.w, h.y + h.z);
+                else v[e] = make_float2(h.x + h.w, h.z - h.y);
+            }
+            fft_group_sync<C::TPF>(1 + grp);
+            {
+                const int np2 = (p2 + 1 == TB / 2) ? 0 : p2 + 1;
+                const int ny = (p2 + 1 == TB / 2) ? y + G2 : y;
+                if (ny < N) stage(ny, np2);
+            }
+            fft_inverse<N>(v, xb, tw, t, 1 + grp);
+            float pw[16];
+#pragma unroll
+            for (int e = 0; e < 16; e++) pw[e] = fmaf(v[e].x, v[e].x, v[e].y * v[e].y);
+            tree_row_stats<N>(pw, 2 * p2, y, t, lane, warp, cx, (dbg && p.dbg_img == p2) ? p.image_out : nullptr);
+        }
+    }
+    __syncthreads();
+
+    for (int img = 0; img < NIMG; img++) {
+        const int si = 2 * img;
+        const bool report_zero = p.stats_out != nullptr && slot == 0 && img == p.dbg_img;
+        if (!sValid[si] && !report_zero) continue;
+        const uint32_t* hw = hist + (size_t)img * p.nbins;
+        const int per = p.nbins / kThreads2;
+        uint32_t local = 0;
+        for (int i = 0; i < per; i++) {
+            const uint32_t c = hw[tid * per + i];
+            hun[tid * per + i] = c;
+            local += c;
+        }
+        uint32_t inc = local;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            uint32_t o = __shfl_up_sync(0xffffffffu, inc, d);
+            if (lane >= d) inc += o;
+        }
+        __shared__ uint32_t wtot[kWarps2];
+        if (lane == 31) wtot[warp] = inc;
+        __syncthreads();
+        uint32_t base = inc - local;
+        for (int w = 0; w < warp; w++) base += wtot[w];
+        for (int i = 0; i < per; i++) { cum[tid * per + i] = base; base += hun[tid * per + i]; }
+        __syncthreads();
+        if (tid == 0) {
+            int overflow = 0;
+            float sigma = 0.f;
+            if (sValid[si]) {
+                // median: the bin where the cumulative count crosses N^2/2, linear inside the bin
+                const float target = 0.5f * (float)N * (float)N;
+                int lo_b = 0, hi_b = p.nbins - 1;
+                while (lo_b < hi_b) {
+                    const int mid = (lo_b + hi_b + 1) >> 1;
+                    if ((float)cum[mid] <= target) lo_b = mid; else hi_b = mid - 1;
+                }
+                const float hb = (float)hun[lo_b];
+                const float w = kPowerRange * sMean[si] / (float)p.nbins;
+                const float med = ((float)lo_b + (hb > 0.f ? (target - (float)cum[lo_b]) / hb : 0.5f)) * w;
+                if (lo_b == p.nbins - 1) overflow = 1;           // median beyond the histogram range
+                sigma = sqrtf(med / 0.6931471805599453f);
+            }
+            float bv = -CUDART_INF_F;
+            int bp = 0;
+            for (int w = 0; w < kWarps2; w++) {
+                const float ov = sBest[w * NSL + si];
+                const int op = sBpos[w * NSL + si];
+                if (ov > bv || (ov == bv && op < bp)) { bv = ov; bp = op; }
+            }
+            const float peak = sValid[si] ? sqrtf(fmaxf(bv, 0.f)) : 0.f;
+            const float snr = sigma > 0.f ? peak / sigma : 0.f;
+            const int x = bp % N, yy = bp / N;
+            rf_cand c;
+            c.dm_idx = blk.dm_idx; c.dt_idx = -1; c.t_idx = 1 + blk.tb * NIMG + img;
+            c.l_pix = x < N / 2 ? x : x - N;
+            c.m_pix = yy < N / 2 ? yy : yy - N;
+            c.peak = peak; c.sigma = sigma; c.snr = snr;
+            if (overflow) atomicAdd(&p.counters[0], 1);
+            if (report_zero) *p.stats_out = c;
+            if (p.cand_count != nullptr && sValid[si] && snr >= p.threshold) {
+                int idx = atomicAdd(p.cand_count, 1);
+                if (idx < p.cand_capacity) p.cand_items[idx] = c;
             }
         }
         __syncthreads();
