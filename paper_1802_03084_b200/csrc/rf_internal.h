@@ -115,6 +115,11 @@ struct Workspace {
     BlockDesc* dbg_block = nullptr;
     int blk_batch = 0;
     size_t visI_elems = 0, ht_elems = 0, cs_elems = 0, ss_elems = 0;
+    float2* visS = nullptr;          // [n_gen_slots][nbl*nchan][tpitch] sliding sums for widths off the tree
+    int32_t* gen_slot = nullptr;     // device [ndt]: slot in visS or -1
+    std::vector<int32_t> h_gen_slot; // host copy
+    size_t visS_elems = 0;
+    int n_gen_slots = 0;
     // periodicity search
     float2* slab = nullptr;          // [n_slabs][nbl*nchan][slab_pitch] time spectra as (S, -i S) pairs
     size_t slab_elems = 0;

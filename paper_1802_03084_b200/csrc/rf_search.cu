@@ -268,6 +268,29 @@ int ensure_tree_workspace(rf_plan* p) {
         w.ss_elems = ss_elems + ss_elems / 8;
     }
     if (!w.dbg_block) RF_CUDA_CHECK(cudaMalloc((void**)&w.dbg_block, sizeof(BlockDesc)));
+    // sliding-sum arrays: one per width > 1 that is searched by the per-image path (bounded memory)
+    std::vector<int32_t> slot(p->ndt, -1);
+    int n_slots = 0;
+    const size_t budget = (size_t)24 << 30;
+    for (int k = 0; k < p->ndt; k++) {
+        bool in_tree = false;
+        for (int l = 0; l < 4; l++) in_tree |= (p->tree_dt_idx[l] == k);
+        if (in_tree || p->dts[k] <= 1 || p->dts[k] >= p->nint) continue;
+        if ((size_t)(n_slots + 1) * visI_elems * sizeof(float2) > budget) break;
+        slot[k] = n_slots++;
+    }
+    if (slot != w.h_gen_slot || !w.gen_slot) {
+        cudaFree(w.gen_slot); w.gen_slot = nullptr;
+        RF_CUDA_CHECK(cudaMalloc((void**)&w.gen_slot, (size_t)p->ndt * sizeof(int32_t)));
+        RF_CUDA_CHECK(cudaMemcpy(w.gen_slot, slot.data(), (size_t)p->ndt * sizeof(int32_t), cudaMemcpyHostToDevice));
+        w.h_gen_slot = slot;
+    }
+    w.n_gen_slots = n_slots;
+    if (n_slots > 0 && (!w.visS || w.visS_elems < (size_t)n_slots * visI_elems)) {
+        cudaFree(w.visS); w.visS = nullptr;
+        RF_CUDA_CHECK(cudaMalloc((void**)&w.visS, (size_t)n_slots * visI_elems * sizeof(float2)));
+        w.visS_elems = (size_t)n_slots * visI_elems;
+    }
     return RF_OK;
 }
 
@@ -308,6 +331,7 @@ void free_workspace(rf_plan* p) {
     cudaFree(w.ticket); cudaFree(w.counters); cudaFree(w.dbg_desc);
     cudaFree(w.visI); cudaFree(w.Ht); cudaFree(w.sumsq_t); cudaFree(w.cellsum); cudaFree(w.dbg_block);
     cudaFree(w.mean_partial); cudaFree(w.mean_p); cudaFree(w.mean_i);
+    cudaFree(w.visS); cudaFree(w.gen_slot);
     cudaFree(w.slab); cudaFree(w.pblocks); cudaFree(w.zero_delay); cudaFree(w.time_tw);
     w = Workspace{};
 }
@@ -390,7 +414,24 @@ int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out
     }
     // ---- every other width: one gridding + transform per image
     SearchParams sp = base_params(p, vis);
-    if (p->tree_tb > 0 && p->n_blocks > 0) sp.visI = p->ws.visI;     // transposed above for the tree path
+    if (p->tree_tb > 0 && p->n_blocks > 0) {
+        sp.visI = p->ws.visI;     // transposed above for the tree path
+        if (p->ws.n_gen_slots > 0 && p->n_gen_images > 0) {
+            if ((rc = mark(p, st, -1)) != RF_OK) return rc;
+            for (int k = 0; k < p->ndt; k++) {
+                const int sl = p->ws.h_gen_slot[k];
+                if (sl < 0) continue;
+                k_sliding_sum<<<dim3(p->nbl * p->nchan, (p->tpitch + 255) / 256), 256, 0, st>>>(
+                    p->ws.visI, p->ws.visS + (size_t)sl * p->ws.visI_elems, p->dts[k], p->tpitch);
+                RF_CUDA_CHECK(cudaGetLastError());
+                p->last_launches += 1;
+            }
+            if ((rc = mark(p, st, 2)) != RF_OK) return rc;
+            sp.visS = p->ws.visS;
+            sp.gen_slot = p->ws.gen_slot;
+            sp.visS_stride = (long long)p->ws.visI_elems;
+        }
+    }
     sp.cand_items = out->items;
     sp.cand_count = out->count;
     sp.cand_capacity = out->capacity;

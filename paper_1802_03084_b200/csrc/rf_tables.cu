@@ -326,7 +326,30 @@ int build_image_list(rf_plan* p) {
             bool in_tree = false;
             for (int l = 0; l < 4; l++) in_tree |= (p->tree_dt_idx[l] == k);
             if (in_tree) { in_tree_dm[d] |= nj > 0; continue; }
-            for (int j = 0; j < nj; j++) imgs.push_back({d, k, j, dt});
+        }
+    }
+    // DM trials sorted by their sweep and taken in groups of kDmGroup neighbours (both paths)
+    std::vector<int> order(p->ndm);
+    for (int d = 0; d < p->ndm; d++) order[d] = d;
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return p->h_maxdelay[a] < p->h_maxdelay[b]; });
+    int dm_group = kDmGroup;
+    if (const char* e = getenv("RF_DMGROUP")) dm_group = std::max(1, atoi(e));
+    // Image order of the per-image path: per width, DM groups, output integration j in the OUTER loop and
+    // the DM trials of the group inside.  Concurrent CTAs of one column group (blockIdx.x = image) then read
+    // the same (baseline, channel) rows at times a few integrations apart: the 32-byte sectors of the
+    // gather are shared in L2 instead of being fetched from HBM once per image at random addresses.
+    for (int k = 0; k < p->ndt; k++) {
+        bool in_tree = false;
+        for (int l = 0; l < 4; l++) in_tree |= (p->tree_dt_idx[l] == k);
+        if (in_tree) continue;
+        const int dt = p->dts[k];
+        for (int g0 = 0; g0 < p->ndm; g0 += dm_group) {
+            const int g1 = std::min(p->ndm, g0 + dm_group);
+            int max_nj = 0;
+            for (int i = g0; i < g1; i++) max_nj = std::max(max_nj, p->h_num_t[(size_t)order[i] * p->ndt + k]);
+            for (int j = 0; j < max_nj; j++)
+                for (int i = g0; i < g1; i++)
+                    if (j < p->h_num_t[(size_t)order[i] * p->ndt + k]) imgs.push_back({order[i], k, j, dt});
         }
     }
     // Block order of the tree path: DM trials sorted by their sweep and taken in groups of
@@ -335,11 +358,6 @@ int build_image_list(rf_plan* p) {
     // few integrations of delay), so the gather is served from L2 instead of re-reading the whole
     // Stokes-I array from HBM once per DM trial.
     if (p->tree_tb > 0) {
-        std::vector<int> order(p->ndm);
-        for (int d = 0; d < p->ndm; d++) order[d] = d;
-        std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return p->h_maxdelay[a] < p->h_maxdelay[b]; });
-        int dm_group = kDmGroup;
-        if (const char* e = getenv("RF_DMGROUP")) dm_group = std::max(1, atoi(e));
         for (int g0 = 0; g0 < p->ndm; g0 += dm_group) {
             const int g1 = std::min(p->ndm, g0 + dm_group);
             int max_search = 0;

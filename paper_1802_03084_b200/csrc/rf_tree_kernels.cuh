@@ -92,6 +92,21 @@ __global__ void k_stokes_transpose(const float* __restrict__ vis, float2* __rest
     }
 }
 
+// Sliding sums over dt integrations of the time-fastest Stokes-I array, out[e][t] = sum_{q<dt} visI[e][t+q]
+// (terms past the pitch dropped: those t are never searched).  A width that is not on the boxcar tree then
+// costs the per-image gather ONE 8-byte read per (baseline, channel) instead of dt (row 8a-2; the sum is the
+// same boxcar, formed once per segment instead of once per DM trial).  grid (nelem, ceil(tpitch/256)).
+__global__ void __launch_bounds__(256) k_sliding_sum(const float2* __restrict__ visI, float2* __restrict__ out,
+                                                     int dt, int tpitch) {
+    const int t = blockIdx.y * 256 + threadIdx.x;
+    if (t >= tpitch) return;
+    const float2* src = visI + (size_t)blockIdx.x * tpitch;
+    float re = 0.f, im = 0.f;
+    const int n = min(dt, tpitch - t);
+    for (int q = 0; q < n; q++) { const float2 a = __ldg(src + t + q); re += a.x; im += a.y; }
+    out[(size_t)blockIdx.x * tpitch + t] = make_float2(re, im);
+}
+
 // ------------------------------------------------------------------------------------------
 // Tree pass 0: gather + grid.  grid = (n_parts, n_blk); block = 256 = 8 warp streams.  Dynamic smem:
 //   sdelay [nchan] int | red [8][2*TB-1] float.
