@@ -101,17 +101,18 @@ int launch_batch(rf_plan* p, const SearchParams& sp, cudaStream_t st) {
 }
 
 // ---------------------------------------------------------------- boxcar-tree path
-template <int N> int tree_nbins(int tb) { return N <= 1024 ? 2048 : (N == 2048 ? 4096 : (tb == 2 ? 8192 : 4096)); }
+template <int N> int tree_nbins(int) { return N <= 1024 ? 2048 : 4096; }
 
 template <int N> size_t smem_tree1(int ntiles) {
     return (size_t)ntiles * (fft_padded_size(N) + 1) * sizeof(float2) + FftCfg<N>::TW_TOTAL * sizeof(float2);
 }
-template <int N, int TB> size_t smem_tree2(int nbins, int cpad) {
-    const size_t g2 = kThreads2 / FftCfg<N>::TPF;
+template <int N> constexpr int tree2_threads() { return N >= 2048 ? 256 : kThreads2; }
+template <int N, int TB> size_t smem_tree2(int nbins, int cpad, int nthreads = kThreads2) {
+    const size_t g2 = nthreads / FftCfg<N>::TPF;
     const size_t xb = g2 * fft_padded_size(N) * sizeof(float2);
     const size_t fin = (size_t)2 * nbins * sizeof(uint32_t);
     return std::max(xb, fin) + FftCfg<N>::TW_TOTAL * sizeof(float2) + g2 * cpad * sizeof(float4) +
-           (size_t)((2 * TB) / 2) * nbins * sizeof(uint32_t) + 64 * 4 + (size_t)2 * kWarps2 * (2 * TB - 1) * 4;
+           (size_t)(N >= 2048 ? 2 * TB - 1 : TB) * nbins * sizeof(uint32_t) + 64 * 4 + (size_t)2 * kWarps2 * (2 * TB - 1) * 4;
 }
 
 // event kinds: 0 = grid + column FFT (generic pass 1 / tree column FFT), 1 = row FFT + statistics,
@@ -128,14 +129,15 @@ int launch_tree(rf_plan* p, const TreeParams& tp, cudaStream_t st) {
         if ((rc = mark(p, st, 3)) != RF_OK) return rc;
     }
     {
-        auto kern = k_tree_colfft<N, TB, NCOL, QH>;
+        constexpr int NTH = N >= 4096 ? 512 : kThreads;   // two concurrent 4096-point transforms per CTA
+        auto kern = k_tree_colfft<N, TB, NCOL, QH, NTH>;
         const size_t smem = smem_tree1<N>(QH * NCOL);
         static size_t configured = 0;
         if (smem > configured) {
             RF_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             configured = smem;
         }
-        kern<<<dim3(tp.ngroups, tp.n_blk, TB / QH), kThreads, smem, st>>>(tp);
+        kern<<<dim3(tp.ngroups, tp.n_blk, TB / QH), NTH, smem, st>>>(tp);
         RF_CUDA_CHECK(cudaGetLastError());
         if ((rc = mark(p, st, 0)) != RF_OK) return rc;
     }
@@ -152,14 +154,15 @@ int launch_tree(rf_plan* p, const TreeParams& tp, cudaStream_t st) {
         return mark(p, st, 1);
     }
     {
-        auto kern = k_tree_rowfft_stats<N, TB>;
-        const size_t smem = smem_tree2<N, TB>(tp.nbins, tp.cpad);
+        constexpr int NT2 = tree2_threads<N>();
+        auto kern = k_tree_rowfft_stats<N, TB, NT2>;
+        const size_t smem = smem_tree2<N, TB>(tp.nbins, tp.cpad, NT2);
         static size_t configured = 0;
         if (smem > configured) {
             RF_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             configured = smem;
         }
-        kern<<<dim3(tp.n_blk), kThreads2, smem, st>>>(tp);
+        kern<<<dim3(tp.n_blk), NT2, smem, st>>>(tp);
         RF_CUDA_CHECK(cudaGetLastError());
         if ((rc = mark(p, st, 1)) != RF_OK) return rc;
     }
@@ -241,11 +244,13 @@ int ensure_tree_workspace(rf_plan* p) {
     int blk_batch = p->user_batch > 0 ? std::max(1, p->user_batch / p->tree_tb) : 0;
     if (blk_batch <= 0) {
         // pass 2 runs one CTA per block and per SM: whole waves of blocks per launch
-        const size_t budget = (size_t)4 << 30;
-        blk_batch = (int)std::min<size_t>(4096, std::max<size_t>(1, budget / (h_per_blk * sizeof(float2))));
         int dev = 0, sms = 148;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        // at least two blocks per SM per launch (N >= 2048 runs two row-pass CTAs per SM), bounded by 40 GB
+        const size_t budget = std::min<size_t>((size_t)40 << 30,
+                                               std::max<size_t>((size_t)4 << 30, (size_t)2 * sms * h_per_blk * sizeof(float2)));
+        blk_batch = (int)std::min<size_t>(4096, std::max<size_t>(1, budget / (h_per_blk * sizeof(float2))));
         if (blk_batch > sms) blk_batch -= blk_batch % sms;
     }
     if (!w.Ht || w.blk_batch != blk_batch || w.ht_elems != h_per_blk * blk_batch) {

@@ -217,8 +217,8 @@ __global__ void __launch_bounds__(kThreads) k_tree_gather(const TreeParams p) {
 // (blockIdx.z selects which: QH < TB keeps two columns per CTA when N = 1024, i.e. whole 32-byte
 // sectors in the store), from the compact grid into zeroed tiles, transforms the QH*NCOL columns
 // in place (inverse, along v) and stores the half plane.
-template <int N, int TB, int NCOL, int QH>
-__global__ void __launch_bounds__(kThreads) k_tree_colfft(const TreeParams p) {
+template <int N, int TB, int NCOL, int QH, int NTH>
+__global__ void __launch_bounds__(NTH) k_tree_colfft(const TreeParams p) {
     using C = FftCfg<N>;
     constexpr int PITCH = fft_padded_size(N) + 1;
     constexpr int NF = QH * NCOL;
@@ -236,27 +236,27 @@ __global__ void __launch_bounds__(kThreads) k_tree_colfft(const TreeParams p) {
 
     // ---- prologue: every global load of the set-up is issued before the tile is cleared
     const float2 tw0 = p.twiddles[tid < C::TW_TOTAL ? tid : 0];
-    const float2 tw1 = p.twiddles[tid + kThreads < C::TW_TOTAL ? tid + kThreads : 0];
+    const float2 tw1 = p.twiddles[tid + NTH < C::TW_TOTAL ? tid + NTH : 0];
     float2 pv[KPRE];
     uint32_t pm[KPRE];
 #pragma unroll
     for (int k = 0; k < KPRE; k++) {
-        const int i = tid + k * kThreads;
+        const int i = tid + k * NTH;
         pv[k] = make_float2(0.f, 0.f);
         pm[k] = 0u;
         if (i < nval) { pv[k] = cs[(i / QH) * TB + i % QH]; pm[k] = cm[i / QH]; }
     }
-    for (int i = tid; i < NF * PITCH; i += kThreads) tile[i] = make_float2(0.f, 0.f);
+    for (int i = tid; i < NF * PITCH; i += NTH) tile[i] = make_float2(0.f, 0.f);
     if (tid < C::TW_TOTAL) tw[tid] = tw0;
-    if (tid + kThreads < C::TW_TOTAL) tw[tid + kThreads] = tw1;
+    if (tid + NTH < C::TW_TOTAL) tw[tid + NTH] = tw1;
     __syncthreads();
     // ---- scatter the cells of these columns: value i = (cell i / QH, integration q0 + i % QH)
 #pragma unroll
     for (int k = 0; k < KPRE; k++) {
-        const int i = tid + k * kThreads;
+        const int i = tid + k * NTH;
         if (i < nval) tile[((i % QH) * NCOL + ((pm[k] >> 12) & 0xf)) * PITCH + fft_pad(pm[k] & 0xfff)] = pv[k];
     }
-    for (int i = tid + KPRE * kThreads; i < nval; i += kThreads) {
+    for (int i = tid + KPRE * NTH; i < nval; i += NTH) {
         const uint32_t m = cm[i / QH];
         tile[((i % QH) * NCOL + ((m >> 12) & 0xf)) * PITCH + fft_pad(m & 0xfff)] = cs[(i / QH) * TB + i % QH];
     }
@@ -264,7 +264,7 @@ __global__ void __launch_bounds__(kThreads) k_tree_colfft(const TreeParams p) {
 
     // ---- column FFTs in place (inverse, along v)
     {
-        constexpr int G1 = kThreads / C::TPF;
+        constexpr int G1 = NTH / C::TPF;
         const int grp = tid / C::TPF, t = tid % C::TPF;
 #ifdef RF_EXP_NOFFT
         if (p.nchan < 0)
@@ -292,7 +292,7 @@ __global__ void __launch_bounds__(kThreads) k_tree_colfft(const TreeParams p) {
 #ifdef RF_EXP_NOSTORE
         if (p.nchan < 0)
 #endif
-        for (int y = y0; y < N; y += kThreads / SEG) {
+        for (int y = y0; y < N; y += NTH / SEG) {
             const float2 a = ta[fft_pad(y)], b = tb[fft_pad(y)];
             Hs[((size_t)y * (TB / 2) + q0 / 2 + pr) * p.cpad + g * NCOL + c] = make_float4(a.x, a.y, b.x, b.y);
         }
@@ -313,6 +313,7 @@ struct TreeStatsCtx {
     int* sBpos;
     float B;
     int nbins, nimg;
+    bool wide;              // one 32-bit counter per bin and image (N >= 2048) instead of two packed 16-bit ones
 };
 
 template <int N>
@@ -321,8 +322,8 @@ __device__ __forceinline__ void tree_row_stats(const float (&x)[16], int img, in
     constexpr int TPF = N / 16;
     if (!cx.sValid[img]) return;
     const float A = cx.sA[img];
-    uint32_t* hw = cx.hist + (img >> 1) * cx.nbins;
-    const uint32_t inc = (img & 1) ? 65536u : 1u;
+    uint32_t* hw = cx.hist + (cx.wide ? img : (img >> 1)) * cx.nbins;
+    const uint32_t inc = (!cx.wide && (img & 1)) ? 65536u : 1u;
     const unsigned nbm1 = (unsigned)cx.nbins - 1u;
     float m = x[0];
 #pragma unroll
@@ -370,13 +371,17 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 constexpr int kThreads2 = 512;          // tree pass 2: one CTA of 16 warps per SM
 constexpr int kWarps2 = kThreads2 / 32;
 
-template <int N, int TB>
-__global__ void __launch_bounds__(kThreads2, 1) k_tree_rowfft_stats(const TreeParams p) {
+// NT2 = threads per CTA: 512 (one CTA per SM) up to N = 1024; 256 for N >= 2048, where one transform already
+// needs 128 or 256 threads and two or three smaller CTAs per SM hide its barriers better than one large one.
+template <int N, int TB, int NT2>
+__global__ void __launch_bounds__(NT2, NT2 == 512 ? 1 : 2) k_tree_rowfft_stats(const TreeParams p) {
+    constexpr int NWP = NT2 / 32;
     using C = FftCfg<N>;
-    constexpr int G2 = kThreads2 / C::TPF;
+    constexpr int G2 = NT2 / C::TPF;
     constexpr int XB = fft_padded_size(N);
     constexpr int NIMG = 2 * TB - 1;
-    constexpr int NW = (NIMG + 1) / 2;
+    constexpr bool WIDE = N >= 2048;                  // 16-bit counters would wrap: N^2 pixels in few central bins
+    constexpr int NW = WIDE ? NIMG : (NIMG + 1) / 2;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2* xbuf = reinterpret_cast<float2*>(smem_raw);
     // region 0 holds the FFT exchange buffers, later the unpacked histogram + prefix sums
@@ -389,7 +394,7 @@ __global__ void __launch_bounds__(kThreads2, 1) k_tree_rowfft_stats(const TreePa
     float* sSig = sScale + 16;                                               // [16] sigma_rms per image
     int* sValid = reinterpret_cast<int*>(sSig + 16);                         // [16]
     float* sBest = reinterpret_cast<float*>(sValid + 16);                    // [16 warps][NIMG]
-    int* sBpos = reinterpret_cast<int*>(sBest + kWarps2 * NIMG);             // [16 warps][NIMG]
+    int* sBpos = reinterpret_cast<int*>(sBest + NWP * NIMG);             // [16 warps][NIMG]
     uint32_t* hun = reinterpret_cast<uint32_t*>(xbuf);                       // after the row loop
     uint32_t* cum = hun + p.nbins;
 
@@ -408,9 +413,9 @@ __global__ void __launch_bounds__(kThreads2, 1) k_tree_rowfft_stats(const TreePa
     };
     stage(grp, 0);
 
-    for (int i = tid; i < NW * p.nbins; i += kThreads2) hist[i] = 0u;
-    load_twiddles<N>(tw, p.twiddles, tid, kThreads2);
-    for (int i = tid; i < kWarps2 * NIMG; i += kThreads2) { sBest[i] = -CUDART_INF_F; sBpos[i] = 0; }
+    for (int i = tid; i < NW * p.nbins; i += NT2) hist[i] = 0u;
+    load_twiddles<N>(tw, p.twiddles, tid, NT2);
+    for (int i = tid; i < NWP * NIMG; i += NT2) { sBest[i] = -CUDART_INF_F; sBpos[i] = 0; }
     if (tid < NIMG) {
         int l = 0, off = 0;
         while (tid >= off + (TB >> l)) { off += TB >> l; l++; }
@@ -427,7 +432,7 @@ __global__ void __launch_bounds__(kThreads2, 1) k_tree_rowfft_stats(const TreePa
     }
     __syncthreads();
 
-    TreeStatsCtx<C::TPF> cx{hist, sA, sScale, sValid, sBest, sBpos, 0.5f * (float)p.nbins, p.nbins, NIMG};
+    TreeStatsCtx<C::TPF> cx{hist, sA, sScale, sValid, sBest, sBpos, 0.5f * (float)p.nbins, p.nbins, NIMG, WIDE};
     float2* xb = xbuf + grp * XB;
     const bool dbg = p.image_out != nullptr && slot == 0;
 
@@ -497,12 +502,12 @@ __global__ void __launch_bounds__(kThreads2, 1) k_tree_rowfft_stats(const TreePa
     for (int img = 0; img < NIMG; img++) {
         const bool report_zero = p.stats_out != nullptr && slot == 0 && img == p.dbg_img;
         if (!sValid[img] && !report_zero) continue;            // block-uniform
-        const uint32_t* hw = hist + (img >> 1) * p.nbins;
-        const int sh = (img & 1) * 16;
-        const int per = p.nbins / kThreads2;
+        const uint32_t* hw = hist + (WIDE ? img : (img >> 1)) * p.nbins;
+        const int sh = WIDE ? 0 : (img & 1) * 16;
+        const int per = p.nbins / NT2;
         uint32_t local = 0;
         for (int i = 0; i < per; i++) {
-            const uint32_t c = (hw[tid * per + i] >> sh) & 0xffffu;
+            const uint32_t c = WIDE ? hw[tid * per + i] : (hw[tid * per + i] >> sh) & 0xffffu;
             hun[tid * per + i] = c;
             local += c;
         }
@@ -512,11 +517,11 @@ __global__ void __launch_bounds__(kThreads2, 1) k_tree_rowfft_stats(const TreePa
             uint32_t o = __shfl_up_sync(0xffffffffu, inc, d);
             if (lane >= d) inc += o;
         }
-        __shared__ uint32_t wtot[kWarps2];
+        __shared__ uint32_t wtot[NWP];
         if (lane == 31) wtot[warp] = inc;
         __syncthreads();
         uint32_t base = inc - local, total = 0;
-        for (int w = 0; w < kWarps2; w++) { if (w < warp) base += wtot[w]; total += wtot[w]; }
+        for (int w = 0; w < NWP; w++) { if (w < warp) base += wtot[w]; total += wtot[w]; }
         for (int i = 0; i < per; i++) { cum[tid * per + i] = base; base += hun[tid * per + i]; }
         __syncthreads();
         if (warp == 0) {
@@ -531,7 +536,7 @@ __global__ void __launch_bounds__(kThreads2, 1) k_tree_rowfft_stats(const TreePa
             if (lane == 0) {
                 float bv = -CUDART_INF_F;
                 int bp = 0;
-                for (int w = 0; w < kWarps2; w++) {
+                for (int w = 0; w < NWP; w++) {
                     const float ov = sBest[w * NIMG + img];
                     const int op = sBpos[w * NIMG + img];
                     if (ov > bv || (ov == bv && op < bp)) { bv = ov; bp = op; }
@@ -659,7 +664,7 @@ __global__ void __launch_bounds__(kThreads2, 1) k_tree_rowfft_power(const TreePa
     }
     __syncthreads();
 
-    TreeStatsCtx<C::TPF> cx{hist, sA, sScale, sValid, sBest, sBpos, 0.f, p.nbins, NSL};
+    TreeStatsCtx<C::TPF> cx{hist, sA, sScale, sValid, sBest, sBpos, 0.f, p.nbins, NSL, false};
     float2* xb = xbuf + grp * XB;
     const bool dbg = p.image_out != nullptr && slot == 0;
     for (int y = grp; y < N; y += G2) {
