@@ -267,6 +267,25 @@ def run_ours(args, cfg):
     torch.cuda.synchronize(dev)
     e2e_ms = (time.perf_counter() - t0) * 1e3
 
+    # ---- optional: the periodicity search of the same segment, device-resident
+    periodic = None
+    if args.periodic:
+        def pstep():
+            plan.search_periodic_raw(dvis.data_ptr(), stream.cuda_stream, items.data_ptr(), capacity, count.data_ptr())
+        pstep()
+        barrier()
+        p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        p0.record(stream)
+        for _ in range(args.steps):
+            pstep()
+        p1.record(stream)
+        barrier()
+        p_ms = p0.elapsed_time(p1) / args.steps
+        n_freq = sum(plan.periodic_nt(d) // 2 for d in range(cfg.ndm))
+        periodic = {"ms_per_step": p_ms, "frequency_images_per_step": n_freq, "value": n_freq / (p_ms * 1e-3),
+                    "unit": "frequency images/s", "candidates": int(count.item()),
+                    "gpu_launches": int(plan.get_counters()["kernel_launches"])}
+
     t_all = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device=dev)
     if world > 1:
         dist.all_reduce(t_all, op=dist.ReduceOp.MAX)
@@ -303,6 +322,8 @@ def run_ours(args, cfg):
             "gpu_launches": int(launches) * args.steps,
             "roofline": _roofline(alg, k_ms, k_n, ms_per_step, traffic),
         }
+        if periodic is not None:
+            line["periodic"] = periodic
         if world == 1 and not args.no_cpu_baseline:
             v, cores, sample = oracle_throughput(cfg, vis, args.ref_images)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
@@ -469,6 +490,7 @@ def main():
     ap.add_argument("--batch", type=int, default=0, help="images per batch (0 = library default)")
     ap.add_argument("--ref-images", type=int, default=512, help="oracle sample size per timing")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--periodic", action="store_true", help="also time rf_search_periodic (8f-3) on the same segment")
     ap.add_argument("--meansub", action="store_true", help="also run the prep stage (mean-visibility subtraction, 8f-1)")
     args = ap.parse_args()
     cfg = W.get_config(args.config)

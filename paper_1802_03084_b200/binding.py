@@ -269,6 +269,10 @@ class Plan:
         """rf_plan_periodic_nt: length of the time transform of one DM trial (0 = trial skipped)."""
         return int(self._lib.rf_plan_periodic_nt(self._h, dm_idx))
 
+    def search_periodic_raw(self, vis_ptr: int, stream: int, items_ptr: int, capacity: int, count_ptr: int) -> None:
+        out = _CandOut(items_ptr, capacity, count_ptr)
+        _check(self._lib.rf_search_periodic(self._h, vis_ptr, stream, C.byref(out)))
+
     def search_periodic(self, vis, capacity: int = 1 << 16, stream=None):
         """rf_search_periodic: candidates (dt_idx = -1, t_idx = fluctuation-frequency bin k) and their count."""
         import torch
