@@ -201,7 +201,7 @@ int rf_inject(rf_plan* plan, void* vis_dev, double amp, double l_pix, double m_p
  * is searched in power P = |I_k|^2: peak = sqrt(max P) (first maximum in row-major order), sigma =
  * sqrt(median(P)/ln 2), snr = peak/sigma.  Candidates with snr >= threshold are appended to cand_out with
  * dt_idx = -1 and t_idx = k (fluctuation frequency k/(NT inttime) Hz).  Honours rf_plan_set_meansub and
- * the channel weights; ignores the search span.  Needs a plan on the boxcar-tree kernels (npix 256..1024
+ * the channel weights; ignores the search span.  Needs a plan on the boxcar-tree kernels (npix >= 256
  * and a power-of-two width <= 8 in dt_list), else RF_ERR_STATE.  Enqueues on cuda_stream; one host
  * synchronisation at entry (block-list upload), none after the first kernel.
  *   rf_debug_periodic_image: power image [npix][npix] (float32, DEVICE) and/or statistics of one

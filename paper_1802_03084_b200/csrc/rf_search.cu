@@ -574,7 +574,7 @@ int ensure_periodic_workspace(rf_plan* p, int nt_max, int n_dm_live) {
 int launch_search_periodic(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out, int dbg_dm, int dbg_k,
                            float* power_dev, rf_cand* stats_dev) {
     if (p->tree_tb == 0) {
-        set_error("the periodicity search runs on the boxcar-tree kernels: the plan needs npix in 256..1024 and "
+        set_error("the periodicity search runs on the boxcar-tree kernels: the plan needs npix >= 256 and "
                   "a power-of-two width <= 8 in dt_list");
         return RF_ERR_STATE;
     }

@@ -286,8 +286,8 @@ void configure_tree(rf_plan* p) {
     // which dt values ride the image-domain boxcar tree (B3)
     p->tree_tb = 0;
     for (int l = 0; l < 4; l++) p->tree_dt_idx[l] = -1;
-    // npix >= 2048: one CTA per block starves the GPU and the shared-memory tiles shrink to 1-2
-    // columns; measured slower than the generic path (hi-res config: 2.7 s vs 1.2 s), so off.
+    // every size from 256 up rides the tree (N >= 2048: 256-thread row-pass CTAs, see launch_tree); RF_TREE_MAXPIX
+    // lowers the limit for experiments
     int tree_maxpix = 4096;
     if (const char* e = getenv("RF_TREE_MAXPIX")) tree_maxpix = atoi(e);
     if (p->use_tree && p->npix >= 256 && p->npix <= tree_maxpix) {

@@ -18,7 +18,7 @@ def _rand_vis(shape, seed):
     return (rng.standard_normal(shape, dtype=np.float32) + 1j * rng.standard_normal(shape, dtype=np.float32)).astype(np.complex64)
 
 
-def _compare_all(plan, dvis, vis, f, uvw, cell, npix, dms, dts, thr, inttime, weights=None, min_match=1):
+def _compare_all(plan, dvis, vis, f, uvw, cell, npix, dms, dts, thr, inttime, weights=None, min_match=1, pix_slack=0):
     gpu, n = plan.search(dvis, capacity=1 << 15)
     assert n == len(gpu)
     ref, stats = O.search(vis, f, uvw, inttime, npix, cell, dms, dts, thr, chan_weights=weights, return_all_stats=True)
@@ -29,7 +29,11 @@ def _compare_all(plan, dvis, vis, f, uvw, cell, npix, dms, dts, thr, inttime, we
         assert abs(stats[key][4] - thr) <= NEAR_THR * thr, (key, stats[key][4])
     for key in set(g) & set(o):
         assert abs(float(g[key]["snr"]) - o[key].snr) <= SNR_TOL * o[key].snr, key
-        assert (int(g[key]["l_pix"]), int(g[key]["m_pix"])) == (o[key].l_pix, o[key].m_pix), key
+        if pix_slack == 0:
+            assert (int(g[key]["l_pix"]), int(g[key]["m_pix"])) == (o[key].l_pix, o[key].m_pix), key
+        else:   # heavily oversampled images: neighbouring pixels tie within float32 rounding (A20); the peak VALUE decides
+            assert abs(int(g[key]["l_pix"]) - o[key].l_pix) <= pix_slack and abs(int(g[key]["m_pix"]) - o[key].m_pix) <= pix_slack, key
+            assert abs(float(g[key]["peak"]) - o[key].peak) <= 1e-5 * o[key].peak, key
     assert len(set(g) & set(o)) >= min_match
     assert plan.get_counters()["stats_overflow"] == 0
     return g
@@ -110,4 +114,28 @@ def test_candidate_overflow_keeps_counting():
     assert n == plan.num_images() == 388 and len(rec) == 10           # count runs past capacity, items are capped
     keys = {(int(c["dm_idx"]), int(c["t_idx"])) for c in rec}
     assert len(keys) == 10 and all(float(c["sigma"]) > 0 for c in rec)
+    plan.destroy()
+
+
+def test_npix_2048_tree_path():
+    """npix 2048 is used by none of the five configs: the boxcar tree with 256-thread row-pass CTAs and 32-bit
+    histograms (two 128-thread transform groups per CTA), every image at threshold 0 plus one image pixel by pixel."""
+    import torch
+    import paper_1802_03084_b200 as R
+    cfg = W.get_config("tiny")
+    npix, nint, dts = 2048, 14, (1, 2, 4)
+    f, uvw = W.channel_freqs_hz(cfg), W.baseline_uvw_m(cfg)
+    cell = W.default_cell_rad(cfg, uvw) * 64 / npix * 0.8
+    dms = np.array([0.0, 30.0])
+    vis = _rand_vis((nint, cfg.nbl, cfg.nchan, 2), 2048)
+    vis = O.inject_transient(vis, f, uvw, cfg.inttime_s, cell, 1.0, 300, -700, 30.0, 2, 4).astype(np.complex64)
+    plan = R.Plan(f, uvw, 2, nint, cfg.inttime_s, npix, cell, dms, dts, 0.0)
+    d = torch.from_numpy(vis).cuda()
+    g = _compare_all(plan, d, vis, f, uvw, cell, npix, dms, dts, 0.0, cfg.inttime_s, min_match=10, pix_slack=1)
+    assert len(g) == plan.num_images()
+    delays = O.delay_table(f, dms, cfg.inttime_s)
+    iu, iv, keep = O.cell_table(uvw, f, npix, cell)
+    ref = O.search_image(vis, delays, iu, iv, keep, npix, 1, 2, 2)
+    img, _ = plan.debug_image(d, 1, 1, 2)
+    assert np.abs(img - ref).max() <= PIX_TOL * np.sqrt((ref ** 2).mean())
     plan.destroy()
