@@ -134,7 +134,9 @@ int rf_plan_set_batch(rf_plan* plan, int images_per_batch);
 /* End-to-end convenience entry with HOST buffers: copies the segment host->device into a
  * plan-owned staging buffer, runs rf_search on the plan's own stream, copies the candidates
  * back and SYNCHRONISES.  vis_host: complex64 [nint][nbl][nchan][npol] (pinned memory makes
- * the copy asynchronous and fast; pageable works).  cand_host: capacity records; *count_host
+ * the copy asynchronous and fast; pageable works).  On the boxcar-tree path the segment is uploaded in chunks
+ * of 64 integrations on a second stream and the search, which consumes the segment front to back, runs behind
+ * the upload (each launch waits only for the integrations it reads).  cand_host: capacity records; *count_host
  * receives the number found (may exceed capacity = overflow).                     */
 int rf_search_host(rf_plan* plan, const void* vis_host, rf_cand* cand_host, int32_t capacity,
                    int32_t* count_host);

@@ -1,4 +1,5 @@
 // rf_api.cu -- the C-ABI of include/realfast.h: validation, plan lifetime, error strings.
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -92,6 +93,8 @@ int rf_plan_destroy(rf_plan* p) {
     for (cudaEvent_t e : p->events) cudaEventDestroy(e);
     cudaFree(p->stage_vis); cudaFree(p->stage_cand); cudaFree(p->stage_count);
     if (p->own_stream) cudaStreamDestroy(p->own_stream);
+    if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
+    for (cudaEvent_t e : p->chunk_done) cudaEventDestroy(e);
     if (p->tab_stream) cudaStreamDestroy(p->tab_stream);
     rf::free_workspace(p);
     free_tables(p);
@@ -124,10 +127,35 @@ int rf_search_host(rf_plan* p, const void* vis_host, rf_cand* cand_host, int32_t
         p->stage_capacity = capacity;
     }
     cudaStream_t st = p->own_stream;
-    RF_CUDA_CHECK(cudaMemcpyAsync(p->stage_vis, vis_host, vis_bytes, cudaMemcpyHostToDevice, st));
     rf_cand_out out{p->stage_cand, capacity, p->stage_count};
-    int rc = rf::launch_search(p, p->stage_vis, st, &out);
-    if (rc != RF_OK) return rc;
+    int rc;
+    if (p->tree_tb > 0 && p->n_blocks > 0 && !p->meansub && p->n_kept > 0) {
+        // The boxcar-tree search consumes the segment front to back: upload it in chunks on a copy stream and
+        // let the search run behind the upload (each launch waits only for the integrations it reads).
+        const int rows = 64;
+        const int n_chunks = (p->nint + rows - 1) / rows;
+        if (!p->copy_stream) RF_CUDA_CHECK(cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking));
+        while ((int)p->chunk_done.size() < n_chunks) {
+            cudaEvent_t e;
+            RF_CUDA_CHECK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+            p->chunk_done.push_back(e);
+        }
+        const size_t row_bytes = (size_t)p->nbl * p->nchan * p->npol * 8;
+        for (int c = 0; c < n_chunks; c++) {
+            const size_t lo = (size_t)c * rows, hi = std::min<size_t>(p->nint, lo + rows);
+            RF_CUDA_CHECK(cudaMemcpyAsync(static_cast<char*>(p->stage_vis) + lo * row_bytes,
+                                          static_cast<const char*>(vis_host) + lo * row_bytes, (hi - lo) * row_bytes,
+                                          cudaMemcpyHostToDevice, p->copy_stream));
+            RF_CUDA_CHECK(cudaEventRecord(p->chunk_done[c], p->copy_stream));
+        }
+        rf::HostFeed feed{p->chunk_done.data(), rows, n_chunks};
+        rc = rf::launch_search(p, p->stage_vis, st, &out, &feed);
+        if (rc != RF_OK) { cudaStreamSynchronize(p->copy_stream); return rc; }
+    } else {
+        RF_CUDA_CHECK(cudaMemcpyAsync(p->stage_vis, vis_host, vis_bytes, cudaMemcpyHostToDevice, st));
+        rc = rf::launch_search(p, p->stage_vis, st, &out);
+        if (rc != RF_OK) return rc;
+    }
     RF_CUDA_CHECK(cudaMemcpyAsync(count_host, p->stage_count, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
     RF_CUDA_CHECK(cudaStreamSynchronize(st));
     const int32_t n = *count_host < capacity ? *count_host : capacity;

@@ -27,6 +27,7 @@ inline int cols_per_group(int npix) { return npix <= 512 ? 16 : (npix == 1024 ? 
 constexpr int kWarpsPerCta = 8;     // 256 threads everywhere
 constexpr int kThreads = 32 * kWarpsPerCta;
 constexpr int kDmGroup = 8;         // DM trials interleaved in time by the tree path's block order
+constexpr int kUnitBlocks = 4;      // consecutive time blocks of a DM group kept together in the tree path's block order
 constexpr int kTreeUnroll = 8;      // iterations of the tree gather kept in flight per warp
 constexpr int kStreamIters = 64;    // target length of one warp stream of the tree gather
 constexpr float kHistRange = 3.5f;  // histogram covers +-kHistRange * sigma_rms
@@ -152,6 +153,7 @@ struct rf_plan {
     std::vector<uint8_t> h_keep;
     std::vector<int32_t> h_maxdelay;           // [ndm]
     std::vector<int32_t> h_num_t;              // [ndm][ndt]
+    std::vector<int32_t> h_block_deadline;     // [n_blocks] integrations [0, deadline) are all a tree block (and those before it) read
     // derived
     int n_kept = 0, n_dropped = 0;
     int ncol = 0;                    // occupied half-plane columns 0..ncol-1 (ncol <= npix/2+1)
@@ -170,7 +172,8 @@ struct rf_plan {
     rf_cand* stage_cand = nullptr;
     int32_t* stage_count = nullptr;
     int stage_capacity = 0;
-    cudaStream_t own_stream = nullptr;
+    cudaStream_t own_stream = nullptr, copy_stream = nullptr;
+    std::vector<cudaEvent_t> chunk_done;       // upload events of rf_search_host
     // per-kernel event timing
     bool profile = false;
     std::vector<cudaEvent_t> events;
@@ -201,7 +204,10 @@ int launch_inject(rf_plan* p, void* vis, double amp, double l_pix, double m_pix,
 // rf_search.cu
 int ensure_workspace(rf_plan* p);
 void free_workspace(rf_plan* p);
-int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out);
+// rf_search_host: the segment arrives in chunks of rows_per_chunk integrations (a multiple of 32); chunk c is
+// on the device once chunk_done[c] has fired
+struct HostFeed { const cudaEvent_t* chunk_done; int rows_per_chunk, n_chunks; };
+int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out, const HostFeed* feed = nullptr);
 int launch_debug_image(rf_plan* p, const void* vis, int dm_idx, int dt_idx, int t_idx,
                        float* image_dev, rf_cand* stats_dev, cudaStream_t st);
 int periodic_nt(const rf_plan* p, int dm_idx);   // length of the time transform of one DM trial (0 = none)

@@ -184,21 +184,23 @@ int launch_tree_batch(rf_plan* p, TreeParams& tp, cudaStream_t st) {
     return RF_ERR_ARG;
 }
 
-int launch_prep(rf_plan* p, const void* vis, cudaStream_t st) {
+// Stokes-I transpose of the integrations [t_lo, t_hi) (multiples of 32; t_hi = tpitch covers the zero pad)
+int launch_prep_rows(rf_plan* p, const void* vis, cudaStream_t st, int t_lo, int t_hi) {
     const int nelem = p->nbl * p->nchan;
     const float2* mi = p->meansub ? p->ws.mean_i : nullptr;
-    dim3 grid((nelem + 31) / 32, (p->tpitch + 31) / 32), block(32, 8);
+    dim3 grid((nelem + 31) / 32, (t_hi - t_lo + 31) / 32), block(32, 8);
     const float* v = reinterpret_cast<const float*>(vis);
     int rc;
     if ((rc = mark(p, st, -1)) != RF_OK) return rc;
     switch (p->npol) {
-        case 1: k_stokes_transpose<1><<<grid, block, 0, st>>>(v, p->ws.visI, mi, p->nint, nelem, p->tpitch); break;
-        case 2: k_stokes_transpose<2><<<grid, block, 0, st>>>(v, p->ws.visI, mi, p->nint, nelem, p->tpitch); break;
-        default: k_stokes_transpose<4><<<grid, block, 0, st>>>(v, p->ws.visI, mi, p->nint, nelem, p->tpitch); break;
+        case 1: k_stokes_transpose<1><<<grid, block, 0, st>>>(v, p->ws.visI, mi, p->nint, nelem, p->tpitch, t_lo); break;
+        case 2: k_stokes_transpose<2><<<grid, block, 0, st>>>(v, p->ws.visI, mi, p->nint, nelem, p->tpitch, t_lo); break;
+        default: k_stokes_transpose<4><<<grid, block, 0, st>>>(v, p->ws.visI, mi, p->nint, nelem, p->tpitch, t_lo); break;
     }
     RF_CUDA_CHECK(cudaGetLastError());
     return mark(p, st, 2);
 }
+int launch_prep(rf_plan* p, const void* vis, cudaStream_t st) { return launch_prep_rows(p, vis, st, 0, p->tpitch); }
 
 TreeParams tree_params(rf_plan* p) {
     TreeParams tp{};
@@ -387,7 +389,7 @@ int ensure_workspace(rf_plan* p) {
     return RF_OK;
 }
 
-int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out) {
+int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out, const HostFeed* feed) {
     int rc = ensure_workspace(p);
     if (rc == RF_OK) rc = ensure_tree_workspace(p);
     if (rc != RF_OK) return rc;
@@ -404,8 +406,26 @@ int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out
     }
     // ---- power-of-two widths: blocks of TB integrations through the boxcar tree
     if (p->tree_tb > 0 && p->n_blocks > 0) {
-        if ((rc = launch_prep(p, vis, st)) != RF_OK) return rc;
-        p->last_launches += 1;
+        // Stokes-I transpose of the rows a launch needs, as they become available: the whole segment at once
+        // for a device-resident segment, chunk by chunk behind the upload for rf_search_host (blocks are sorted
+        // by the last integration they read, build_image_list)
+        int rows_ready = 0;
+        auto need_rows = [&](int rows) -> int {
+            rows = std::min(rows, p->tpitch);
+            while (rows_ready < rows) {
+                int hi = p->tpitch;
+                if (feed) {
+                    const int c = rows_ready / feed->rows_per_chunk;
+                    if (c < feed->n_chunks) RF_CUDA_CHECK(cudaStreamWaitEvent(st, feed->chunk_done[c], 0));
+                    if (c + 1 < feed->n_chunks) hi = (c + 1) * feed->rows_per_chunk;
+                }
+                int r = launch_prep_rows(p, vis, st, rows_ready, hi);
+                if (r != RF_OK) return r;
+                p->last_launches += 1;
+                rows_ready = hi;
+            }
+            return RF_OK;
+        };
         TreeParams tp = tree_params(p);
         tp.cand_items = out->items;
         tp.cand_count = out->count;
@@ -413,9 +433,11 @@ int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out
         for (int64_t base = 0; base < p->n_blocks; base += p->ws.blk_batch) {
             tp.blocks = p->d.blocks + base;
             tp.n_blk = (int)std::min<int64_t>(p->ws.blk_batch, p->n_blocks - base);
+            if ((rc = need_rows(p->h_block_deadline[base + tp.n_blk - 1])) != RF_OK) return rc;
             if ((rc = launch_tree_batch(p, tp, st)) != RF_OK) return rc;
             p->last_launches += 3;
         }
+        if ((rc = need_rows(p->tpitch)) != RF_OK) return rc;      // widths off the tree read the whole array
     }
     // ---- every other width: one gridding + transform per image
     SearchParams sp = base_params(p, vis);

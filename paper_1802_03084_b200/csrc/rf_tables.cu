@@ -357,15 +357,36 @@ int build_image_list(rf_plan* p) {
     // read nearly the same window of every (baseline, channel) row (neighbouring DMs differ by a
     // few integrations of delay), so the gather is served from L2 instead of re-reading the whole
     // Stokes-I array from HBM once per DM trial.
+    // Units of one DM group x one time block are then sorted by the last integration they read ("deadline"
+    // = tb*TB + TB + largest sweep of the group): the search consumes the segment front to back, so
+    // rf_search_host can start it while the upload of the later integrations is still in flight, and a
+    // launch never needs rows beyond the deadline of its last block (h_block_deadline).
+    p->h_block_deadline.clear();
     if (p->tree_tb > 0) {
+        struct Unit { int g0, tb, deadline; };
+        std::vector<Unit> units;
         for (int g0 = 0; g0 < p->ndm; g0 += dm_group) {
             const int g1 = std::min(p->ndm, g0 + dm_group);
-            int max_search = 0;
-            for (int i = g0; i < g1; i++) if (in_tree_dm[order[i]]) max_search = std::max(max_search, nsearch_of[order[i]]);
-            for (int tb = 0; tb * p->tree_tb < max_search; tb++)
-                for (int i = g0; i < g1; i++) {
+            int max_search = 0, sweep = 0;
+            for (int i = g0; i < g1; i++)
+                if (in_tree_dm[order[i]]) {
+                    max_search = std::max(max_search, nsearch_of[order[i]]);
+                    sweep = std::max(sweep, p->h_maxdelay[order[i]]);
+                }
+            // a unit = kUnitBlocks consecutive time blocks of the group: neighbouring blocks share 128-byte lines
+            for (int tb = 0; tb * p->tree_tb < max_search; tb += kUnitBlocks)
+                units.push_back({g0, tb, std::min(p->tpitch, (tb + kUnitBlocks) * p->tree_tb + sweep)});
+        }
+        std::stable_sort(units.begin(), units.end(), [](const Unit& a, const Unit& b) { return a.deadline < b.deadline; });
+        for (const Unit& u : units) {
+            const int g1 = std::min(p->ndm, u.g0 + dm_group);
+            for (int tb = u.tb; tb < u.tb + kUnitBlocks; tb++)
+                for (int i = u.g0; i < g1; i++) {
                     const int d = order[i];
-                    if (in_tree_dm[d] && tb * p->tree_tb < nsearch_of[d]) blocks.push_back({d, tb, nsearch_of[d], 0});
+                    if (in_tree_dm[d] && tb * p->tree_tb < nsearch_of[d]) {
+                        blocks.push_back({d, tb, nsearch_of[d], 0});
+                        p->h_block_deadline.push_back(u.deadline);
+                    }
                 }
         }
     }

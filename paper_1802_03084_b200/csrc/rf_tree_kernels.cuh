@@ -64,9 +64,9 @@ __host__ __device__ constexpr int tree_off(int tb, int l) {
 // Stokes-I sum of the time means, subtracted on the fly (mean-visibility subtraction).
 template <int NPOL>
 __global__ void k_stokes_transpose(const float* __restrict__ vis, float2* __restrict__ visI,
-                                   const float2* __restrict__ mean_i, int nint, int nelem, int tpitch) {
+                                   const float2* __restrict__ mean_i, int nint, int nelem, int tpitch, int t_first) {
     __shared__ float2 tile[32][33];
-    const int e0 = blockIdx.x * 32, t0 = blockIdx.y * 32;
+    const int e0 = blockIdx.x * 32, t0 = t_first + blockIdx.y * 32;    // t_first: row range of a chunked upload
     for (int r = threadIdx.y; r < 32; r += 8) {
         const int t = t0 + r, e = e0 + threadIdx.x;
         float2 s = make_float2(0.f, 0.f);
