@@ -5,6 +5,7 @@
 // sized so that the half-plane hand-off H between the two FFT passes stays L2-resident.
 #include <algorithm>
 #include <cstdio>
+#include <cstdlib>
 
 #include "rf_tree_kernels.cuh"
 
@@ -430,12 +431,25 @@ int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out
         tp.cand_items = out->items;
         tp.cand_count = out->count;
         tp.cand_capacity = out->capacity;
-        for (int64_t base = 0; base < p->n_blocks; base += p->ws.blk_batch) {
+        // behind an upload the launches start small (one wave of row-pass CTAs), so that the first ones wait for
+        // few integrations; once a launch needs the whole segment anyway the batches are full-sized
+        int small = p->ws.blk_batch;
+        if (feed) {
+            int dev = 0, sms = 148;
+            cudaGetDevice(&dev);
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+            small = std::min(small, sms);
+            if (const char* e = getenv("RF_FEED_BATCH")) small = std::max(1, std::min(p->ws.blk_batch, atoi(e)));
+        }
+        for (int64_t base = 0; base < p->n_blocks;) {
+            int n = (int)std::min<int64_t>(p->ws.blk_batch, p->n_blocks - base);
+            if (feed && p->h_block_deadline[base + std::min(n, small) - 1] < p->nint) n = std::min(n, small);
             tp.blocks = p->d.blocks + base;
-            tp.n_blk = (int)std::min<int64_t>(p->ws.blk_batch, p->n_blocks - base);
-            if ((rc = need_rows(p->h_block_deadline[base + tp.n_blk - 1])) != RF_OK) return rc;
+            tp.n_blk = n;
+            if ((rc = need_rows(p->h_block_deadline[base + n - 1])) != RF_OK) return rc;
             if ((rc = launch_tree_batch(p, tp, st)) != RF_OK) return rc;
             p->last_launches += 3;
+            base += n;
         }
         if ((rc = need_rows(p->tpitch)) != RF_OK) return rc;      // widths off the tree read the whole array
     }
