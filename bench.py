@@ -119,7 +119,18 @@ def _roofline(alg, k_ms, k_n, ms_per_step, traffic=None):
             "kernel_launches_per_step": {n: k_n[i] for i, n in enumerate(names)},
             "kernel_alg_gbs": {n: (alg["kind"][i] / (k_ms[i] * 1e-3) / 1e9 if k_ms[i] > 0 else 0.0)
                                for i, n in enumerate(names)},
-            "path": {"alg_bytes_per_step": alg["total"], "achieved": path_gbs, "frac": path_gbs / peak}}
+            "path": {"alg_bytes_per_step": alg["total"], "achieved": path_gbs, "frac": path_gbs / peak,
+                     **_own_bytes(traffic, k_n, ms_per_step, peak)}}
+
+
+def _own_bytes(traffic, k_n, ms_per_step, peak):
+    """The bytes THIS design moves per step (a design that moves fewer bytes than the model reports
+    its own count too): ncu DRAM bytes per launch of each tree kernel x its launches per step.  The fraction of the
+    HBM peak they amount to says how far from HBM-bound the step is (the kernels are bound on chip)."""
+    if not traffic or any(traffic.get(k) is None for k in (0, 1, 3)):
+        return {}
+    own = sum(traffic[k] * k_n[k] for k in (0, 1, 3))
+    return {"dram_bytes_per_step_ncu": own, "dram_frac": own / (ms_per_step * 1e-3) / 1e9 / peak}
 
 
 def _oracle_worker(args):
