@@ -286,7 +286,14 @@ __global__ void __launch_bounds__(NTH) k_tree_colfft(const TreeParams p) {
     {
         constexpr int SEG = NCOL * QH / 2;
         float4* Hs = reinterpret_cast<float4*>(p.Ht + (size_t)slot * N * p.cpad * TB);
-        const int i = tid % SEG, pr = i / NCOL, c = i % NCOL, y0 = tid / SEG;
+        // Row of each thread within the NTH/SEG rows of an iteration: a bit permutation of tid / SEG chosen so that
+        // the 16 lanes of a half-warp (16/SEG rows x SEG tiles, tile pitch = 1 mod 16 words) read 16 different
+        // 8-byte bank pairs (identity order: 2-way conflicts, rows y and y + 1 collide on neighbouring tiles).
+        int y0 = tid / SEG;
+        if (SEG == 8) y0 = (y0 & ~3) | ((y0 & 1) << 1) | ((y0 >> 1) & 1);
+        else if (SEG == 4) y0 = (y0 & ~15) | ((y0 & 1) << 1) | ((y0 & 2) << 2) | ((y0 >> 2) & 1) | ((y0 & 8) >> 1);
+        else if (SEG == 2) y0 = (y0 & ~15) | ((y0 & 7) << 1) | ((y0 >> 3) & 1);
+        const int i = tid % SEG, pr = i / NCOL, c = i % NCOL;
         const float2* ta = tile + (2 * pr * NCOL + c) * PITCH;
         const float2* tb = ta + NCOL * PITCH;
 #ifdef RF_EXP_NOSTORE
