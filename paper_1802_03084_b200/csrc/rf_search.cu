@@ -105,7 +105,8 @@ int launch_batch(rf_plan* p, const SearchParams& sp, cudaStream_t st) {
 template <int N> int tree_nbins(int) { return N <= 1024 ? 2048 : 4096; }
 
 template <int N> size_t smem_tree1(int ntiles) {
-    return (size_t)ntiles * (fft_padded_size(N) + 1) * sizeof(float2) + FftCfg<N>::TW_TOTAL * sizeof(float2);
+    return (size_t)ntiles * (fft_padded_size(N) + 1) * sizeof(float2) + FftCfg<N>::TW_TOTAL * sizeof(float2) +
+           (size_t)ntiles * FftCfg<N>::TPF * sizeof(uint32_t);
 }
 template <int N> constexpr int tree2_threads() { return N >= 2048 ? 256 : kThreads2; }
 template <int N, int TB> size_t smem_tree2(int nbins, int cpad, int nthreads = kThreads2) {
