@@ -176,7 +176,7 @@ int launch_tree_batch(rf_plan* p, TreeParams& tp, cudaStream_t st) {
     switch (key) {
 #define RF_TCASE(N, TB, NCOL, QH) case N * 16 + TB: tp.nbins = tree_nbins<N>(TB); return launch_tree<N, TB, NCOL, QH>(p, tp, st);
         RF_TCASE(256, 2, 16, 2) RF_TCASE(256, 4, 8, 4) RF_TCASE(256, 8, 4, 8)
-        RF_TCASE(512, 2, 8, 2) RF_TCASE(512, 4, 4, 4) RF_TCASE(512, 8, 2, 8)
+        RF_TCASE(512, 2, 8, 2) RF_TCASE(512, 4, 4, 4) RF_TCASE(512, 8, 2, 4)
         RF_TCASE(1024, 2, 4, 2) RF_TCASE(1024, 4, 2, 4) RF_TCASE(1024, 8, 2, 4)
         RF_TCASE(2048, 2, 2, 2) RF_TCASE(2048, 4, 2, 2)
         RF_TCASE(4096, 2, 2, 2) RF_TCASE(4096, 4, 2, 2)
