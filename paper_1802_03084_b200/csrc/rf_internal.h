@@ -53,8 +53,9 @@ struct BlockDesc {
     int32_t dm_idx, tb, nsearch, pad;
 };
 
-// Tree-path gather entry (4 bytes): one (baseline, channel) sample of one half-plane cell.
-//   bits 0..11 channel; bits 12..27 baseline; bit 28 EDGE: the cell lies on column 0 or N/2 (Parseval
+// Tree-path gather entry (8 bytes): one (baseline, channel) sample of one half-plane cell.
+//   x: (baseline * nchan + channel) * tpitch = offset of the sample's time series in visI (< 2^32, checked)
+//   y: bits 0..11 channel (for its delay); bit 28 EDGE: the cell lies on column 0 or N/2 (Parseval
 //   weight 1 instead of 2); bit 29 END: last iteration of its cell (every entry of that iteration
 //   carries it); bit 30 conjugate; bit 31 valid (0 = padding, weight 0).
 // Tree-path cell (4 bytes): bits 0..11 grid row; bits 12..15 column inside its column group;
@@ -69,7 +70,7 @@ struct GridLists {
 
 // Work lists of the boxcar-tree path (built by build_grid_lists, see rf_tables.cu).
 struct TreeLists {
-    uint32_t* entries = nullptr;     // device [n_iters * lg]
+    uint2* entries = nullptr;        // device [n_iters * lg]
     int32_t* stream_iter = nullptr;  // device [n_streams + 1] first iteration of each warp stream
     int32_t* stream_cell = nullptr;  // device [n_streams + 1] first cell of each warp stream
     uint32_t* cells = nullptr;       // device [n_cells] sorted by (column, row)

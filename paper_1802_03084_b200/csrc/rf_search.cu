@@ -581,7 +581,9 @@ int launch_time_fft_nt(rf_plan* p, int nt, int dm_idx, int slab_idx, cudaStream_
 
 int ensure_periodic_workspace(rf_plan* p, int nt_max, int n_dm_live) {
     Workspace& w = p->ws;
-    const size_t per_slab = (size_t)p->nbl * p->nchan * nt_max;
+    // the slab has the pitch of visI: the gather entries hold element * tpitch (nt_max <= nint < tpitch)
+    (void)nt_max;
+    const size_t per_slab = (size_t)p->nbl * p->nchan * p->tpitch;
     const size_t budget = (size_t)6 << 30;
     int n_slabs = (int)std::min<size_t>(8, std::max<size_t>(1, budget / (per_slab * sizeof(float2))));
     n_slabs = std::max(1, std::min(n_slabs, n_dm_live));
@@ -591,7 +593,7 @@ int ensure_periodic_workspace(rf_plan* p, int nt_max, int n_dm_live) {
         w.slab_elems = per_slab * n_slabs;
     }
     w.n_slabs = n_slabs;
-    w.slab_pitch = nt_max;
+    w.slab_pitch = p->tpitch;
     if (!w.zero_delay) {
         RF_CUDA_CHECK(cudaMalloc((void**)&w.zero_delay, (size_t)p->nchan * sizeof(int32_t)));
         RF_CUDA_CHECK(cudaMemset(w.zero_delay, 0, (size_t)p->nchan * sizeof(int32_t)));

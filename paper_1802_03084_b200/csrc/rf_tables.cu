@@ -214,11 +214,14 @@ int build_grid_lists(rf_plan* p) {
         tl.lg = LG;
         tl.cpad = (p->ncol + kColsPerGroup - 1) / kColsPerGroup * kColsPerGroup;
         tl.ngroups = tl.cpad / kColsPerGroup;
-        std::vector<uint32_t> entries, cells;
+        std::vector<uint2> entries;
+        std::vector<uint32_t> cells;
         std::vector<int32_t> stream_iter, stream_cell, group_cell(tl.ngroups + 1, 0);
         entries.reserve(raw.size() * 5 / 4 + 1024);
         int64_t iters = 0, stream_start = 0;
-        auto pad_entry = [&]() -> uint32_t { return raw.empty() ? 0u : (raw[0].ch | ((raw[0].elem / (uint32_t)p->nchan) << 12)); };   // a kept sample, weight 0
+        // entry = (row offset of the (baseline, channel) series in visI, channel | flags)
+        auto make_entry = [&](const Raw& r, uint32_t flags) { return make_uint2(r.elem * (uint32_t)p->tpitch, r.ch | flags); };
+        auto pad_entry = [&]() -> uint2 { return raw.empty() ? make_uint2(0u, 0u) : make_entry(raw[0], 0u); };   // a kept sample, weight 0
         auto close_stream = [&]() {
             for (; (iters - stream_start) % kTreeUnroll; iters++)
                 for (int j = 0; j < LG; j++) entries.push_back(pad_entry());
@@ -245,8 +248,8 @@ int build_grid_lists(rf_plan* p) {
                     const int k = it * LG + j;
                     const bool valid = k < n;
                     const Raw& r = raw[c0 + (valid ? k : 0)];        // padding repeats a kept sample, weight 0
-                    entries.push_back(r.ch | ((r.elem / (uint32_t)p->nchan) << 12) | (edge ? (1u << 28) : 0u) |
-                                      (it == cit - 1 ? (1u << 29) : 0u) | (r.conj << 30) | (valid ? (1u << 31) : 0u));
+                    entries.push_back(make_entry(r, (edge ? (1u << 28) : 0u) | (it == cit - 1 ? (1u << 29) : 0u) |
+                                                    (r.conj << 30) | (valid ? (1u << 31) : 0u)));
                 }
             iters += cit;
             c0 = c1;
@@ -303,6 +306,11 @@ void configure_tree(rf_plan* p) {
         if (p->tree_tb == 1) p->tree_tb = 2;      // the pair transform needs two integrations
     }
     p->tpitch = p->tree_tb ? ((p->nint + p->tree_tb + 15) / 16) * 16 : 0;
+    // gather entries hold (baseline * nchan + channel) * tpitch in 32 bits
+    if ((unsigned long long)p->nbl * p->nchan * p->tpitch >= (1ull << 32)) {
+        p->tree_tb = 0; p->tpitch = 0;
+        for (int l = 0; l < 4; l++) p->tree_dt_idx[l] = -1;
+    }
 }
 
 int build_image_list(rf_plan* p) {

@@ -26,7 +26,7 @@ namespace rf {
 struct TreeParams {
     const float2* visI;             // [nbl*nchan][tpitch]
     const int32_t* delay;           // [ndm][nchan]
-    const uint32_t* entries;        // gather entries, [n_iters][LG]
+    const uint2* entries;           // gather entries, [n_iters][LG]
     const int32_t* stream_iter;     // [n_streams + 1]
     const int32_t* stream_cell;     // [n_streams + 1]
     const uint32_t* cells;          // [n_cells]
@@ -119,7 +119,7 @@ __global__ void __launch_bounds__(256) k_sliding_sum(const float2* __restrict__ 
 // q), so sigma_rms of every image of the block is known before any pixel exists.
 // No tile, no barriers inside the loop, few registers: latency is hidden by occupancy.
 template <int TB>
-__global__ void __launch_bounds__(kThreads) k_tree_gather(const TreeParams p) {
+__global__ void __launch_bounds__(kThreads, 4) k_tree_gather(const TreeParams p) {
     constexpr int NIMG = 2 * TB - 1;
     constexpr int LG = 32 / TB, U = kTreeUnroll;
     constexpr int LEVELS = (TB == 8) ? 4 : (TB == 4 ? 3 : 2);      // log2(TB) + 1
@@ -137,9 +137,9 @@ __global__ void __launch_bounds__(kThreads) k_tree_gather(const TreeParams p) {
     const int it_end = has ? p.stream_iter[s + 1] : 0;
     int cell = has ? p.stream_cell[s] : 0;
     const int32_t* drow = p.delay + (size_t)(p.zero_row >= 0 ? p.zero_row : blk.dm_idx) * p.nchan;
-    uint32_t en[U];                        // entries of the next batch of iterations (prefetched)
+    uint2 en[U];                           // entries of the next batch of iterations (prefetched)
 #pragma unroll
-    for (int u = 0; u < U; u++) en[u] = 0u;
+    for (int u = 0; u < U; u++) en[u] = make_uint2(0u, 0u);
     if (it_beg < it_end) {
 #pragma unroll
         for (int u = 0; u < U; u++) en[u] = p.entries[(size_t)(it_beg + u) * LG + j];
@@ -150,6 +150,7 @@ __global__ void __launch_bounds__(kThreads) k_tree_gather(const TreeParams p) {
     float ps[LEVELS];
 #pragma unroll
     for (int l = 0; l < LEVELS; l++) ps[l] = 0.f;
+    // the sample of entry (x, y) is vbase[x + delay[channel(y)]]: one 32-bit add, one 64-bit scaled add
     const float2* vbase = p.visI + (size_t)blk.pad * p.slab_stride + blk.tb * TB + q;
     float2* cs = p.cellsum + (size_t)slot * p.n_cells * TB + q;
     float2 acc = make_float2(0.f, 0.f);
@@ -160,10 +161,10 @@ __global__ void __launch_bounds__(kThreads) k_tree_gather(const TreeParams p) {
         uint32_t e[U];
         float2 x[U];
 #pragma unroll
-        for (int u = 0; u < U; u++) e[u] = en[u];
-#pragma unroll
-        for (int u = 0; u < U; u++)
-            x[u] = __ldg(vbase + (size_t)(((e[u] >> 12) & 0xffffu) * p.nchan + (e[u] & 0xfffu)) * p.tpitch + sdelay[e[u] & 0xfffu]);
+        for (int u = 0; u < U; u++) {
+            e[u] = en[u].y;
+            x[u] = __ldg(vbase + (en[u].x + (uint32_t)sdelay[en[u].y & 0xfffu]));
+        }
         if (it + U < it_end) {
 #pragma unroll
             for (int u = 0; u < U; u++) en[u] = p.entries[(size_t)(it + U + u) * LG + j];
