@@ -341,7 +341,9 @@ __device__ __forceinline__ void tree_row_stats(const float (&x)[16], int img, in
     constexpr int TPF = N / 16;
     if (!cx.sValid[img]) return;
     const float A = cx.sA[img];
-    uint32_t* hw = cx.hist + (cx.wide ? img : (img >> 1)) * cx.nbins;
+    // 32-bit shared-memory address of this image's histogram, formed once: per pixel one scaled add + one RED
+    uint32_t hw = (uint32_t)__cvta_generic_to_shared(cx.hist) + (uint32_t)((cx.wide ? img : (img >> 1)) * cx.nbins) * 4u;
+    asm volatile("" : "+r"(hw));          // keep the sum in a register (the compiler re-forms it per pixel otherwise)
     const uint32_t inc = (!cx.wide && (img & 1)) ? 65536u : 1u;
     const unsigned nbm1 = (unsigned)cx.nbins - 1u;
     float m = x[0];
@@ -352,7 +354,7 @@ __device__ __forceinline__ void tree_row_stats(const float (&x)[16], int img, in
 #ifdef RF_EXP_NOHIST
         if (bin == 12345678u)
 #endif
-        atomicAdd(hw + min(bin, nbm1), inc);
+        asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(hw + min(bin, nbm1) * 4u), "r"(inc) : "memory");
         m = fmaxf(m, x[e]);
     }
     // running peak of this warp: a new maximum is rare after the first rows, so one vote decides.
