@@ -108,7 +108,7 @@ struct Workspace {
     int32_t* counters = nullptr;     // [4] device counters: stats_overflow, ...
     ImgDesc* dbg_desc = nullptr;     // one descriptor for rf_debug_image
     int batch = 0, rsplit = 1;
-    size_t h_elems = 0;
+    size_t cap_H = 0, cap_sumsq = 0, cap_hist = 0, cap_peak_val = 0, cap_peak_pos = 0, cap_ticket = 0;   // elements
     // boxcar-tree path
     float2* visI = nullptr;          // [nbl*nchan][tpitch] Stokes-I (pol sum), time fastest
     float2* Ht = nullptr;            // [blk_batch][npix][cpad_tree][TB]
@@ -203,7 +203,7 @@ int launch_cand_spectrum(rf_plan* p, const void* vis, int dm_idx, int dt_idx, in
 int launch_inject(rf_plan* p, void* vis, double amp, double l_pix, double m_pix, double dm, int width, int t0,
                   cudaStream_t st);
 // rf_search.cu
-int ensure_workspace(rf_plan* p);
+int ensure_workspace(rf_plan* p, bool need_generic);
 void free_workspace(rf_plan* p);
 // rf_search_host: the segment arrives in chunks of rows_per_chunk integrations (a multiple of 32); chunk c is
 // on the device once chunk_done[c] has fired

@@ -235,6 +235,19 @@ TreeParams tree_params(rf_plan* p) {
     return tp;
 }
 
+// Device buffers only ever grow (25 % headroom): the sizes follow the gridding lists, which change with every
+// rf_plan_set_uvw (streaming: once per segment), and a cudaFree / cudaMalloc pair synchronises the device.
+template <class T> int grow(T** ptr, size_t* cap, size_t need, bool zero = false) {
+    if (*ptr && *cap >= need) return RF_OK;
+    cudaFree(*ptr);
+    *ptr = nullptr;
+    const size_t want = need + need / 4 + 16;
+    RF_CUDA_CHECK(cudaMalloc((void**)ptr, want * sizeof(T)));
+    *cap = want;
+    if (zero) RF_CUDA_CHECK(cudaMemset(*ptr, 0, want * sizeof(T)));
+    return RF_OK;
+}
+
 int ensure_tree_workspace(rf_plan* p) {
     if (p->tree_tb == 0) return RF_OK;
     Workspace& w = p->ws;
@@ -257,12 +270,9 @@ int ensure_tree_workspace(rf_plan* p) {
         blk_batch = (int)std::min<size_t>(4096, std::max<size_t>(1, budget / (h_per_blk * sizeof(float2))));
         if (blk_batch > sms) blk_batch -= blk_batch % sms;
     }
-    if (!w.Ht || w.blk_batch != blk_batch || w.ht_elems != h_per_blk * blk_batch) {
-        cudaFree(w.Ht); w.Ht = nullptr;
-        RF_CUDA_CHECK(cudaMalloc((void**)&w.Ht, h_per_blk * blk_batch * sizeof(float2)));
-        w.blk_batch = blk_batch;
-        w.ht_elems = h_per_blk * blk_batch;
-    }
+    w.blk_batch = blk_batch;
+    int rc_grow = grow(&w.Ht, &w.ht_elems, h_per_blk * blk_batch);
+    if (rc_grow != RF_OK) return rc_grow;
     // compact grid and Parseval partials follow the gridding lists (uvw / flags may change them)
     const size_t cs_elems = (size_t)blk_batch * std::max(1, p->d.tree.n_cells) * p->tree_tb;
     if (!w.cellsum || w.cs_elems < cs_elems) {
@@ -346,14 +356,22 @@ void free_workspace(rf_plan* p) {
 }
 
 // Batch = images whose half-plane hand-off fits a fixed workspace budget; row split chosen so that
-// pass 2 launches at least two CTAs per SM.
-int ensure_workspace(rf_plan* p) {
+// pass 2 launches at least two CTAs per SM.  The per-image buffers exist only when the plan (or the debug hook)
+// sends images down that path.
+int ensure_workspace(rf_plan* p, bool need_generic) {
+    Workspace& w = p->ws;
     if (!p->d.twiddles) {
         float2 tw[16 + 256];
         host_twiddles(p->npix, tw);
         RF_CUDA_CHECK(cudaMalloc((void**)&p->d.twiddles, sizeof(tw)));
         RF_CUDA_CHECK(cudaMemcpy(p->d.twiddles, tw, sizeof(tw), cudaMemcpyHostToDevice));
     }
+    if (!w.counters) {
+        RF_CUDA_CHECK(cudaMalloc((void**)&w.counters, 4 * sizeof(int32_t)));
+        RF_CUDA_CHECK(cudaMemset(w.counters, 0, 4 * sizeof(int32_t)));
+        RF_CUDA_CHECK(cudaMalloc((void**)&w.dbg_desc, sizeof(ImgDesc)));
+    }
+    if (!need_generic) return RF_OK;
     const size_t h_per_img = (size_t)p->npix * p->d.gen.cpad;    // float2 elements
     int batch = p->user_batch;
     if (batch <= 0) {
@@ -371,28 +389,19 @@ int ensure_workspace(rf_plan* p) {
     while ((batch / 2) * rsplit < 2 * sms && rsplit * 2 <= max_split) rsplit *= 2;
     if (p->npix <= 128) rsplit = 1;                              // exact statistics keep whole images per CTA
     p->nbins = p->npix <= 256 ? 4096 : 2048;
-    Workspace& w = p->ws;
-    if (w.H && w.batch == batch && w.rsplit == rsplit && w.h_elems == h_per_img * batch) return RF_OK;
-    free_workspace(p);
     w.batch = batch;
     w.rsplit = rsplit;
-    w.h_elems = h_per_img * batch;
-    RF_CUDA_CHECK(cudaMalloc((void**)&w.H, w.h_elems * sizeof(float2)));
-    RF_CUDA_CHECK(cudaMalloc((void**)&w.sumsq, (size_t)batch * p->d.gen.ngroups * sizeof(float)));
-    RF_CUDA_CHECK(cudaMalloc((void**)&w.hist, (size_t)batch * p->nbins * sizeof(uint32_t)));
-    RF_CUDA_CHECK(cudaMalloc((void**)&w.peak_val, (size_t)batch * rsplit * sizeof(float)));
-    RF_CUDA_CHECK(cudaMalloc((void**)&w.peak_pos, (size_t)batch * rsplit * sizeof(int32_t)));
-    RF_CUDA_CHECK(cudaMalloc((void**)&w.ticket, (size_t)(batch / 2) * sizeof(uint32_t)));
-    RF_CUDA_CHECK(cudaMalloc((void**)&w.counters, 4 * sizeof(int32_t)));
-    RF_CUDA_CHECK(cudaMalloc((void**)&w.dbg_desc, sizeof(ImgDesc)));
-    RF_CUDA_CHECK(cudaMemset(w.hist, 0, (size_t)batch * p->nbins * sizeof(uint32_t)));
-    RF_CUDA_CHECK(cudaMemset(w.ticket, 0, (size_t)(batch / 2) * sizeof(uint32_t)));
-    RF_CUDA_CHECK(cudaMemset(w.counters, 0, 4 * sizeof(int32_t)));
-    return RF_OK;
+    int rc;
+    if ((rc = grow(&w.H, &w.cap_H, h_per_img * batch)) != RF_OK) return rc;
+    if ((rc = grow(&w.sumsq, &w.cap_sumsq, (size_t)batch * p->d.gen.ngroups)) != RF_OK) return rc;
+    if ((rc = grow(&w.hist, &w.cap_hist, (size_t)batch * p->nbins, true)) != RF_OK) return rc;   // kernels leave it zeroed
+    if ((rc = grow(&w.peak_val, &w.cap_peak_val, (size_t)batch * rsplit)) != RF_OK) return rc;
+    if ((rc = grow(&w.peak_pos, &w.cap_peak_pos, (size_t)batch * rsplit)) != RF_OK) return rc;
+    return grow(&w.ticket, &w.cap_ticket, (size_t)(batch / 2), true);
 }
 
 int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out, const HostFeed* feed) {
-    int rc = ensure_workspace(p);
+    int rc = ensure_workspace(p, p->n_gen_images > 0);
     if (rc == RF_OK) rc = ensure_tree_workspace(p);
     if (rc != RF_OK) return rc;
     RF_CUDA_CHECK(cudaMemsetAsync(out->count, 0, sizeof(int32_t), st));
@@ -488,7 +497,7 @@ int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out
 
 int launch_debug_image(rf_plan* p, const void* vis, int dm_idx, int dt_idx, int t_idx,
                        float* image_dev, rf_cand* stats_dev, cudaStream_t st) {
-    int rc = ensure_workspace(p);
+    int rc = ensure_workspace(p, true);
     if (rc == RF_OK) rc = ensure_tree_workspace(p);
     if (rc == RF_OK && p->meansub && p->n_kept > 0) rc = launch_time_mean(p, vis, st);
     if (rc != RF_OK) return rc;
@@ -617,7 +626,7 @@ int launch_search_periodic(rf_plan* p, const void* vis, cudaStream_t st, rf_cand
                   "a power-of-two width <= 8 in dt_list");
         return RF_ERR_STATE;
     }
-    int rc = ensure_workspace(p);
+    int rc = ensure_workspace(p, false);
     if (rc == RF_OK) rc = ensure_tree_workspace(p);
     if (rc != RF_OK) return rc;
     const bool dbg = dbg_dm >= 0;
