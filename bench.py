@@ -120,7 +120,9 @@ def _roofline(alg, k_ms, k_n, ms_per_step, traffic=None):
             "kernel_alg_gbs": {n: (alg["kind"][i] / (k_ms[i] * 1e-3) / 1e9 if k_ms[i] > 0 else 0.0)
                                for i, n in enumerate(names)},
             "path": {"alg_bytes_per_step": alg["total"], "achieved": path_gbs, "frac": path_gbs / peak,
-                     **_own_bytes(traffic, k_n, ms_per_step, peak)}}
+                     **_own_bytes(traffic, k_n, ms_per_step, peak)},
+            # what ncu says actually limits each kernel (the model bytes above are not what this design moves)
+            **({"limiters_ncu": traffic["limiters"]} if traffic and traffic.get("limiters") else {})}
 
 
 def _own_bytes(traffic, k_n, ms_per_step, peak):
@@ -315,7 +317,7 @@ def run_ours(args, cfg):
             with open(tpath) as fh:       # one ncu --set full capture of this launch configuration
                 tj = json.load(fh)
             traffic = {0: tj.get("pass1_dram_bytes_per_launch"), 1: tj.get("pass2_dram_bytes_per_launch"),
-                       3: tj.get("gather_dram_bytes_per_launch")}
+                       3: tj.get("gather_dram_bytes_per_launch"), "limiters": tj.get("limiters")}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
