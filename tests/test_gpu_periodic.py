@@ -124,3 +124,48 @@ def test_needs_the_tree_kernels():
     with pytest.raises(R.RealfastError):
         plan.search_periodic(d)
     plan.destroy()
+
+
+def test_lband_full_size_sampled():
+    """BASELINE.json configs[1] at full size (351 baselines x 256 channels, 1024 integrations, 512^2, 64 DM trials):
+    the whole rf_search_periodic, then sampled (dm, k) images against the oracle -- power image amplitude pixel by
+    pixel, S/N, peak pixel, presence in the candidate list; transform lengths 1024, 512 and 256 all occur."""
+    import torch
+    import paper_1802_03084_b200 as R
+    cfg = W.get_config("lband")
+    f, uvw, dms = W.channel_freqs_hz(cfg), W.baseline_uvw_m(cfg), W.dm_list(cfg)
+    cell = W.default_cell_rad(cfg, uvw)
+    plan = R.Plan(f, uvw, cfg.npol, cfg.nint, cfg.inttime_s, cfg.npix, cell, dms, cfg.dt_list, cfg.threshold)
+    d = torch.from_numpy(W.make_segment(cfg, inject=False)).cuda()
+    d_true = 20                                                      # a pulse train at trial 20's DM, period 16
+    for t0 in range(5, 700, 16):                                     # rf_inject has its own parity test (O9)
+        plan.inject(d, 0.06, -40, 25, float(dms[d_true]), 1, t0)
+    vis = d.cpu().numpy()                                            # both sides read these bytes
+    gpu, n = plan.search_periodic(d, capacity=1 << 16)
+    assert n == len(gpu) and plan.get_counters()["stats_overflow"] == 0
+    g = {(int(c["dm_idx"]), int(c["t_idx"])): c for c in gpu}
+    delays = O.delay_table(f, dms, cfg.inttime_s)
+    nts = [O.periodicity_nt(cfg.nint, int(delays[i].max())) for i in range(len(dms))]
+    assert [plan.periodic_nt(i) for i in range(len(dms))] == nts and {1024, 512, 256} <= set(nts)
+    iu, iv, keep = O.cell_table(uvw, f, cfg.npix, cell)
+    rng = np.random.default_rng(5)
+    found_harmonic = False
+    for dm_idx in (0, d_true, 63):
+        nt = nts[dm_idx]
+        spec = O.periodicity_spectrum(vis, delays[dm_idx], nt)
+        ks = sorted({1, nt // 2, nt // 16, 2 * (nt // 16)} | set(int(x) for x in rng.integers(1, nt // 2 + 1, 3)))
+        for k in ks:
+            img = O.periodicity_image(spec[k], iu, iv, keep, cfg.npix)
+            ref = img.real ** 2 + img.imag ** 2
+            amp, y, x, sigma, snr = O.periodicity_stats(ref)
+            got, st = plan.debug_periodic_image(d, dm_idx, k)
+            assert np.abs(np.sqrt(got) - np.sqrt(ref)).max() <= PIX_TOL * np.sqrt(ref.mean()), (dm_idx, k)
+            assert abs(float(st["snr"]) - snr) <= SNR_TOL * snr, (dm_idx, k)
+            lm = (x if x < cfg.npix // 2 else x - cfg.npix, y if y < cfg.npix // 2 else y - cfg.npix)
+            if snr > cfg.threshold * (1 + NEAR_THR):
+                assert (dm_idx, k) in g and (int(g[(dm_idx, k)]["l_pix"]), int(g[(dm_idx, k)]["m_pix"])) == lm
+                found_harmonic |= dm_idx == d_true and lm == (-40, 25)
+            elif snr < cfg.threshold * (1 - NEAR_THR):
+                assert (dm_idx, k) not in g
+    assert found_harmonic                                            # the pulse train is seen at its DM and pixel
+    plan.destroy()
