@@ -224,7 +224,10 @@ def run_ours(args, cfg):
     dev = torch.device("cuda", local)
 
     f, uvw, dms, cell = _setup(cfg)
-    vis = W.make_segment(cfg)                              # every rank: its own replica of the segment shape
+    # segment round-robin: rank r searches the r-th consecutive segment of the observation
+    # (its own noise rows; same array, band and trial grid), no data-path collective
+    import dataclasses
+    vis = W.make_segment(dataclasses.replace(cfg, stride_int=cfg.nint), segment=rank) if world > 1 else W.make_segment(cfg)
     hvis = torch.from_numpy(vis).pin_memory()
     dvis = hvis.to(dev, non_blocking=True)
     plan = R.Plan(f, uvw, cfg.npol, cfg.nint, cfg.inttime_s, cfg.npix, cell, dms, cfg.dt_list, cfg.threshold)
