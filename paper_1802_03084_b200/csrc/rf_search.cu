@@ -1,8 +1,9 @@
 // rf_search.cu -- workspace, kernel dispatch and the batch loop of rf_search.
 //
 // The search loop over (DM trial x sampling time x integration) (Fig. 2) is
-// flattened at plan time into a device-resident image list; rf_search walks it in batches
-// sized so that the half-plane hand-off H between the two FFT passes stays L2-resident.
+// flattened at plan time into device-resident work lists (blocks of the boxcar-tree path, images of the
+// per-image path); rf_search walks them in batches sized to whole waves of row-pass CTAs within a
+// workspace budget for the half-plane hand-off between the two FFT passes.
 #include <algorithm>
 #include <cstdio>
 #include <cstdlib>

@@ -211,19 +211,19 @@ __global__ void __launch_bounds__(kThreads, 4) k_tree_gather(const TreeParams p)
 }
 
 // ------------------------------------------------------------------------------------------
-// Tree pass 1: column FFTs.  grid = (ngroups, n_blk) -- the column groups of one block run together,
-// so their 32-byte pieces of one H line meet in L2 before the line is written back; block = 256.
-// Dynamic smem:  tile [TB*NCOL][PITCH] float2 (column f = q*NCOL + c) | tw
+// Tree pass 1: column FFTs.  grid = (ngroups, n_blk, TB/QH) -- the column groups of one block run together,
+// so their 32-byte pieces of one H line meet in L2 before the line is written back; block = NTH.
+// Dynamic smem:  tile [QH*NCOL][PITCH] float2 (column f = q*NCOL + c) | tw | occ [QH*NCOL][N/16] u32
 // The CTA scatters the cells of its NCOL uv columns, for QH of the block's TB integrations
-// (blockIdx.z selects which: QH < TB keeps two columns per CTA when N = 1024, i.e. whole 32-byte
-// sectors in the store), from the compact grid into zeroed tiles, transforms the QH*NCOL columns
-// in place (inverse, along v) and stores the half plane.
+// (blockIdx.z selects which: QH < TB keeps two columns per CTA, i.e. whole 32-byte sectors in the
+// store, with tiles small enough for four CTAs per SM), from the compact grid into its tiles,
+// transforms the QH*NCOL columns in place (inverse, along v) and stores the half plane.
 template <int N, int TB, int NCOL, int QH, int NTH>
 __global__ void __launch_bounds__(NTH) k_tree_colfft(const TreeParams p) {
     using C = FftCfg<N>;
     constexpr int PITCH = fft_padded_size(N) + 1;
     constexpr int NF = QH * NCOL;
-    constexpr int KPRE = 3;                // compact-grid values per thread loaded ahead of the tile clear
+    constexpr int KPRE = 3;                // compact-grid values per thread loaded before shared memory is touched
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2* tile = reinterpret_cast<float2*>(smem_raw);
     float2* tw = tile + NF * PITCH;
