@@ -125,9 +125,10 @@ int launch_tree(rf_plan* p, const TreeParams& tp, cudaStream_t st) {
     int rc;
     {
         auto kern = k_tree_gather<TB>;
-        const size_t smem = (size_t)p->nchan * sizeof(int) + (size_t)kWarpsPerCta * (2 * TB - 1) * sizeof(float);
+        const size_t smem = (size_t)p->nchan * sizeof(int) + (size_t)kWarpsPerCta * 2 * (2 * TB - 1) * sizeof(float);
+        if (tp.n_blk & 1) { set_error("internal: odd block count %d in a tree launch", tp.n_blk); return RF_ERR_STATE; }
         if ((rc = mark(p, st, -1)) != RF_OK) return rc;
-        kern<<<dim3(tp.n_parts, tp.n_blk), kThreads, smem, st>>>(tp);
+        kern<<<dim3(tp.n_parts, tp.n_blk / 2), kThreads, smem, st>>>(tp);
         RF_CUDA_CHECK(cudaGetLastError());
         if ((rc = mark(p, st, 3)) != RF_OK) return rc;
     }
@@ -223,6 +224,7 @@ TreeParams tree_params(rf_plan* p) {
     tp.sumsq = p->ws.sumsq_t;
     tp.counters = p->ws.counters;
     tp.dbg_img = -1;
+    tp.dbg_slot = 0;
     tp.zero_row = -1;
     tp.slab_stride = 0;
     tp.tpitch = p->tpitch;
@@ -271,6 +273,7 @@ int ensure_tree_workspace(rf_plan* p) {
         blk_batch = (int)std::min<size_t>(4096, std::max<size_t>(1, budget / (h_per_blk * sizeof(float2))));
         if (blk_batch > sms) blk_batch -= blk_batch % sms;
     }
+    blk_batch = std::max(2, blk_batch & ~1);          // launches hold whole block pairs
     w.blk_batch = blk_batch;
     int rc_grow = grow(&w.Ht, &w.ht_elems, h_per_blk * blk_batch);
     if (rc_grow != RF_OK) return rc_grow;
@@ -287,7 +290,7 @@ int ensure_tree_workspace(rf_plan* p) {
         RF_CUDA_CHECK(cudaMalloc((void**)&w.sumsq_t, (ss_elems + ss_elems / 8) * sizeof(float)));
         w.ss_elems = ss_elems + ss_elems / 8;
     }
-    if (!w.dbg_block) RF_CUDA_CHECK(cudaMalloc((void**)&w.dbg_block, sizeof(BlockDesc)));
+    if (!w.dbg_block) RF_CUDA_CHECK(cudaMalloc((void**)&w.dbg_block, 2 * sizeof(BlockDesc)));
     // sliding-sum arrays: one per width > 1 that is searched by the per-image path (bounded memory)
     std::vector<int32_t> slot(p->ndt, -1);
     int n_slots = 0;
@@ -449,8 +452,8 @@ int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out
             int dev = 0, sms = 148;
             cudaGetDevice(&dev);
             cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-            small = std::min(small, sms);
-            if (const char* e = getenv("RF_FEED_BATCH")) small = std::max(1, std::min(p->ws.blk_batch, atoi(e)));
+            small = std::min(small, sms) & ~1;
+            if (const char* e = getenv("RF_FEED_BATCH")) small = std::max(2, std::min(p->ws.blk_batch, atoi(e)) & ~1);
         }
         for (int64_t base = 0; base < p->n_blocks;) {
             int n = (int)std::min<int64_t>(p->ws.blk_batch, p->n_blocks - base);
@@ -508,13 +511,15 @@ int launch_debug_image(rf_plan* p, const void* vis, int dm_idx, int dt_idx, int 
         const int per = p->tree_tb >> l;
         int nsearch = p->nint - p->h_maxdelay[dm_idx];
         if (p->span > 0) nsearch = std::min(nsearch, p->span);
-        BlockDesc b{dm_idx, t_idx / per, nsearch, 0};
-        RF_CUDA_CHECK(cudaMemcpyAsync(p->ws.dbg_block, &b, sizeof(b), cudaMemcpyHostToDevice, st));
+        const int tb = t_idx / per;
+        BlockDesc b[2] = {{dm_idx, tb & ~1, nsearch, 0}, {dm_idx, tb | 1, nsearch, 0}};      // the block and its pair partner
+        RF_CUDA_CHECK(cudaMemcpyAsync(p->ws.dbg_block, b, sizeof(b), cudaMemcpyHostToDevice, st));
         RF_CUDA_CHECK(cudaStreamSynchronize(st));
         if ((rc = launch_prep(p, vis, st)) != RF_OK) return rc;
         TreeParams tp = tree_params(p);
         tp.blocks = p->ws.dbg_block;
-        tp.n_blk = 1;
+        tp.n_blk = 2;
+        tp.dbg_slot = tb & 1;
         tp.image_out = image_dev;
         tp.stats_out = stats_dev;
         tp.dbg_img = tree_off(p->tree_tb, l) + t_idx % per;
@@ -659,7 +664,7 @@ int launch_search_periodic(rf_plan* p, const void* vis, cudaStream_t st, rf_cand
         for (size_t i = c0; i < c1; i++) {
             const int nt = periodic_nt(p, dms[i]);
             for (int tb = 0; tb < nt / TB; tb++) {
-                if (dbg && tb != (dbg_k - 1) / nimg) continue;
+                if (dbg && (tb | 1) != (((dbg_k - 1) / nimg) | 1)) continue;      // the block and its pair partner
                 blocks.push_back({dms[i], tb, nt, (int)(i - c0)});
             }
         }
@@ -691,6 +696,7 @@ int launch_search_periodic(rf_plan* p, const void* vis, cudaStream_t st, rf_cand
         tp.image_out = power_dev;
         tp.stats_out = stats_dev;
         tp.dbg_img = (dbg_k - 1) % nimg;
+        tp.dbg_slot = ((dbg_k - 1) / nimg) & 1;
     }
     for (size_t c = 0; c + 1 < chunk_first.size(); c++) {
         const size_t c0 = c * w.n_slabs, c1 = std::min(dms.size(), c0 + w.n_slabs);

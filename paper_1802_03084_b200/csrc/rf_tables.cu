@@ -270,7 +270,7 @@ int build_grid_lists(rf_plan* p) {
         return upload(p, &tl.group_cell, group_cell.data(), group_cell.size());
     };
     int rc = emit(p->d.gen, cols_per_group(N));
-    if (rc == RF_OK && p->tree_tb > 0) rc = emit_tree(p->d.tree, tree_cols_per_group(N, p->tree_tb), 32 / p->tree_tb);
+    if (rc == RF_OK && p->tree_tb > 0) rc = emit_tree(p->d.tree, tree_cols_per_group(N, p->tree_tb), 16 / p->tree_tb);   // 2 TB lanes per entry
     if (rc == RF_OK) RF_CUDA_CHECK(cudaStreamSynchronize(p->tab_stream));
     return rc;
 }
@@ -305,7 +305,8 @@ void configure_tree(rf_plan* p) {
         }
         if (p->tree_tb == 1) p->tree_tb = 2;      // the pair transform needs two integrations
     }
-    p->tpitch = p->tree_tb ? ((p->nint + p->tree_tb + 15) / 16) * 16 : 0;
+    // read-ahead of the last block PAIR of a DM (the gather reads 2 TB integrations per entry)
+    p->tpitch = p->tree_tb ? ((p->nint + 2 * p->tree_tb + 15) / 16) * 16 : 0;
     // gather entries hold (baseline * nchan + channel) * tpitch in 32 bits
     if ((unsigned long long)p->nbl * p->nchan * p->tpitch >= (1ull << 32)) {
         p->tree_tb = 0; p->tpitch = 0;
@@ -371,28 +372,35 @@ int build_image_list(rf_plan* p) {
     // launch never needs rows beyond the deadline of its last block (h_block_deadline).
     p->h_block_deadline.clear();
     if (p->tree_tb > 0) {
+        const int TB = p->tree_tb;
+        // blocks per DM, rounded up to an even count: the gather kernel serves PAIRS of consecutive time blocks
+        // (slots 2y, 2y + 1 of a launch); the padding block lies past the searched range and holds no valid image
+        std::vector<int> nblk(p->ndm, 0);
+        for (int d = 0; d < p->ndm; d++)
+            if (in_tree_dm[d]) nblk[d] = (((nsearch_of[d] + TB - 1) / TB) + 1) & ~1;
         struct Unit { int g0, tb, deadline; };
         std::vector<Unit> units;
         for (int g0 = 0; g0 < p->ndm; g0 += dm_group) {
             const int g1 = std::min(p->ndm, g0 + dm_group);
-            int max_search = 0, sweep = 0;
+            int max_blk = 0, sweep = 0;
             for (int i = g0; i < g1; i++)
                 if (in_tree_dm[order[i]]) {
-                    max_search = std::max(max_search, nsearch_of[order[i]]);
+                    max_blk = std::max(max_blk, nblk[order[i]]);
                     sweep = std::max(sweep, p->h_maxdelay[order[i]]);
                 }
             // a unit = kUnitBlocks consecutive time blocks of the group: neighbouring blocks share 128-byte lines
-            for (int tb = 0; tb * p->tree_tb < max_search; tb += kUnitBlocks)
-                units.push_back({g0, tb, std::min(p->tpitch, (tb + kUnitBlocks) * p->tree_tb + sweep)});
+            for (int tb = 0; tb < max_blk; tb += kUnitBlocks)
+                units.push_back({g0, tb, std::min(p->tpitch, (tb + kUnitBlocks) * TB + sweep)});
         }
         std::stable_sort(units.begin(), units.end(), [](const Unit& a, const Unit& b) { return a.deadline < b.deadline; });
         for (const Unit& u : units) {
             const int g1 = std::min(p->ndm, u.g0 + dm_group);
-            for (int tb = u.tb; tb < u.tb + kUnitBlocks; tb++)
+            for (int tb = u.tb; tb < u.tb + kUnitBlocks; tb += 2)
                 for (int i = u.g0; i < g1; i++) {
                     const int d = order[i];
-                    if (in_tree_dm[d] && tb * p->tree_tb < nsearch_of[d]) {
-                        blocks.push_back({d, tb, nsearch_of[d], 0});
+                    if (tb >= nblk[d]) continue;
+                    for (int h = 0; h < 2; h++) {
+                        blocks.push_back({d, tb + h, nsearch_of[d], 0});
                         p->h_block_deadline.push_back(u.deadline);
                     }
                 }

@@ -43,6 +43,7 @@ struct TreeParams {
     float* image_out;               // debug: image `dbg_img` of block 0
     rf_cand* stats_out;
     int32_t dbg_img;                // -1 = off
+    int32_t dbg_slot;               // block of the launch the debug outputs refer to
     int32_t tpitch, nchan, ncol, cpad, ngroups, nbins, n_blk, n_cells, n_streams, n_parts;
     int32_t zero_row;               // >= 0: periodicity mode, every block uses this (all-zero) delay row
     long long slab_stride;          // periodicity mode: visI is [slab][nbl*nchan][tpitch], block.pad = slab
@@ -108,11 +109,14 @@ __global__ void __launch_bounds__(256) k_sliding_sum(const float2* __restrict__ 
 }
 
 // ------------------------------------------------------------------------------------------
-// Tree pass 0: gather + grid.  grid = (n_parts, n_blk); block = 256 = 8 warp streams.  Dynamic smem:
-//   sdelay [nchan] int | red [8][2*TB-1] float.
-// "Time in lanes": lane = (entry j = lane / TB, integration q = lane % TB).  One iteration reads
-// LG = 32/TB entries; the TB dedispersed samples of an entry are ONE coalesced 8*TB-byte read of
-// visI[bl*nchan + ch][t0 + delay[ch] + q].  The lane accumulates over the iterations of a cell in a
+// Tree pass 0: gather + grid.  grid = (n_parts, n_blk / 2); block = 256 = 8 warp streams.  Dynamic smem:
+//   sdelay [nchan] int | red [8][2][2*TB-1] float.
+// One CTA serves a PAIR of blocks: slots 2y and 2y + 1 of the launch are consecutive time blocks of the same
+// DM (build_image_list), i.e. 2 TB consecutive integrations.
+// "Time in lanes": lane = (entry j = lane / 2TB, block of the pair h = (lane / TB) & 1, integration q = lane % TB).
+// One iteration reads LG = 16/TB entries; the 2 TB dedispersed samples of an entry are ONE coalesced 16*TB-byte
+// read of visI[bl*nchan + ch][t0 + delay[ch] + 0 .. 2TB-1] (a warp load touches two 128-byte pieces instead of
+// four 64-byte ones: half the L1 wavefronts per byte).  The lane accumulates over the iterations of a cell in a
 // register; the END iteration sums the LG lane groups with xor shuffles and group 0 writes the cell
 // sum (TB contiguous complex values) to the compact grid.  Parseval sums of every boxcar-tree node,
 // sum_cells w |sum_{q in node} G_q|^2, are taken at the same place (another log2(TB) xor steps over
@@ -121,16 +125,16 @@ __global__ void __launch_bounds__(256) k_sliding_sum(const float2* __restrict__ 
 template <int TB>
 __global__ void __launch_bounds__(kThreads, 4) k_tree_gather(const TreeParams p) {
     constexpr int NIMG = 2 * TB - 1;
-    constexpr int LG = 32 / TB, U = kTreeUnroll;
+    constexpr int LG = 16 / TB, U = kTreeUnroll;
     constexpr int LEVELS = (TB == 8) ? 4 : (TB == 4 ? 3 : 2);      // log2(TB) + 1
     extern __shared__ __align__(16) unsigned char smem_raw[];
     int* sdelay = reinterpret_cast<int*>(smem_raw);
     float* red = reinterpret_cast<float*>(sdelay + p.nchan);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int part = blockIdx.x, slot = blockIdx.y;
+    const int part = blockIdx.x, slot = 2 * blockIdx.y;            // the pair (slot, slot + 1)
     const BlockDesc blk = p.blocks[slot];
-    const int j = lane / TB, q = lane % TB;
+    const int j = lane / (2 * TB), h = (lane / TB) & 1, q = lane % TB;
     const int s = part * kWarpsPerCta + warp;
     const bool has = s < p.n_streams;
     const int it_beg = has ? p.stream_iter[s] : 0;
@@ -151,8 +155,8 @@ __global__ void __launch_bounds__(kThreads, 4) k_tree_gather(const TreeParams p)
 #pragma unroll
     for (int l = 0; l < LEVELS; l++) ps[l] = 0.f;
     // the sample of entry (x, y) is vbase[x + delay[channel(y)]]: one 32-bit add, one 64-bit scaled add
-    const float2* vbase = p.visI + (size_t)blk.pad * p.slab_stride + blk.tb * TB + q;
-    float2* cs = p.cellsum + (size_t)slot * p.n_cells * TB + q;
+    const float2* vbase = p.visI + (size_t)blk.pad * p.slab_stride + blk.tb * TB + h * TB + q;
+    float2* cs = p.cellsum + (size_t)(slot + h) * p.n_cells * TB + q;
     float2 acc = make_float2(0.f, 0.f);
 #ifdef RF_EXP_NOGATHER
     if (p.nchan < 0)
@@ -177,7 +181,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_tree_gather(const TreeParams p)
             acc.y = fmaf(wi, x[u].y, acc.y);
             if (e[u] & (1u << 29)) {                                      // warp-uniform: cell complete
 #pragma unroll
-                for (int d = TB; d < 32; d <<= 1) {
+                for (int d = 2 * TB; d < 32; d <<= 1) {
                     acc.x += __shfl_xor_sync(0xffffffffu, acc.x, d);
                     acc.y += __shfl_xor_sync(0xffffffffu, acc.y, d);
                 }
@@ -195,18 +199,19 @@ __global__ void __launch_bounds__(kThreads, 4) k_tree_gather(const TreeParams p)
             }
         }
     }
-    // node (level l, i) is held by the lanes of group 0 with q >> l == i (all of them hold the same sum)
+    // node (level l, i) of block h is held by the lanes of group 0 with q >> l == i (all of them hold the same sum)
     if (j == 0) {
 #pragma unroll
         for (int l = 0; l < LEVELS; l++)
-            if ((q & ((1 << l) - 1)) == 0) red[warp * NIMG + tree_off(TB, l) + (q >> l)] = ps[l];
+            if ((q & ((1 << l) - 1)) == 0) red[(warp * 2 + h) * NIMG + tree_off(TB, l) + (q >> l)] = ps[l];
     }
     __syncthreads();
-    if (tid < NIMG) {
+    if (tid < 2 * NIMG) {
+        const int hh = tid / NIMG, node = tid % NIMG;
         float tot = 0.f;
 #pragma unroll
-        for (int w = 0; w < kWarpsPerCta; w++) tot += red[w * NIMG + tid];
-        p.sumsq[((size_t)slot * NIMG + tid) * p.n_parts + part] = tot * p.norm * p.norm;
+        for (int w = 0; w < kWarpsPerCta; w++) tot += red[(w * 2 + hh) * NIMG + node];
+        p.sumsq[((size_t)(slot + hh) * NIMG + node) * p.n_parts + part] = tot * p.norm * p.norm;
     }
 }
 
@@ -455,7 +460,7 @@ __global__ void __launch_bounds__(NT2, NT2 == 512 ? 1 : 2) k_tree_rowfft_stats(c
 
     TreeStatsCtx<C::TPF> cx{hist, sA, sScale, sValid, sBest, sBpos, 0.5f * (float)p.nbins, p.nbins, NIMG, WIDE};
     float2* xb = xbuf + grp * XB;
-    const bool dbg = p.image_out != nullptr && slot == 0;
+    const bool dbg = p.image_out != nullptr && slot == p.dbg_slot;
 
     for (int y = grp; y < N; y += G2) {
         float s2p[16], s4p[16];
@@ -521,7 +526,7 @@ __global__ void __launch_bounds__(NT2, NT2 == 512 ? 1 : 2) k_tree_rowfft_stats(c
 
     // ---- per image: unpack the histogram, prefix sums, median / MAD, S/N, threshold
     for (int img = 0; img < NIMG; img++) {
-        const bool report_zero = p.stats_out != nullptr && slot == 0 && img == p.dbg_img;
+        const bool report_zero = p.stats_out != nullptr && slot == p.dbg_slot && img == p.dbg_img;
         if (!sValid[img] && !report_zero) continue;            // block-uniform
         const uint32_t* hw = hist + (WIDE ? img : (img >> 1)) * p.nbins;
         const int sh = WIDE ? 0 : (img & 1) * 16;
@@ -687,7 +692,7 @@ __global__ void __launch_bounds__(kThreads2, 1) k_tree_rowfft_power(const TreePa
 
     TreeStatsCtx<C::TPF> cx{hist, sA, sScale, sValid, sBest, sBpos, 0.f, p.nbins, NSL, false};
     float2* xb = xbuf + grp * XB;
-    const bool dbg = p.image_out != nullptr && slot == 0;
+    const bool dbg = p.image_out != nullptr && slot == p.dbg_slot;
     for (int y = grp; y < N; y += G2) {
 #pragma unroll 1
         for (int p2 = 0; p2 < TB / 2; p2++) {
@@ -721,7 +726,7 @@ __global__ void __launch_bounds__(kThreads2, 1) k_tree_rowfft_power(const TreePa
 
     for (int img = 0; img < NIMG; img++) {
         const int si = 2 * img;
-        const bool report_zero = p.stats_out != nullptr && slot == 0 && img == p.dbg_img;
+        const bool report_zero = p.stats_out != nullptr && slot == p.dbg_slot && img == p.dbg_img;
         if (!sValid[si] && !report_zero) continue;
         const uint32_t* hw = hist + (size_t)img * p.nbins;
         const int per = p.nbins / kThreads2;
