@@ -54,10 +54,11 @@ struct BlockDesc {
 };
 
 // Tree-path gather entry (8 bytes): one (baseline, channel) sample of one half-plane cell.
-//   x: (baseline * nchan + channel) * tpitch = offset of the sample's time series in visI (< 2^32, checked)
+//   x: (baseline * nchan + channel) * tpitch = offset of the sample's time series in visI (< 2^32, checked);
+//      padding entries point at the all-zero series that follows the last one
 //   y: bits 0..11 channel (for its delay); bit 28 EDGE: the cell lies on column 0 or N/2 (Parseval
 //   weight 1 instead of 2); bit 29 END: last iteration of its cell (every entry of that iteration
-//   carries it); bit 30 conjugate; bit 31 valid (0 = padding, weight 0).
+//   carries it); bit 31 conjugate (= the sign bit of the imaginary part).
 // Tree-path cell (4 bytes): bits 0..11 grid row; bits 12..15 column inside its column group;
 //   bit 16: the cell lies on column 0 or N/2 (Parseval weight 1 instead of 2).
 // Half-plane gridding lists for one choice of columns-per-CTA.

@@ -254,10 +254,12 @@ template <class T> int grow(T** ptr, size_t* cap, size_t need, bool zero = false
 int ensure_tree_workspace(rf_plan* p) {
     if (p->tree_tb == 0) return RF_OK;
     Workspace& w = p->ws;
-    const size_t visI_elems = (size_t)p->nbl * p->nchan * p->tpitch;
+    // one extra, all-zero series after the last (baseline, channel): the padding entries of the gather read it
+    const size_t visI_elems = ((size_t)p->nbl * p->nchan + 1) * p->tpitch;
     if (!w.visI || w.visI_elems != visI_elems) {
         cudaFree(w.visI); w.visI = nullptr;
         RF_CUDA_CHECK(cudaMalloc((void**)&w.visI, visI_elems * sizeof(float2)));
+        RF_CUDA_CHECK(cudaMemset(w.visI, 0, visI_elems * sizeof(float2)));
         w.visI_elems = visI_elems;
     }
     const size_t h_per_blk = (size_t)p->npix * p->d.tree.cpad * p->tree_tb;   // float2 elements
@@ -580,7 +582,7 @@ int launch_time_fft_nt(rf_plan* p, int nt, int dm_idx, int slab_idx, cudaStream_
     while ((64 << lg) < nt) lg++;
     const float2* tw = p->ws.time_tw + (size_t)lg * (16 + 256);
     const int32_t* dd = p->d.delay + (size_t)dm_idx * p->nchan;
-    float2* slab = p->ws.slab + (size_t)slab_idx * p->nbl * p->nchan * p->ws.slab_pitch;
+    float2* slab = p->ws.slab + (size_t)slab_idx * ((size_t)p->nbl * p->nchan + 1) * p->ws.slab_pitch;
     switch (nt) {
         case 64: return launch_time_fft<64>(p, dd, tw, slab, st);
         case 128: return launch_time_fft<128>(p, dd, tw, slab, st);
@@ -598,13 +600,14 @@ int ensure_periodic_workspace(rf_plan* p, int nt_max, int n_dm_live) {
     Workspace& w = p->ws;
     // the slab has the pitch of visI: the gather entries hold element * tpitch (nt_max <= nint < tpitch)
     (void)nt_max;
-    const size_t per_slab = (size_t)p->nbl * p->nchan * p->tpitch;
+    const size_t per_slab = ((size_t)p->nbl * p->nchan + 1) * p->tpitch;       // incl. the all-zero series (see visI)
     const size_t budget = (size_t)6 << 30;
     int n_slabs = (int)std::min<size_t>(8, std::max<size_t>(1, budget / (per_slab * sizeof(float2))));
     n_slabs = std::max(1, std::min(n_slabs, n_dm_live));
     if (!w.slab || w.slab_elems < per_slab * n_slabs) {
         cudaFree(w.slab); w.slab = nullptr;
         RF_CUDA_CHECK(cudaMalloc((void**)&w.slab, per_slab * n_slabs * sizeof(float2)));
+        RF_CUDA_CHECK(cudaMemset(w.slab, 0, per_slab * n_slabs * sizeof(float2)));
         w.slab_elems = per_slab * n_slabs;
     }
     w.n_slabs = n_slabs;
@@ -688,7 +691,7 @@ int launch_search_periodic(rf_plan* p, const void* vis, cudaStream_t st, rf_cand
     tp.delay = w.zero_delay;
     tp.zero_row = 0;
     tp.tpitch = w.slab_pitch;
-    tp.slab_stride = (long long)p->nbl * p->nchan * w.slab_pitch;
+    tp.slab_stride = ((long long)p->nbl * p->nchan + 1) * w.slab_pitch;
     tp.cand_items = out ? out->items : nullptr;
     tp.cand_count = out ? out->count : nullptr;
     tp.cand_capacity = out ? out->capacity : 0;

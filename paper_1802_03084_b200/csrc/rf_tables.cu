@@ -221,7 +221,8 @@ int build_grid_lists(rf_plan* p) {
         int64_t iters = 0, stream_start = 0;
         // entry = (row offset of the (baseline, channel) series in visI, channel | flags)
         auto make_entry = [&](const Raw& r, uint32_t flags) { return make_uint2(r.elem * (uint32_t)p->tpitch, r.ch | flags); };
-        auto pad_entry = [&]() -> uint2 { return raw.empty() ? make_uint2(0u, 0u) : make_entry(raw[0], 0u); };   // a kept sample, weight 0
+        // padding reads the all-zero series that follows the last (baseline, channel) in visI
+        auto pad_entry = [&]() -> uint2 { return make_uint2((uint32_t)p->nbl * (uint32_t)p->nchan * (uint32_t)p->tpitch, 0u); };
         auto close_stream = [&]() {
             for (; (iters - stream_start) % kTreeUnroll; iters++)
                 for (int j = 0; j < LG; j++) entries.push_back(pad_entry());
@@ -247,9 +248,9 @@ int build_grid_lists(rf_plan* p) {
                 for (int j = 0; j < LG; j++) {
                     const int k = it * LG + j;
                     const bool valid = k < n;
-                    const Raw& r = raw[c0 + (valid ? k : 0)];        // padding repeats a kept sample, weight 0
-                    entries.push_back(make_entry(r, (edge ? (1u << 28) : 0u) | (it == cit - 1 ? (1u << 29) : 0u) |
-                                                    (r.conj << 30) | (valid ? (1u << 31) : 0u)));
+                    const uint32_t flags = (edge ? (1u << 28) : 0u) | (it == cit - 1 ? (1u << 29) : 0u);
+                    if (valid) entries.push_back(make_entry(raw[c0 + k], flags | (raw[c0 + k].conj << 31)));
+                    else { uint2 e = pad_entry(); e.y |= flags; entries.push_back(e); }
                 }
             iters += cit;
             c0 = c1;
@@ -308,7 +309,7 @@ void configure_tree(rf_plan* p) {
     // read-ahead of the last block PAIR of a DM (the gather reads 2 TB integrations per entry)
     p->tpitch = p->tree_tb ? ((p->nint + 2 * p->tree_tb + 15) / 16) * 16 : 0;
     // gather entries hold (baseline * nchan + channel) * tpitch in 32 bits
-    if ((unsigned long long)p->nbl * p->nchan * p->tpitch >= (1ull << 32)) {
+    if (((unsigned long long)p->nbl * p->nchan + 1) * p->tpitch >= (1ull << 32)) {
         p->tree_tb = 0; p->tpitch = 0;
         for (int l = 0; l < 4; l++) p->tree_dt_idx[l] = -1;
     }

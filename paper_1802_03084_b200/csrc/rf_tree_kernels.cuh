@@ -175,10 +175,8 @@ __global__ void __launch_bounds__(kThreads, 4) k_tree_gather(const TreeParams p)
         }
 #pragma unroll
         for (int u = 0; u < U; u++) {
-            const float wr = (e[u] >> 31) ? 1.f : 0.f;                    // padding: weight 0
-            const float wi = (e[u] & (1u << 30)) ? -wr : wr;              // conjugate
-            acc.x = fmaf(wr, x[u].x, acc.x);
-            acc.y = fmaf(wi, x[u].y, acc.y);
+            acc.x += x[u].x;                                              // padding entries read zeros
+            acc.y += __uint_as_float(__float_as_uint(x[u].y) ^ (e[u] & 0x80000000u));     // conjugate: bit 31
             if (e[u] & (1u << 29)) {                                      // warp-uniform: cell complete
 #pragma unroll
                 for (int d = 2 * TB; d < 32; d <<= 1) {
