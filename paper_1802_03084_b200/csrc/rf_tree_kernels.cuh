@@ -156,6 +156,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_tree_gather(const TreeParams p)
     for (int l = 0; l < LEVELS; l++) ps[l] = 0.f;
     // the sample of entry (x, y) is vbase[x + delay[channel(y)]]: one 32-bit add, one 64-bit scaled add
     const float2* vbase = p.visI + (size_t)blk.pad * p.slab_stride + blk.tb * TB + h * TB + q;
+    asm volatile("" : "+l"(vbase));     // one register pointer: a sample's address is then a single 32 x 8 + 64-bit multiply-add
     float2* cs = p.cellsum + (size_t)(slot + h) * p.n_cells * TB + q;
     float2 acc = make_float2(0.f, 0.f);
 #ifdef RF_EXP_NOGATHER
