@@ -204,8 +204,8 @@ int rf_inject(rf_plan* plan, void* vis_dev, double amp, double l_pix, double m_p
  * sqrt(median(P)/ln 2), snr = peak/sigma.  Candidates with snr >= threshold are appended to cand_out with
  * dt_idx = -1 and t_idx = k (fluctuation frequency k/(NT inttime) Hz).  Honours rf_plan_set_meansub and
  * the channel weights; ignores the search span.  Needs a plan on the boxcar-tree kernels (npix >= 256
- * and a power-of-two width <= 8 in dt_list), else RF_ERR_STATE.  Enqueues on cuda_stream; one host
- * synchronisation at entry (block-list upload), none after the first kernel.
+ * and a power-of-two width <= 8 in dt_list), else RF_ERR_STATE.  Enqueues on cuda_stream; the first call of a
+ * plan (and the first after the debug hook) synchronises once to upload its block list, later calls do not.
  *   rf_debug_periodic_image: power image [npix][npix] (float32, DEVICE) and/or statistics of one
  *   (dm_idx, k), through the same kernels.                                                          */
 int rf_search_periodic(rf_plan* plan, const void* vis_dev, void* cuda_stream, rf_cand_out* cand_out);

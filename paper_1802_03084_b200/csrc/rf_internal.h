@@ -128,6 +128,7 @@ struct Workspace {
     size_t slab_elems = 0;
     int n_slabs = 0, slab_pitch = 0;
     BlockDesc* pblocks = nullptr;    // block list of the periodicity search
+    std::vector<BlockDesc> h_pblocks; // its host copy (re-uploaded only when it changes)
     size_t pblocks_cap = 0;
     int32_t* zero_delay = nullptr;   // [nchan] zeros: the slabs are already dedispersed
     float2* time_tw = nullptr;       // [7][16 + 256] twiddles of the time transforms, NT = 64 << i

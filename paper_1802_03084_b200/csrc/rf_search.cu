@@ -7,6 +7,7 @@
 #include <algorithm>
 #include <cstdio>
 #include <cstdlib>
+#include <cstring>
 
 #include "rf_tree_kernels.cuh"
 
@@ -673,13 +674,20 @@ int launch_search_periodic(rf_plan* p, const void* vis, cudaStream_t st, rf_cand
         }
     }
     chunk_first.push_back(blocks.size());
-    if (!w.pblocks || w.pblocks_cap < blocks.size()) {
-        cudaFree(w.pblocks); w.pblocks = nullptr;
-        RF_CUDA_CHECK(cudaMalloc((void**)&w.pblocks, blocks.size() * sizeof(BlockDesc)));
-        w.pblocks_cap = blocks.size();
+    // uploaded only when it differs from the list already on the device (first call, debug hook, new geometry):
+    // repeated searches of a plan enqueue without synchronising
+    const bool same = w.pblocks && w.h_pblocks.size() == blocks.size() &&
+                      memcmp(w.h_pblocks.data(), blocks.data(), blocks.size() * sizeof(BlockDesc)) == 0;
+    if (!same) {
+        if (!w.pblocks || w.pblocks_cap < blocks.size()) {
+            cudaFree(w.pblocks); w.pblocks = nullptr;
+            RF_CUDA_CHECK(cudaMalloc((void**)&w.pblocks, blocks.size() * sizeof(BlockDesc)));
+            w.pblocks_cap = blocks.size();
+        }
+        RF_CUDA_CHECK(cudaStreamSynchronize(st));  // an earlier search on this stream may still read the old list
+        RF_CUDA_CHECK(cudaMemcpy(w.pblocks, blocks.data(), blocks.size() * sizeof(BlockDesc), cudaMemcpyHostToDevice));
+        w.h_pblocks = blocks;
     }
-    RF_CUDA_CHECK(cudaMemcpyAsync(w.pblocks, blocks.data(), blocks.size() * sizeof(BlockDesc), cudaMemcpyHostToDevice, st));
-    RF_CUDA_CHECK(cudaStreamSynchronize(st));      // `blocks` lives on this stack frame
     if (p->meansub) {
         if ((rc = launch_time_mean(p, vis, st)) != RF_OK) return rc;
         p->last_launches += 2;
