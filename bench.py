@@ -207,6 +207,18 @@ def run_reference(args, cfg):
     print(json.dumps(line), flush=True)
 
 
+def _ensure_built(local_rank: int) -> None:
+    """A fresh checkout has no librealfast_b200.so (built artefacts are not in the history): local rank 0 compiles
+    it (nvcc, sm_100a; a no-op when it is up to date), the other ranks wait for it."""
+    from paper_1802_03084_b200 import build as _b
+    if local_rank == 0:
+        _b.build()
+        return
+    t0 = time.time()
+    while _b.needs_build() and time.time() - t0 < 600:
+        time.sleep(1.0)
+
+
 def run_ours(args, cfg):
     import torch
     import torch.distributed as dist
@@ -218,6 +230,7 @@ def run_ours(args, cfg):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    _ensure_built(local)
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
@@ -382,6 +395,7 @@ def run_stream(args, cfg):
         raise SystemExit("--config stream is a single-GPU measurement (replicas: run one per GPU)")
     dev = torch.device("cuda", 0)
     torch.cuda.set_device(dev)
+    _ensure_built(0)
     nseg_cfg = cfg.n_segments
     n_warm, n_timed = args.warmup, args.steps
     n_total = n_warm + n_timed
