@@ -136,11 +136,10 @@ def test_lband_full_size_sampled():
     f, uvw, dms = W.channel_freqs_hz(cfg), W.baseline_uvw_m(cfg), W.dm_list(cfg)
     cell = W.default_cell_rad(cfg, uvw)
     plan = R.Plan(f, uvw, cfg.npol, cfg.nint, cfg.inttime_s, cfg.npix, cell, dms, cfg.dt_list, cfg.threshold)
-    d = torch.from_numpy(W.make_segment(cfg, inject=False)).cuda()
     d_true = 20                                                      # a pulse train at trial 20's DM, period 16
-    for t0 in range(5, 700, 16):                                     # rf_inject has its own parity test (O9)
-        plan.inject(d, 0.06, -40, 25, float(dms[d_true]), 1, t0)
-    vis = d.cpu().numpy()                                            # both sides read these bytes
+    train = [W.generate.Transient(0.06, -40, 25, float(dms[d_true]), 1, t0) for t0 in range(5, 700, 16)]
+    vis = W.make_segment(cfg, sources=train)                         # the seeded generator: both sides read these bytes
+    d = torch.from_numpy(vis).cuda()
     gpu, n = plan.search_periodic(d, capacity=1 << 16)
     assert n == len(gpu) and plan.get_counters()["stats_overflow"] == 0
     g = {(int(c["dm_idx"]), int(c["t_idx"])): c for c in gpu}
