@@ -27,6 +27,7 @@ inline int cols_per_group(int npix) { return npix <= 512 ? 16 : (npix == 1024 ? 
 constexpr int kWarpsPerCta = 8;     // 256 threads everywhere
 constexpr int kThreads = 32 * kWarpsPerCta;
 constexpr int kDmGroup = 8;         // DM trials interleaved in time by the tree path's block order
+constexpr size_t kSlidingSumBudget = (size_t)24 << 30;   // bytes of sliding-sum arrays (widths off the tree) per plan
 constexpr int kUnitBlocks = 4;      // consecutive time blocks of a DM group kept together in the tree path's block order
 constexpr int kTreeUnroll = 8;      // iterations of the tree gather kept in flight per warp
 constexpr int kStreamIters = 64;    // target length of one warp stream of the tree gather
@@ -89,6 +90,8 @@ struct DeviceTables {
     // gridding lists: generic path (colgrp = cols_per_group) and boxcar-tree path
     GridLists gen;
     TreeLists tree;
+    TreeLists tree2;                 // TB = 2 lists for the widths off the tree (pairs of pre-summed images)
+    BlockDesc* blocks2 = nullptr;    // their blocks, all such widths one after the other (rf_plan::aux_first)
     ImgDesc* images = nullptr;       // [n_gen_images] images searched by the generic path
     BlockDesc* blocks = nullptr;     // [n_blocks] blocks searched by the tree path
     // plan inputs on device
@@ -156,6 +159,8 @@ struct rf_plan {
     std::vector<uint8_t> h_keep;
     std::vector<int32_t> h_maxdelay;           // [ndm]
     std::vector<int32_t> h_num_t;              // [ndm][ndt]
+    std::vector<int32_t> aux_width;            // [ndt] 1 = width off the tree searched as TB = 2 blocks of sliding sums
+    std::vector<int64_t> aux_first;            // [ndt + 1] first block of each width in d.blocks2
     std::vector<int32_t> h_block_deadline;     // [n_blocks] integrations [0, deadline) are all a tree block (and those before it) read
     // derived
     int n_kept = 0, n_dropped = 0;

@@ -174,8 +174,9 @@ int launch_tree(rf_plan* p, const TreeParams& tp, cudaStream_t st) {
     return RF_OK;
 }
 
-int launch_tree_batch(rf_plan* p, TreeParams& tp, cudaStream_t st) {
-    const int key = p->npix * 16 + p->tree_tb;
+int launch_tree_batch(rf_plan* p, TreeParams& tp, cudaStream_t st, int tb = 0) {
+    if (tb == 0) tb = p->tree_tb;
+    const int key = p->npix * 16 + tb;
     switch (key) {
 #define RF_TCASE(N, TB, NCOL, QH) case N * 16 + TB: tp.nbins = tree_nbins<N>(TB); return launch_tree<N, TB, NCOL, QH>(p, tp, st);
         RF_TCASE(256, 2, 16, 2) RF_TCASE(256, 4, 8, 4) RF_TCASE(256, 8, 4, 8)
@@ -185,7 +186,7 @@ int launch_tree_batch(rf_plan* p, TreeParams& tp, cudaStream_t st) {
         RF_TCASE(4096, 2, 2, 2) RF_TCASE(4096, 4, 2, 2)
 #undef RF_TCASE
     }
-    set_error("unsupported tree configuration npix %d tb %d", p->npix, p->tree_tb);
+    set_error("unsupported tree configuration npix %d tb %d", p->npix, tb);
     return RF_ERR_ARG;
 }
 
@@ -227,6 +228,7 @@ TreeParams tree_params(rf_plan* p) {
     tp.dbg_img = -1;
     tp.dbg_slot = 0;
     tp.zero_row = -1;
+    tp.q_stride = 1;
     tp.slab_stride = 0;
     tp.tpitch = p->tpitch;
     tp.nchan = p->nchan;
@@ -297,7 +299,7 @@ int ensure_tree_workspace(rf_plan* p) {
     // sliding-sum arrays: one per width > 1 that is searched by the per-image path (bounded memory)
     std::vector<int32_t> slot(p->ndt, -1);
     int n_slots = 0;
-    const size_t budget = (size_t)24 << 30;
+    const size_t budget = kSlidingSumBudget;
     for (int k = 0; k < p->ndt; k++) {
         bool in_tree = false;
         for (int l = 0; l < 4; l++) in_tree |= (p->tree_dt_idx[l] == k);
@@ -312,10 +314,15 @@ int ensure_tree_workspace(rf_plan* p) {
         w.h_gen_slot = slot;
     }
     w.n_gen_slots = n_slots;
-    if (n_slots > 0 && (!w.visS || w.visS_elems < (size_t)n_slots * visI_elems)) {
+    // tail: the padding block pairs of the TB = 2 pass read up to 2 dt integrations past the end of a series
+    // (into the next one; past the last one here) -- their images are invalid but must be finite (pair transform)
+    size_t tail = 64;
+    for (int k = 0; k < p->ndt; k++) if (slot[k] >= 0) tail = std::max(tail, (size_t)4 * p->dts[k] + 64);
+    if (n_slots > 0 && (!w.visS || w.visS_elems < (size_t)n_slots * visI_elems + tail)) {
         cudaFree(w.visS); w.visS = nullptr;
-        RF_CUDA_CHECK(cudaMalloc((void**)&w.visS, (size_t)n_slots * visI_elems * sizeof(float2)));
-        w.visS_elems = (size_t)n_slots * visI_elems;
+        RF_CUDA_CHECK(cudaMalloc((void**)&w.visS, ((size_t)n_slots * visI_elems + tail) * sizeof(float2)));
+        RF_CUDA_CHECK(cudaMemset(w.visS, 0, ((size_t)n_slots * visI_elems + tail) * sizeof(float2)));
+        w.visS_elems = (size_t)n_slots * visI_elems + tail;
     }
     return RF_OK;
 }
@@ -469,12 +476,8 @@ int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out
             base += n;
         }
         if ((rc = need_rows(p->tpitch)) != RF_OK) return rc;      // widths off the tree read the whole array
-    }
-    // ---- every other width: one gridding + transform per image
-    SearchParams sp = base_params(p, vis);
-    if (p->tree_tb > 0 && p->n_blocks > 0) {
-        sp.visI = p->ws.visI;     // transposed above for the tree path
-        if (p->ws.n_gen_slots > 0 && p->n_gen_images > 0) {
+        // ---- widths off the tree: sliding sums once per segment (B7) ...
+        if (p->ws.n_gen_slots > 0) {
             if ((rc = mark(p, st, -1)) != RF_OK) return rc;
             for (int k = 0; k < p->ndt; k++) {
                 const int sl = p->ws.h_gen_slot[k];
@@ -485,6 +488,48 @@ int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out
                 p->last_launches += 1;
             }
             if ((rc = mark(p, st, 2)) != RF_OK) return rc;
+        }
+        // ---- ... searched by the tree kernels as blocks of two consecutive output integrations (stride dt)
+        for (int k = 0; k < p->ndt; k++) {
+            const int sl = p->ws.h_gen_slot[k];
+            const int64_t nb2 = p->aux_first[k + 1] - p->aux_first[k];
+            if (!p->aux_width[k] || sl < 0 || nb2 == 0) continue;
+            TreeParams t2 = tree_params(p);
+            const TreeLists& l2 = p->d.tree2;
+            t2.entries = l2.entries; t2.stream_iter = l2.stream_iter; t2.stream_cell = l2.stream_cell;
+            t2.cells = l2.cells; t2.group_cell = l2.group_cell;
+            t2.n_cells = l2.n_cells; t2.n_streams = l2.n_streams; t2.n_parts = l2.n_parts;
+            t2.cpad = l2.cpad; t2.ngroups = l2.ngroups;
+            t2.visI = p->ws.visS + (size_t)sl * p->ws.visI_elems;
+            t2.q_stride = p->dts[k];
+            t2.dt_idx[0] = k;
+            for (int l = 1; l < 4; l++) t2.dt_idx[l] = -1;
+            t2.norm = tp.norm / (float)p->dts[k];
+            t2.cand_items = out->items; t2.cand_count = out->count; t2.cand_capacity = out->capacity;
+            // batch bounded by the workspaces of the main tree (same buffers, used one after the other)
+            const size_t per_h = (size_t)p->npix * l2.cpad * 2, per_cs = (size_t)std::max(1, l2.n_cells) * 2,
+                         per_ss = (size_t)3 * std::max(1, l2.n_parts);
+            int64_t b2 = std::min<int64_t>({4096, (int64_t)(p->ws.ht_elems / per_h), (int64_t)(p->ws.cs_elems / per_cs),
+                                            (int64_t)(p->ws.ss_elems / per_ss)});
+            int dev = 0, sms = 148;
+            cudaGetDevice(&dev);
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+            if (b2 > sms) b2 -= b2 % sms;
+            b2 &= ~(int64_t)1;
+            if (b2 < 2) { set_error("internal: tree workspace too small for the TB = 2 pass"); return RF_ERR_STATE; }
+            for (int64_t base = 0; base < nb2; base += b2) {
+                t2.blocks = p->d.blocks2 + p->aux_first[k] + base;
+                t2.n_blk = (int)std::min<int64_t>(b2, nb2 - base);
+                if ((rc = launch_tree_batch(p, t2, st, 2)) != RF_OK) return rc;
+                p->last_launches += 3;
+            }
+        }
+    }
+    // ---- every other width: one gridding + transform per image
+    SearchParams sp = base_params(p, vis);
+    if (p->tree_tb > 0 && p->n_blocks > 0) {
+        sp.visI = p->ws.visI;     // transposed above for the tree path
+        if (p->ws.n_gen_slots > 0 && p->n_gen_images > 0) {      // sliding sums formed above
             sp.visS = p->ws.visS;
             sp.gen_slot = p->ws.gen_slot;
             sp.visS_stride = (long long)p->ws.visI_elems;

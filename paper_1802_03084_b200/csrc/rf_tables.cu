@@ -272,6 +272,7 @@ int build_grid_lists(rf_plan* p) {
     };
     int rc = emit(p->d.gen, cols_per_group(N));
     if (rc == RF_OK && p->tree_tb > 0) rc = emit_tree(p->d.tree, tree_cols_per_group(N, p->tree_tb), 16 / p->tree_tb);   // 2 TB lanes per entry
+    if (rc == RF_OK && p->tree_tb > 0) rc = emit_tree(p->d.tree2, tree_cols_per_group(N, 2), 16 / 2);
     if (rc == RF_OK) RF_CUDA_CHECK(cudaStreamSynchronize(p->tab_stream));
     return rc;
 }
@@ -348,10 +349,48 @@ int build_image_list(rf_plan* p) {
     // the DM trials of the group inside.  Concurrent CTAs of one column group (blockIdx.x = image) then read
     // the same (baseline, channel) rows at times a few integrations apart: the 32-byte sectors of the
     // gather are shared in L2 instead of being fetched from HBM once per image at random addresses.
+    // Widths off the tree, when the plan has the time-fastest Stokes-I array: their sliding-sum array (B7) is
+    // searched by the TREE kernels as blocks of TB = 2 consecutive output integrations (gather stride dt, only the
+    // level-0 images are valid), bounded by the memory of the sliding-sum arrays; the rest takes the per-image path.
+    p->aux_width.assign(p->ndt, 0);
+    p->aux_first.assign(p->ndt + 1, 0);
+    std::vector<BlockDesc> blocks2;
+    if (p->tree_tb > 0) {
+        const size_t per_slot = ((size_t)p->nbl * p->nchan + 1) * p->tpitch * sizeof(float2);
+        size_t n_slots = 0;
+        for (int k = 0; k < p->ndt; k++) {
+            bool in_tree = false;
+            for (int l = 0; l < 4; l++) in_tree |= (p->tree_dt_idx[l] == k);
+            if (in_tree || p->dts[k] <= 1 || p->dts[k] >= p->nint || (n_slots + 1) * per_slot > kSlidingSumBudget) continue;
+            if (getenv("RF_NO_AUX")) continue;
+            n_slots++;
+            p->aux_width[k] = 1;
+        }
+    }
+    for (int k = 0; k < p->ndt; k++) {
+        p->aux_first[k] = (int64_t)blocks2.size();
+        if (!p->aux_width[k]) continue;
+        for (int g0 = 0; g0 < p->ndm; g0 += dm_group) {
+            const int g1 = std::min(p->ndm, g0 + dm_group);
+            int max_blk = 0;
+            std::vector<int> nblk(g1 - g0, 0);
+            for (int i = g0; i < g1; i++) {
+                const int nj = p->h_num_t[(size_t)order[i] * p->ndt + k];
+                nblk[i - g0] = nj > 0 ? (((nj + 1) / 2) + 1) & ~1 : 0;          // blocks of 2 images, even count (pairs)
+                max_blk = std::max(max_blk, nblk[i - g0]);
+            }
+            for (int tb = 0; tb < max_blk; tb += 2)
+                for (int i = g0; i < g1; i++)
+                    if (tb < nblk[i - g0])
+                        for (int h = 0; h < 2; h++)      // nsearch field = number of valid images of this (dm, width)
+                            blocks2.push_back({order[i], tb + h, p->h_num_t[(size_t)order[i] * p->ndt + k], 0});
+        }
+    }
+    p->aux_first[p->ndt] = (int64_t)blocks2.size();
     for (int k = 0; k < p->ndt; k++) {
         bool in_tree = false;
         for (int l = 0; l < 4; l++) in_tree |= (p->tree_dt_idx[l] == k);
-        if (in_tree) continue;
+        if (in_tree || p->aux_width[k]) continue;
         const int dt = p->dts[k];
         for (int g0 = 0; g0 < p->ndm; g0 += dm_group) {
             const int g1 = std::min(p->ndm, g0 + dm_group);
@@ -411,6 +450,7 @@ int build_image_list(rf_plan* p) {
     p->n_blocks = (int64_t)blocks.size();
     int rc = upload(p, &p->d.images, imgs.data(), imgs.size());
     if (rc == RF_OK) rc = upload(p, &p->d.blocks, blocks.data(), blocks.size());
+    if (rc == RF_OK) rc = upload(p, &p->d.blocks2, blocks2.data(), blocks2.size());
     if (rc == RF_OK) RF_CUDA_CHECK(cudaStreamSynchronize(p->tab_stream));
     return rc;
 }

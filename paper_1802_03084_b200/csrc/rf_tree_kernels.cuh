@@ -45,6 +45,7 @@ struct TreeParams {
     int32_t dbg_img;                // -1 = off
     int32_t dbg_slot;               // block of the launch the debug outputs refer to
     int32_t tpitch, nchan, ncol, cpad, ngroups, nbins, n_blk, n_cells, n_streams, n_parts;
+    int32_t q_stride;               // integrations between the samples of a block (1; dt for widths searched on sliding sums)
     int32_t zero_row;               // >= 0: periodicity mode, every block uses this (all-zero) delay row
     long long slab_stride;          // periodicity mode: visI is [slab][nbl*nchan][tpitch], block.pad = slab
     int32_t dt_idx[4];              // tree level -> index in dt_list, or -1
@@ -155,7 +156,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_tree_gather(const TreeParams p)
 #pragma unroll
     for (int l = 0; l < LEVELS; l++) ps[l] = 0.f;
     // the sample of entry (x, y) is vbase[x + delay[channel(y)]]: one 32-bit add, one 64-bit scaled add
-    const float2* vbase = p.visI + (size_t)blk.pad * p.slab_stride + blk.tb * TB + h * TB + q;
+    const float2* vbase = p.visI + (size_t)blk.pad * p.slab_stride + (size_t)(blk.tb * TB + h * TB + q) * p.q_stride;
     asm volatile("" : "+l"(vbase));     // one register pointer: a sample's address is then a single 32 x 8 + 64-bit multiply-add
     float2* cs = p.cellsum + (size_t)(slot + h) * p.n_cells * TB + q;
     float2 acc = make_float2(0.f, 0.f);
