@@ -36,7 +36,7 @@ void free_tables(rf_plan* p) {
     rf::DeviceTables& d = p->d;
     cudaFree(d.delay); cudaFree(d.cell); cudaFree(d.keep); cudaFree(d.gen.entries); cudaFree(d.gen.warp_chunk);
     cudaFree(d.tree.entries); cudaFree(d.tree.cells); cudaFree(d.tree.stream_iter); cudaFree(d.tree.stream_cell); cudaFree(d.tree.group_cell); cudaFree(d.blocks); cudaFree(d.blocks2);
-    cudaFree(d.tree2.entries); cudaFree(d.tree2.cells); cudaFree(d.tree2.stream_iter); cudaFree(d.tree2.stream_cell); cudaFree(d.tree2.group_cell); cudaFree(d.images); cudaFree(d.freqs); cudaFree(d.uvw); cudaFree(d.dms); cudaFree(d.weights); cudaFree(d.twiddles);
+    for (uint2* e : d.aux_entries) cudaFree(e); cudaFree(d.images); cudaFree(d.freqs); cudaFree(d.uvw); cudaFree(d.dms); cudaFree(d.weights); cudaFree(d.twiddles);
     p->dev_cap.clear();
     d = rf::DeviceTables{};
 }

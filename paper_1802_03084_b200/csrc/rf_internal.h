@@ -90,7 +90,8 @@ struct DeviceTables {
     // gridding lists: generic path (colgrp = cols_per_group) and boxcar-tree path
     GridLists gen;
     TreeLists tree;
-    TreeLists tree2;                 // TB = 2 lists for the widths off the tree (pairs of pre-summed images)
+    std::vector<uint2*> aux_entries; // [ndt] gather entries of a width off the tree: tree.entries with the row pitch of its
+                                     // phase-decimated sum array (null = width not searched that way); sized once
     BlockDesc* blocks2 = nullptr;    // their blocks, all such widths one after the other (rf_plan::aux_first)
     ImgDesc* images = nullptr;       // [n_gen_images] images searched by the generic path
     BlockDesc* blocks = nullptr;     // [n_blocks] blocks searched by the tree path
@@ -121,11 +122,9 @@ struct Workspace {
     BlockDesc* dbg_block = nullptr;
     int blk_batch = 0;
     size_t visI_elems = 0, ht_elems = 0, cs_elems = 0, ss_elems = 0;
-    float2* visS = nullptr;          // [n_gen_slots][nbl*nchan][tpitch] sliding sums for widths off the tree
-    int32_t* gen_slot = nullptr;     // device [ndt]: slot in visS or -1
-    std::vector<int32_t> h_gen_slot; // host copy
+    float2* visS = nullptr;          // phase-decimated boxcar sums of the widths off the tree (B7), one array per width
+    std::vector<size_t> aux_off;     // [ndt + 1] first element of each width's array in visS
     size_t visS_elems = 0;
-    int n_gen_slots = 0;
     // periodicity search
     float2* slab = nullptr;          // [n_slabs][nbl*nchan][slab_pitch] time spectra as (S, -i S) pairs
     size_t slab_elems = 0;
@@ -159,7 +158,8 @@ struct rf_plan {
     std::vector<uint8_t> h_keep;
     std::vector<int32_t> h_maxdelay;           // [ndm]
     std::vector<int32_t> h_num_t;              // [ndm][ndt]
-    std::vector<int32_t> aux_width;            // [ndt] 1 = width off the tree searched as TB = 2 blocks of sliding sums
+    std::vector<int32_t> aux_width;            // [ndt] 1 = width off the tree searched by the tree kernels on its phase-decimated sums
+    std::vector<int32_t> aux_pitch;            // [ndt] row pitch of that array (output integrations per series and phase)
     std::vector<int64_t> aux_first;            // [ndt + 1] first block of each width in d.blocks2
     std::vector<int32_t> h_block_deadline;     // [n_blocks] integrations [0, deadline) are all a tree block (and those before it) read
     // derived
@@ -198,6 +198,7 @@ namespace rf {
 int build_delay_table(rf_plan* p);            // device kernel (float64) -> d.delay, h_delay
 int build_cell_table(rf_plan* p);             // device kernel (float64) -> d.cell/keep, host copies
 int build_grid_lists(rf_plan* p);             // host binning of the cell table -> d.gen, d.tree
+int aux_pitch_of(const rf_plan* p, int dt);   // row pitch of the phase-decimated sum array of a width
 int build_image_list(rf_plan* p);             // (dm, dt, j) loop -> d.images (generic) + d.blocks (tree)
 int tree_cols_per_group(int npix, int tb);
 void configure_tree(rf_plan* p);              // which dt values ride the boxcar tree    // columns per pass-1 CTA of the tree path

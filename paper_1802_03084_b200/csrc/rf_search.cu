@@ -228,7 +228,8 @@ TreeParams tree_params(rf_plan* p) {
     tp.dbg_img = -1;
     tp.dbg_slot = 0;
     tp.zero_row = -1;
-    tp.q_stride = 1;
+    tp.dec = 1;
+    tp.phase_stride = 0;
     tp.slab_stride = 0;
     tp.tpitch = p->tpitch;
     tp.nchan = p->nchan;
@@ -296,33 +297,16 @@ int ensure_tree_workspace(rf_plan* p) {
         w.ss_elems = ss_elems + ss_elems / 8;
     }
     if (!w.dbg_block) RF_CUDA_CHECK(cudaMalloc((void**)&w.dbg_block, 2 * sizeof(BlockDesc)));
-    // sliding-sum arrays: one per width > 1 that is searched by the per-image path (bounded memory)
-    std::vector<int32_t> slot(p->ndt, -1);
-    int n_slots = 0;
-    const size_t budget = kSlidingSumBudget;
-    for (int k = 0; k < p->ndt; k++) {
-        bool in_tree = false;
-        for (int l = 0; l < 4; l++) in_tree |= (p->tree_dt_idx[l] == k);
-        if (in_tree || p->dts[k] <= 1 || p->dts[k] >= p->nint) continue;
-        if ((size_t)(n_slots + 1) * visI_elems * sizeof(float2) > budget) break;
-        slot[k] = n_slots++;
-    }
-    if (slot != w.h_gen_slot || !w.gen_slot) {
-        cudaFree(w.gen_slot); w.gen_slot = nullptr;
-        RF_CUDA_CHECK(cudaMalloc((void**)&w.gen_slot, (size_t)p->ndt * sizeof(int32_t)));
-        RF_CUDA_CHECK(cudaMemcpy(w.gen_slot, slot.data(), (size_t)p->ndt * sizeof(int32_t), cudaMemcpyHostToDevice));
-        w.h_gen_slot = slot;
-    }
-    w.n_gen_slots = n_slots;
-    // tail: the padding block pairs of the TB = 2 pass read up to 2 dt integrations past the end of a series
-    // (into the next one; past the last one here) -- their images are invalid but must be finite (pair transform)
-    size_t tail = 64;
-    for (int k = 0; k < p->ndt; k++) if (slot[k] >= 0) tail = std::max(tail, (size_t)4 * p->dts[k] + 64);
-    if (n_slots > 0 && (!w.visS || w.visS_elems < (size_t)n_slots * visI_elems + tail)) {
+    // phase-decimated sum arrays of the widths off the tree (configure_tree decided which): one after the other
+    w.aux_off.assign(p->ndt + 1, 0);
+    for (int k = 0; k < p->ndt; k++)
+        w.aux_off[k + 1] = w.aux_off[k] + (p->aux_width[k] ? (size_t)p->dts[k] * ((size_t)p->nbl * p->nchan + 1) * p->aux_pitch[k] : 0);
+    const size_t need = w.aux_off[p->ndt];
+    if (need > 0 && (!w.visS || w.visS_elems < need)) {
         cudaFree(w.visS); w.visS = nullptr;
-        RF_CUDA_CHECK(cudaMalloc((void**)&w.visS, ((size_t)n_slots * visI_elems + tail) * sizeof(float2)));
-        RF_CUDA_CHECK(cudaMemset(w.visS, 0, ((size_t)n_slots * visI_elems + tail) * sizeof(float2)));
-        w.visS_elems = (size_t)n_slots * visI_elems + tail;
+        RF_CUDA_CHECK(cudaMalloc((void**)&w.visS, need * sizeof(float2)));
+        RF_CUDA_CHECK(cudaMemset(w.visS, 0, need * sizeof(float2)));      // incl. the all-zero series of every phase
+        w.visS_elems = need;
     }
     return RF_OK;
 }
@@ -364,7 +348,7 @@ void free_workspace(rf_plan* p) {
     cudaFree(w.ticket); cudaFree(w.counters); cudaFree(w.dbg_desc);
     cudaFree(w.visI); cudaFree(w.Ht); cudaFree(w.sumsq_t); cudaFree(w.cellsum); cudaFree(w.dbg_block);
     cudaFree(w.mean_partial); cudaFree(w.mean_p); cudaFree(w.mean_i);
-    cudaFree(w.visS); cudaFree(w.gen_slot);
+    cudaFree(w.visS);
     cudaFree(w.slab); cudaFree(w.pblocks); cudaFree(w.zero_delay); cudaFree(w.time_tw);
     w = Workspace{};
 }
@@ -476,51 +460,39 @@ int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out
             base += n;
         }
         if ((rc = need_rows(p->tpitch)) != RF_OK) return rc;      // widths off the tree read the whole array
-        // ---- widths off the tree: sliding sums once per segment (B7) ...
-        if (p->ws.n_gen_slots > 0) {
-            if ((rc = mark(p, st, -1)) != RF_OK) return rc;
-            for (int k = 0; k < p->ndt; k++) {
-                const int sl = p->ws.h_gen_slot[k];
-                if (sl < 0) continue;
-                k_sliding_sum<<<dim3(p->nbl * p->nchan, (p->tpitch + 255) / 256), 256, 0, st>>>(
-                    p->ws.visI, p->ws.visS + (size_t)sl * p->ws.visI_elems, p->dts[k], p->tpitch);
-                RF_CUDA_CHECK(cudaGetLastError());
-                p->last_launches += 1;
-            }
-            if ((rc = mark(p, st, 2)) != RF_OK) return rc;
-        }
-        // ---- ... searched by the tree kernels as blocks of two consecutive output integrations (stride dt)
+        // ---- widths off the tree (B7): phase-decimated boxcar sums once per segment, then the same three kernels
+        //      on blocks of TB consecutive OUTPUT integrations (level 0 of the tree = the width itself)
         for (int k = 0; k < p->ndt; k++) {
-            const int sl = p->ws.h_gen_slot[k];
             const int64_t nb2 = p->aux_first[k + 1] - p->aux_first[k];
-            if (!p->aux_width[k] || sl < 0 || nb2 == 0) continue;
-            TreeParams t2 = tree_params(p);
-            const TreeLists& l2 = p->d.tree2;
-            t2.entries = l2.entries; t2.stream_iter = l2.stream_iter; t2.stream_cell = l2.stream_cell;
-            t2.cells = l2.cells; t2.group_cell = l2.group_cell;
-            t2.n_cells = l2.n_cells; t2.n_streams = l2.n_streams; t2.n_parts = l2.n_parts;
-            t2.cpad = l2.cpad; t2.ngroups = l2.ngroups;
-            t2.visI = p->ws.visS + (size_t)sl * p->ws.visI_elems;
-            t2.q_stride = p->dts[k];
+            if (!p->aux_width[k] || nb2 == 0) continue;
+            const int dt = p->dts[k], pitch = p->aux_pitch[k], nelem = p->nbl * p->nchan;
+            float2* arr = p->ws.visS + p->ws.aux_off[k];
+            if ((rc = mark(p, st, -1)) != RF_OK) return rc;
+            const int JC = std::max(8, 2048 / dt);
+            const size_t psm = ((size_t)JC * dt + dt + (size_t)JC * dt + JC * dt / 32 + 2) * sizeof(float2);
+            if (psm > 48 * 1024) {    // very wide boxcars: beyond the default dynamic shared-memory window
+                static size_t configured = 0;
+                if (psm > configured) {
+                    RF_CUDA_CHECK(cudaFuncSetAttribute(k_phase_sum, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)psm));
+                    configured = psm;
+                }
+            }
+            k_phase_sum<<<dim3(nelem, (pitch + JC - 1) / JC), 256, psm, st>>>(p->ws.visI, arr, dt, p->tpitch, pitch, nelem, JC);
+            RF_CUDA_CHECK(cudaGetLastError());
+            if ((rc = mark(p, st, 2)) != RF_OK) return rc;
+            p->last_launches += 1;
+            TreeParams t2 = tp;
+            t2.entries = p->d.aux_entries[k];
+            t2.visI = arr;
+            t2.dec = dt;
+            t2.phase_stride = (uint32_t)((size_t)(nelem + 1) * pitch);
             t2.dt_idx[0] = k;
             for (int l = 1; l < 4; l++) t2.dt_idx[l] = -1;
-            t2.norm = tp.norm / (float)p->dts[k];
-            t2.cand_items = out->items; t2.cand_count = out->count; t2.cand_capacity = out->capacity;
-            // batch bounded by the workspaces of the main tree (same buffers, used one after the other)
-            const size_t per_h = (size_t)p->npix * l2.cpad * 2, per_cs = (size_t)std::max(1, l2.n_cells) * 2,
-                         per_ss = (size_t)3 * std::max(1, l2.n_parts);
-            int64_t b2 = std::min<int64_t>({4096, (int64_t)(p->ws.ht_elems / per_h), (int64_t)(p->ws.cs_elems / per_cs),
-                                            (int64_t)(p->ws.ss_elems / per_ss)});
-            int dev = 0, sms = 148;
-            cudaGetDevice(&dev);
-            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-            if (b2 > sms) b2 -= b2 % sms;
-            b2 &= ~(int64_t)1;
-            if (b2 < 2) { set_error("internal: tree workspace too small for the TB = 2 pass"); return RF_ERR_STATE; }
-            for (int64_t base = 0; base < nb2; base += b2) {
+            t2.norm = tp.norm / (float)dt;
+            for (int64_t base = 0; base < nb2; base += p->ws.blk_batch) {
                 t2.blocks = p->d.blocks2 + p->aux_first[k] + base;
-                t2.n_blk = (int)std::min<int64_t>(b2, nb2 - base);
-                if ((rc = launch_tree_batch(p, t2, st, 2)) != RF_OK) return rc;
+                t2.n_blk = (int)std::min<int64_t>(p->ws.blk_batch, nb2 - base);
+                if ((rc = launch_tree_batch(p, t2, st)) != RF_OK) return rc;
                 p->last_launches += 3;
             }
         }
@@ -529,11 +501,6 @@ int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out
     SearchParams sp = base_params(p, vis);
     if (p->tree_tb > 0 && p->n_blocks > 0) {
         sp.visI = p->ws.visI;     // transposed above for the tree path
-        if (p->ws.n_gen_slots > 0 && p->n_gen_images > 0) {      // sliding sums formed above
-            sp.visS = p->ws.visS;
-            sp.gen_slot = p->ws.gen_slot;
-            sp.visS_stride = (long long)p->ws.visI_elems;
-        }
     }
     sp.cand_items = out->items;
     sp.cand_count = out->count;

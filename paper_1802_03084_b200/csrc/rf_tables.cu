@@ -264,6 +264,14 @@ int build_grid_lists(rf_plan* p) {
         tl.n_streams = (int)stream_iter.size() - 1;
         tl.n_parts = (tl.n_streams + kWarpsPerCta - 1) / kWarpsPerCta;
         int rc;
+        // widths searched on phase-decimated sums: the same entries with that array's row pitch
+        if ((int)p->d.aux_entries.size() != p->ndt) p->d.aux_entries.assign(p->ndt, nullptr);
+        for (int k = 0; k < p->ndt; k++) {
+            if (!p->aux_width[k]) continue;
+            std::vector<uint2> e2(entries);
+            for (uint2& e : e2) e.x = (e.x / (uint32_t)p->tpitch) * (uint32_t)p->aux_pitch[k];
+            if ((rc = upload(p, &p->d.aux_entries[k], e2.data(), e2.size())) != RF_OK) return rc;
+        }
         if ((rc = upload(p, &tl.entries, entries.data(), entries.size())) != RF_OK) return rc;
         if ((rc = upload(p, &tl.cells, cells.data(), cells.size())) != RF_OK) return rc;
         if ((rc = upload(p, &tl.stream_iter, stream_iter.data(), stream_iter.size())) != RF_OK) return rc;
@@ -272,7 +280,6 @@ int build_grid_lists(rf_plan* p) {
     };
     int rc = emit(p->d.gen, cols_per_group(N));
     if (rc == RF_OK && p->tree_tb > 0) rc = emit_tree(p->d.tree, tree_cols_per_group(N, p->tree_tb), 16 / p->tree_tb);   // 2 TB lanes per entry
-    if (rc == RF_OK && p->tree_tb > 0) rc = emit_tree(p->d.tree2, tree_cols_per_group(N, 2), 16 / 2);
     if (rc == RF_OK) RF_CUDA_CHECK(cudaStreamSynchronize(p->tab_stream));
     return rc;
 }
@@ -283,6 +290,30 @@ int tree_cols_per_group(int npix, int tb) {
     if (npix <= 512) return (16 * 512) / (npix * tb);     // TB x NCOL = 16 tiles of 512 (32 of 256): 70 KB
     if (npix == 1024) return tb == 2 ? 4 : 2;             // 8 tiles of 1024; TB > 4 is split over blockIdx.z
     return 2;                                             // 4 tiles of 2048 (70 KB) / 4096 (139 KB)
+}
+
+// Row pitch of the phase-decimated sum array of width dt: output integrations j' = t / dt of one series and phase,
+// plus the read-ahead of the last block pair and of the largest delay.
+int aux_pitch_of(const rf_plan* p, int dt) { return (((p->tpitch + dt - 1) / dt + 2 * p->tree_tb + 8) + 7) & ~7; }
+
+// Which widths off the tree are searched by the tree kernels on phase-decimated sums (B7): every width > 1 while the
+// sum arrays fit kSlidingSumBudget (each is about the size of the Stokes-I array); the rest takes the per-image path.
+static void decide_aux_widths(rf_plan* p) {
+    p->aux_width.assign(p->ndt, 0);
+    p->aux_pitch.assign(p->ndt, 0);
+    if (p->tree_tb == 0 || getenv("RF_NO_AUX")) return;
+    size_t bytes = 0;
+    for (int k = 0; k < p->ndt; k++) {
+        bool in_tree = false;
+        for (int l = 0; l < 4; l++) in_tree |= (p->tree_dt_idx[l] == k);
+        const int dt = p->dts[k];
+        if (in_tree || dt <= 1 || dt >= p->nint) continue;
+        const size_t need = (size_t)dt * ((size_t)p->nbl * p->nchan + 1) * aux_pitch_of(p, dt) * sizeof(float2);
+        if (bytes + need > kSlidingSumBudget || need / sizeof(float2) >= (1ull << 32)) continue;
+        bytes += need;
+        p->aux_width[k] = 1;
+        p->aux_pitch[k] = aux_pitch_of(p, dt);
+    }
 }
 
 // Loop + segment semantics (readings A6, A16): all j with
@@ -314,6 +345,7 @@ void configure_tree(rf_plan* p) {
         p->tree_tb = 0; p->tpitch = 0;
         for (int l = 0; l < 4; l++) p->tree_dt_idx[l] = -1;
     }
+    decide_aux_widths(p);
 }
 
 int build_image_list(rf_plan* p) {
@@ -349,24 +381,10 @@ int build_image_list(rf_plan* p) {
     // the DM trials of the group inside.  Concurrent CTAs of one column group (blockIdx.x = image) then read
     // the same (baseline, channel) rows at times a few integrations apart: the 32-byte sectors of the
     // gather are shared in L2 instead of being fetched from HBM once per image at random addresses.
-    // Widths off the tree, when the plan has the time-fastest Stokes-I array: their sliding-sum array (B7) is
-    // searched by the TREE kernels as blocks of TB = 2 consecutive output integrations (gather stride dt, only the
-    // level-0 images are valid), bounded by the memory of the sliding-sum arrays; the rest takes the per-image path.
-    p->aux_width.assign(p->ndt, 0);
+    // Widths off the tree that configure_tree marked (aux_width): blocks of TB consecutive OUTPUT integrations of one
+    // DM, searched by the tree kernels on the phase-decimated sum array of the width (B7); only level 0 is valid.
     p->aux_first.assign(p->ndt + 1, 0);
     std::vector<BlockDesc> blocks2;
-    if (p->tree_tb > 0) {
-        const size_t per_slot = ((size_t)p->nbl * p->nchan + 1) * p->tpitch * sizeof(float2);
-        size_t n_slots = 0;
-        for (int k = 0; k < p->ndt; k++) {
-            bool in_tree = false;
-            for (int l = 0; l < 4; l++) in_tree |= (p->tree_dt_idx[l] == k);
-            if (in_tree || p->dts[k] <= 1 || p->dts[k] >= p->nint || (n_slots + 1) * per_slot > kSlidingSumBudget) continue;
-            if (getenv("RF_NO_AUX")) continue;
-            n_slots++;
-            p->aux_width[k] = 1;
-        }
-    }
     for (int k = 0; k < p->ndt; k++) {
         p->aux_first[k] = (int64_t)blocks2.size();
         if (!p->aux_width[k]) continue;
@@ -374,9 +392,10 @@ int build_image_list(rf_plan* p) {
             const int g1 = std::min(p->ndm, g0 + dm_group);
             int max_blk = 0;
             std::vector<int> nblk(g1 - g0, 0);
+            const int TB = p->tree_tb;
             for (int i = g0; i < g1; i++) {
                 const int nj = p->h_num_t[(size_t)order[i] * p->ndt + k];
-                nblk[i - g0] = nj > 0 ? (((nj + 1) / 2) + 1) & ~1 : 0;          // blocks of 2 images, even count (pairs)
+                nblk[i - g0] = nj > 0 ? (((nj + TB - 1) / TB) + 1) & ~1 : 0;    // blocks of TB images, even count (pairs)
                 max_blk = std::max(max_blk, nblk[i - g0]);
             }
             for (int tb = 0; tb < max_blk; tb += 2)

@@ -45,7 +45,8 @@ struct TreeParams {
     int32_t dbg_img;                // -1 = off
     int32_t dbg_slot;               // block of the launch the debug outputs refer to
     int32_t tpitch, nchan, ncol, cpad, ngroups, nbins, n_blk, n_cells, n_streams, n_parts;
-    int32_t q_stride;               // integrations between the samples of a block (1; dt for widths searched on sliding sums)
+    int32_t dec;                    // 1, or the width dt whose phase-decimated sum array visI points at (B7)
+    uint32_t phase_stride;          // dec > 1: elements per phase = (nbl*nchan + 1) * row pitch
     int32_t zero_row;               // >= 0: periodicity mode, every block uses this (all-zero) delay row
     long long slab_stride;          // periodicity mode: visI is [slab][nbl*nchan][tpitch], block.pad = slab
     int32_t dt_idx[4];              // tree level -> index in dt_list, or -1
@@ -94,19 +95,36 @@ __global__ void k_stokes_transpose(const float* __restrict__ vis, float2* __rest
     }
 }
 
-// Sliding sums over dt integrations of the time-fastest Stokes-I array, out[e][t] = sum_{q<dt} visI[e][t+q]
-// (terms past the pitch dropped: those t are never searched).  A width that is not on the boxcar tree then
-// costs the per-image gather ONE 8-byte read per (baseline, channel) instead of dt (row 8a-2; the sum is the
-// same boxcar, formed once per segment instead of once per DM trial).  grid (nelem, ceil(tpitch/256)).
-__global__ void __launch_bounds__(256) k_sliding_sum(const float2* __restrict__ visI, float2* __restrict__ out,
-                                                     int dt, int tpitch) {
-    const int t = blockIdx.y * 256 + threadIdx.x;
-    if (t >= tpitch) return;
-    const float2* src = visI + (size_t)blockIdx.x * tpitch;
-    float re = 0.f, im = 0.f;
-    const int n = min(dt, tpitch - t);
-    for (int q = 0; q < n; q++) { const float2 a = __ldg(src + t + q); re += a.x; im += a.y; }
-    out[(size_t)blockIdx.x * tpitch + t] = make_float2(re, im);
+// Phase-decimated boxcar sums of the time-fastest Stokes-I array for a width dt that is not on the tree (B7):
+//   out[(phase * (nelem + 1) + e) * pitch + jp] = sum_{q < dt} visI[e][phase + dt * jp + q]     (0 past the array),
+// i.e. the dt-sample boxcar starting at every integration t = phase + dt * jp, stored so that the boxcars one width
+// apart are adjacent.  The dedispersed output integration j of a channel with delay d is the boxcar at t = d + dt j
+// = element (phase d % dt, jp = j + d / dt): consecutive j are contiguous, so the tree gather reads them like native
+// integrations.  grid (nelem, ceil(pitch / JC)), block 256; one CTA = one series x JC output integrations of every
+// phase = a span of JC * dt native integrations staged in shared memory (coalesced read), boxcars formed from
+// shared memory, written phase by phase in runs of JC contiguous values.  Dynamic smem: in [JC*dt + dt] | sums
+// [JC*dt, padded by 1/32] float2.  The all-zero series of every phase is never written.
+__global__ void __launch_bounds__(256) k_phase_sum(const float2* __restrict__ visI, float2* __restrict__ out,
+                                                   int dt, int tpitch, int pitch, int nelem, int JC) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int span = JC * dt;
+    float2* in = reinterpret_cast<float2*>(smem_raw);
+    float2* sums = in + span + dt;
+    const int e = blockIdx.x, j0 = blockIdx.y * JC, t0 = j0 * dt, tid = threadIdx.x;
+    const float2* src = visI + (size_t)e * tpitch;
+    for (int i = tid; i < span + dt; i += 256) in[i] = (t0 + i < tpitch) ? __ldg(src + t0 + i) : make_float2(0.f, 0.f);
+    __syncthreads();
+    for (int i = tid; i < span; i += 256) {
+        float re = 0.f, im = 0.f;
+        for (int q = 0; q < dt; q++) { re += in[i + q].x; im += in[i + q].y; }
+        sums[i + (i >> 5)] = make_float2(re, im);
+    }
+    __syncthreads();
+    for (int idx = tid; idx < span; idx += 256) {
+        const int phase = idx / JC, i = idx % JC, jp = j0 + i;
+        const int k = phase + dt * i;
+        if (jp < pitch) out[((size_t)phase * (nelem + 1) + e) * pitch + jp] = sums[k + (k >> 5)];
+    }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -149,14 +167,20 @@ __global__ void __launch_bounds__(kThreads, 4) k_tree_gather(const TreeParams p)
 #pragma unroll
         for (int u = 0; u < U; u++) en[u] = p.entries[(size_t)(it_beg + u) * LG + j];
     }
-    for (int i = tid; i < p.nchan; i += kThreads) sdelay[i] = drow[i];
+    // dec > 1: integration t = delay + dt j of a series lives at (phase t % dt, output integration t / dt), so the
+    // "delay" added to an entry's row offset is (delay % dt) * phase_stride + delay / dt and the block's TB (2 TB)
+    // consecutive OUTPUT integrations are contiguous
+    for (int i = tid; i < p.nchan; i += kThreads) {
+        const int d = drow[i];
+        sdelay[i] = p.dec > 1 ? (int)((uint32_t)(d % p.dec) * p.phase_stride + (uint32_t)(d / p.dec)) : d;
+    }
     __syncthreads();
 
     float ps[LEVELS];
 #pragma unroll
     for (int l = 0; l < LEVELS; l++) ps[l] = 0.f;
     // the sample of entry (x, y) is vbase[x + delay[channel(y)]]: one 32-bit add, one 64-bit scaled add
-    const float2* vbase = p.visI + (size_t)blk.pad * p.slab_stride + (size_t)(blk.tb * TB + h * TB + q) * p.q_stride;
+    const float2* vbase = p.visI + (size_t)blk.pad * p.slab_stride + blk.tb * TB + h * TB + q;
     asm volatile("" : "+l"(vbase));     // one register pointer: a sample's address is then a single 32 x 8 + 64-bit multiply-add
     float2* cs = p.cellsum + (size_t)(slot + h) * p.n_cells * TB + q;
     float2 acc = make_float2(0.f, 0.f);
