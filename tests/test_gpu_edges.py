@@ -67,6 +67,32 @@ def test_small_sizes_every_image(npix, npol, dts):
     plan.destroy()
 
 
+def test_offtree_widths_per_image_fallback(monkeypatch):
+    """Widths off the tree whose boxcar-sum arrays do not fit the workspace budget take the per-image path
+    (B7).  RF_NO_AUX (read when the plan is created) forces that decision on a small plan; the
+    candidate list must be the oracle's either way, and identical keys to the plan that uses the sum arrays."""
+    import torch
+    import paper_1802_03084_b200 as R
+    cfg = W.get_config("tiny")
+    f, uvw = W.channel_freqs_hz(cfg), W.baseline_uvw_m(cfg)
+    npix, npol, nint, dts = 256, 2, 43, (1, 3, 6)
+    cell = W.default_cell_rad(cfg, uvw) * 64 / npix * 0.8
+    dms = np.array([0.0, 25.0, 60.0])
+    vis = _rand_vis((nint, cfg.nbl, cfg.nchan, npol), 777)
+    vis = O.inject_transient(vis, f, uvw, cfg.inttime_s, cell, 1.0, 5, -9, 60.0, 3, 12).astype(np.complex64)
+    d = torch.from_numpy(vis).cuda()
+    plan_aux = R.Plan(f, uvw, npol, nint, cfg.inttime_s, npix, cell, dms, dts, 0.0)
+    g_aux = _compare_all(plan_aux, d, vis, f, uvw, cell, npix, dms, dts, 0.0, cfg.inttime_s, min_match=20)
+    plan_aux.destroy()
+    monkeypatch.setenv("RF_NO_AUX", "1")
+    plan = R.Plan(f, uvw, npol, nint, cfg.inttime_s, npix, cell, dms, dts, 0.0)
+    g = _compare_all(plan, d, vis, f, uvw, cell, npix, dms, dts, 0.0, cfg.inttime_s, min_match=20)
+    plan.destroy()
+    assert set(g) == set(g_aux) and len(g) == len(g_aux)
+    for key in g:
+        assert abs(float(g[key]["snr"]) - float(g_aux[key]["snr"])) <= SNR_TOL * float(g[key]["snr"]), key
+
+
 def test_degenerate_plans():
     """Nothing kept (all channels flagged): zero candidates, zero image, no crash.  A DM whose sweep is
     longer than the segment contributes no images.  Unsorted channel order gives the same tables as the oracle."""
