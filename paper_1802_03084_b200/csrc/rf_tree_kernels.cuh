@@ -374,16 +374,22 @@ __device__ __forceinline__ void tree_row_stats(const float (&x)[16], int img, in
     uint32_t hw = (uint32_t)__cvta_generic_to_shared(cx.hist) + (uint32_t)((cx.wide ? img : (img >> 1)) * cx.nbins) * 4u;
     asm volatile("" : "+r"(hw));          // keep the sum in a register (the compiler re-forms it per pixel otherwise)
     const uint32_t inc = (!cx.wide && (img & 1)) ? 65536u : 1u;
-    const unsigned nbm1 = (unsigned)cx.nbins - 1u;
+    // bin = clamp(floor(x * A + B), 0, nbins - 1) without a float -> int conversion: one FMA rounded DOWN onto
+    // 1.5 * 2^23 (ulp 1) leaves floor(x * A + B) in the low mantissa bits; B = nbins / 2 is an integer, so the addend
+    // is exact.  As SIGNED integers the bit patterns are ordered like the values (anything below -2^22 bins, incl.
+    // negative floats, clamps to bin 0; +inf clamps to the top), so one 3-input min/max clamps both ends.
+    constexpr int kMagicBits = 0x4B400000;                  // 12582912.0f
+    const float Bm = cx.B + 12582912.0f;
+    const int top = kMagicBits + cx.nbins - 1;
+    hw -= (uint32_t)kMagicBits * 4u;                        // wraps; undone by the scaled add below
     float m = x[0];
 #pragma unroll
     for (int e = 0; e < 16; e++) {
-        // cvt.rmi.u32.f32 saturates: negative (and NaN) -> bin 0; one min clamps the top
-        const unsigned bin = __float2uint_rd(fmaf(x[e], A, cx.B));
+        const int q = min(max(__float_as_int(__fmaf_rd(x[e], A, Bm)), kMagicBits), top);
 #ifdef RF_EXP_NOHIST
-        if (bin == 12345678u)
+        if (q == 12345678)
 #endif
-        asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(hw + min(bin, nbm1) * 4u), "r"(inc) : "memory");
+        asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(hw + (uint32_t)q * 4u), "r"(inc) : "memory");
         m = fmaxf(m, x[e]);
     }
     // running peak of this warp: a new maximum is rare after the first rows, so one vote decides.
