@@ -11,7 +11,8 @@
  *         Hermitian conjugate,
  *     (d) form the image with a 2-D inverse FFT,
  *     (e) reduce it to peak, robust sigma and S/N and keep it if S/N >= threshold
- *         (PAPER.md:86-88).
+ *         (PAPER.md:86-88).  An all-zero image (sigma = 0) has S/N := 0 and is never a
+ *         candidate, whatever the threshold (reading A24).
  *
  * All device work is hand-written CUDA for sm_100a; there is no CPU fallback.
  * Every function returns RF_OK (0) or a negative error code, never throws, never
@@ -55,7 +56,9 @@ typedef struct {
 
 /* Counters of the last rf_search (read after synchronising its stream). */
 typedef struct {
-    int64_t images;           /* (dm, dt, j) images searched                              */
+    int64_t images;           /* (dm, dt, j) images whose statistics the kernels finalised: counted ON
+                                 THE DEVICE, once per image (rf_search_periodic: frequency images); equals
+                                 rf_plan_num_images() after a complete rf_search, 0 when nothing is gridded */
     int64_t vis_gridded;      /* Stokes-I samples gridded = sum_images N_w * dt           */
     int32_t n_kept;           /* N_w: (baseline, channel) samples kept by the cell table  */
     int32_t n_dropped;        /* samples outside the grid or with zero channel weight      */
@@ -86,7 +89,8 @@ int rf_plan_create(rf_plan** out,
                    float threshold_sigma);
 
 /* Enqueue the whole search of one segment on `cuda_stream` (a cudaStream_t, may be
- * 0) and return without synchronising.
+ * 0) and return without synchronising.  The device the plan was created on must be current
+ * (RF_ERR_STATE otherwise; the same holds for every entry point that launches kernels).
  *   vis_dev  DEVICE pointer, complex64 [nint][nbl][nchan][npol] (re,im float32 pairs),
  *            16-byte aligned, borrowed read-only until the stream passes this work.
  * One rf_search in flight per plan (the workspace is per plan).                  */
@@ -99,7 +103,11 @@ int rf_plan_destroy(rf_plan* plan);
 int rf_plan_set_chan_weights(rf_plan* plan, const float* w);
 
 /* Replace the baseline uvw (and optionally the cell size: cell_rad <= 0 keeps it);
- * rebuilds the cell and gridding tables (hour angle changes between segments).    */
+ * rebuilds the cell and gridding tables (hour angle changes between segments).
+ * Deviation from SURVEY.md 8(b), which proposed (plan, uvw_m, cuda_stream): the cell size follows
+ * max|uv| (reading A13) and so changes with uvw, and the rebuild sorts on the host, so it runs on the
+ * plan's own non-blocking stream and returns when the tables are on the device; no caller stream is
+ * involved.  The plan must be idle (no rf_search of it in flight).                              */
 int rf_plan_set_uvw(rf_plan* plan, const double* uvw_m, double cell_rad);
 
 /* Streaming (config 5): search only native integrations t < n_native_ints for every
@@ -130,6 +138,20 @@ int rf_plan_get_counters(rf_plan* plan, rf_counters* out);
 /* Tuning knob (not part of the result): images per batch of the two-pass pipeline;
  * 0 restores the default chosen from npix and the L2 size.                        */
 int rf_plan_set_batch(rf_plan* plan, int images_per_batch);
+
+/* Tuning knobs: none changes a result (candidate sets are identical; S/N agrees to rounding), they
+ * exist for experiments and for tests that force the rarely taken code paths.  There is NO environment-
+ * variable behaviour in the library.  Rebuilds the work lists (the plan must be idle).
+ *   RF_TUNE_AUX_WIDTHS  0: widths off the boxcar tree take the per-image path instead of the tree
+ *                          kernels on phase-decimated sums (B7); default 1
+ *   RF_TUNE_DM_GROUP    DM trials interleaved in time by the block order (L2 locality); default 8
+ *   RF_TUNE_FEED_BATCH  blocks per launch while rf_search_host's upload is in flight; 0 = one wave
+ *   RF_TUNE_TREE_MAXPIX largest npix searched by the boxcar-tree kernels; default 4096            */
+#define RF_TUNE_AUX_WIDTHS  1
+#define RF_TUNE_DM_GROUP    2
+#define RF_TUNE_FEED_BATCH  3
+#define RF_TUNE_TREE_MAXPIX 4
+int rf_plan_set_tuning(rf_plan* plan, int knob, int value);
 
 /* End-to-end convenience entry with HOST buffers: copies the segment host->device into a
  * plan-owned staging buffer, runs rf_search on the plan's own stream, copies the candidates

@@ -16,7 +16,8 @@ are DESIGN.md "Readings", taken from SURVEY.md section 8(c)).
     O9  mock-transient injection
     O10 periodicity search: Fourier transform in time, image each frequency   PAPER.md:100 (footnote 4), 104
 
-Pins (tests/test_oracle_pins.py): every function below is pinned to something
+Pins (tests/test_oracle_tables.py, test_oracle_imaging.py, test_oracle_prep.py, test_oracle_cutout.py,
+test_oracle_inject.py, test_oracle_periodic.py): every function below is pinned to something
 other than itself -- closed forms, exact rational arithmetic, a direct DFT,
 Parseval, the analytic noise variance, an injected source, brute force.  The
 one free choice the paper does not fix is the sigma ESTIMATOR (reading A9:
@@ -242,13 +243,14 @@ def inject_transient(vis: np.ndarray, freqs_hz, uvw_m, inttime_s: float, cell_ra
 LN2 = 0.6931471805599453
 
 
-def periodicity_nt(nint: int, max_delay: int) -> int:
+def periodicity_nt(nint: int, max_delay: int, max_nt: int = 4096) -> int:
     """Length of the time transform of one DM trial: the largest power of two <= nint - max_delay
-    (0 when that is below 64)."""
+    (0 when that is below 64), at most max_nt = 4096 integrations (reading A23: the search transforms
+    the first 4096 dedispersed integrations of longer segments)."""
     n = nint - max_delay
     if n < 64:
         return 0
-    return 1 << (int(n).bit_length() - 1)
+    return min(1 << (int(n).bit_length() - 1), max_nt)
 
 
 def periodicity_spectrum(vis: np.ndarray, delay_dm: np.ndarray, nt: int) -> np.ndarray:
@@ -309,7 +311,7 @@ def periodicity_search(vis: np.ndarray, freqs_hz, uvw_m, inttime_s: float, npix:
             amp, y, x, sigma, snr = periodicity_stats(img.real ** 2 + img.imag ** 2)
             if return_all_stats:
                 stats[(d, k)] = (amp, y, x, sigma, snr)
-            if snr >= threshold:
+            if sigma > 0.0 and snr >= threshold:
                 cands.append(Candidate(d, -1, k, x if x < npix // 2 else x - npix, y if y < npix // 2 else y - npix,
                                        amp, sigma, snr))
     return (cands, stats) if return_all_stats else cands
@@ -330,7 +332,9 @@ def search(vis: np.ndarray, freqs_hz, uvw_m, inttime_s: float, npix: int, cell_r
            return_all_stats: bool = False):
     """The whole loop of Fig. 2 for one segment.
 
-    Returns the list of Candidate with snr >= threshold (order: dm, dt, j).  With
+    Returns the list of Candidate with snr >= threshold (order: dm, dt, j).  An image with sigma = 0
+    (all-zero image) has snr := 0 and yields no candidate whatever the threshold (SURVEY.md 8(b):
+    "All-zero image (sigma = 0) => snr := 0, no candidate"; reading A24).  With
     ``keys`` only those (dm_idx, dt_idx, j) are evaluated (sampled parity at full
     sizes).  With ``return_all_stats`` also returns {key: (peak,y,x,sigma,snr)}.
     """
@@ -354,7 +358,7 @@ def search(vis: np.ndarray, freqs_hz, uvw_m, inttime_s: float, npix: int, cell_r
         peak, y, x, sigma, snr = image_stats(img)
         if return_all_stats:
             stats[(d, k, j)] = (peak, y, x, sigma, snr)
-        if snr >= threshold:
+        if sigma > 0.0 and snr >= threshold:      # sigma = 0 (all-zero image): snr := 0, never a candidate (A24)
             l = x if x < npix // 2 else x - npix
             m = y if y < npix // 2 else y - npix
             cands.append(Candidate(d, k, j, l, m, peak, sigma, snr))

@@ -22,8 +22,9 @@ EXPORTS = [
     "rf_debug_image", "rf_plan_get_counters", "rf_plan_set_batch", "rf_last_error",
     "rf_search_host", "rf_plan_set_profiling", "rf_plan_get_kernel_times", "rf_plan_set_mode",
     "rf_plan_set_meansub", "rf_prep_meansub", "rf_cand_spectrum", "rf_inject",
-    "rf_search_periodic", "rf_plan_periodic_nt", "rf_debug_periodic_image",
+    "rf_search_periodic", "rf_plan_periodic_nt", "rf_debug_periodic_image", "rf_plan_set_tuning",
 ]
+RF_TUNE_AUX_WIDTHS, RF_TUNE_DM_GROUP, RF_TUNE_FEED_BATCH, RF_TUNE_TREE_MAXPIX = 1, 2, 3, 4
 
 # numpy view of rf_cand (32 bytes)
 CAND_DTYPE = np.dtype([("dm_idx", "<i4"), ("dt_idx", "<i4"), ("t_idx", "<i4"), ("l_pix", "<i4"),
@@ -67,6 +68,7 @@ def load_library() -> C.CDLL:
     lib.rf_plan_set_uvw.argtypes = [vp, dp, C.c_double]
     lib.rf_plan_set_search_span.argtypes = [vp, C.c_int]
     lib.rf_plan_set_batch.argtypes = [vp, C.c_int]
+    lib.rf_plan_set_tuning.argtypes = [vp, C.c_int, C.c_int]
     lib.rf_plan_get_tables.argtypes = [vp, ip, ip, C.POINTER(C.c_uint8)]
     lib.rf_plan_num_images.argtypes = [vp]
     lib.rf_plan_num_images.restype = C.c_int64
@@ -148,6 +150,10 @@ class Plan:
 
     def set_batch(self, n: int) -> None:
         _check(self._lib.rf_plan_set_batch(self._h, n))
+
+    def set_tuning(self, knob: int, value: int) -> None:
+        """rf_plan_set_tuning: knobs RF_TUNE_* (no effect on results)."""
+        _check(self._lib.rf_plan_set_tuning(self._h, knob, value))
 
     # -- queries
     def get_tables(self):

@@ -32,6 +32,17 @@ int rebuild_geometry(rf_plan* p) {
     return RF_OK;
 }
 
+// A plan lives on the device it was created on (tables, workspace, kernel attributes): the caller must have that
+// device current when it enqueues work.
+int check_device(const rf_plan* p) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != p->device) {
+        set_error("plan was created on CUDA device %d but device %d is current", p->device, dev);
+        return RF_ERR_STATE;
+    }
+    return RF_OK;
+}
+
 void free_tables(rf_plan* p) {
     rf::DeviceTables& d = p->d;
     cudaFree(d.delay); cudaFree(d.cell); cudaFree(d.keep); cudaFree(d.gen.entries); cudaFree(d.gen.warp_chunk);
@@ -77,6 +88,11 @@ int rf_plan_create(rf_plan** out, const double* freqs_hz, int nchan, const doubl
     p->weights.assign(nchan, 1.0f);
     p->nbins = 2048;
     rf::configure_tree(p);
+    if (cudaGetDevice(&p->device) != cudaSuccess) {
+        set_error("cudaGetDevice failed: %s", cudaGetErrorString(cudaGetLastError()));
+        delete p;
+        return RF_ERR_CUDA;
+    }
     if (cudaStreamCreateWithFlags(&p->tab_stream, cudaStreamNonBlocking) != cudaSuccess) {
         set_error("cudaStreamCreate failed: %s", cudaGetErrorString(cudaGetLastError()));
         delete p;
@@ -109,6 +125,7 @@ int rf_search(rf_plan* p, const void* vis_dev, void* cuda_stream, rf_cand_out* o
         return RF_ERR_ARG;
     }
     if (reinterpret_cast<uintptr_t>(vis_dev) & 15) { set_error("vis_dev must be 16-byte aligned"); return RF_ERR_ARG; }
+    if (int rc_d = check_device(p)) return rc_d;
     return rf::launch_search(p, vis_dev, static_cast<cudaStream_t>(cuda_stream), out);
 }
 
@@ -117,6 +134,7 @@ int rf_search_host(rf_plan* p, const void* vis_host, rf_cand* cand_host, int32_t
         set_error("null pointer argument");
         return RF_ERR_ARG;
     }
+    if (int rc_d = check_device(p)) return rc_d;
     const size_t vis_bytes = (size_t)p->nint * p->nbl * p->nchan * p->npol * 8;
     if (!p->own_stream) RF_CUDA_CHECK(cudaStreamCreateWithFlags(&p->own_stream, cudaStreamNonBlocking));
     if (!p->stage_vis) RF_CUDA_CHECK(cudaMalloc(&p->stage_vis, vis_bytes));
@@ -200,6 +218,7 @@ int rf_plan_set_meansub(rf_plan* p, int enable) {
 int rf_prep_meansub(rf_plan* p, void* vis_dev, void* cuda_stream) {
     if (!p || !vis_dev) { set_error("null pointer argument"); return RF_ERR_ARG; }
     if (reinterpret_cast<uintptr_t>(vis_dev) & 15) { set_error("vis_dev must be 16-byte aligned"); return RF_ERR_ARG; }
+    if (int rc_d = check_device(p)) return rc_d;
     return rf::launch_meansub_inplace(p, vis_dev, static_cast<cudaStream_t>(cuda_stream));
 }
 
@@ -232,6 +251,28 @@ int rf_plan_set_batch(rf_plan* p, int n) {
     return RF_OK;
 }
 
+int rf_plan_set_tuning(rf_plan* p, int knob, int value) {
+    if (!p) { set_error("null plan"); return RF_ERR_ARG; }
+    switch (knob) {
+        case RF_TUNE_AUX_WIDTHS: p->tune_aux = value != 0; break;
+        case RF_TUNE_DM_GROUP:
+            if (value < 1) { set_error("DM group must be >= 1"); return RF_ERR_ARG; }
+            p->tune_dm_group = value;
+            break;
+        case RF_TUNE_FEED_BATCH:
+            if (value < 0) { set_error("feed batch must be >= 0"); return RF_ERR_ARG; }
+            p->tune_feed_batch = value;
+            return RF_OK;                              // read at launch time: nothing to rebuild
+        case RF_TUNE_TREE_MAXPIX:
+            if (value < 0) { set_error("tree maxpix must be >= 0"); return RF_ERR_ARG; }
+            p->tune_tree_maxpix = value;
+            break;
+        default: set_error("unknown tuning knob %d", knob); return RF_ERR_ARG;
+    }
+    rf::configure_tree(p);
+    return rebuild_geometry(p);
+}
+
 int rf_plan_get_tables(rf_plan* p, int32_t* delay_host, int32_t* cell_host, uint8_t* keep_host) {
     if (!p) { set_error("null plan"); return RF_ERR_ARG; }
     if (delay_host) memcpy(delay_host, p->h_delay.data(), p->h_delay.size() * sizeof(int32_t));
@@ -253,6 +294,7 @@ int rf_debug_image(rf_plan* p, const void* vis_dev, int dm_idx, int dt_idx, int 
     if (dm_idx < 0 || dm_idx >= p->ndm || dt_idx < 0 || dt_idx >= p->ndt) { set_error("trial index out of range"); return RF_ERR_STATE; }
     const int dt = p->dts[dt_idx];
     if (t_idx < 0 || (long long)(t_idx + 1) * dt > p->nint - p->h_maxdelay[dm_idx]) { set_error("t_idx out of range"); return RF_ERR_STATE; }
+    if (int rc_d = check_device(p)) return rc_d;
     return rf::launch_debug_image(p, vis_dev, dm_idx, dt_idx, t_idx, image_dev, stats_dev,
                                   static_cast<cudaStream_t>(cuda_stream));
 }
@@ -263,6 +305,7 @@ int rf_cand_spectrum(rf_plan* p, const void* vis_dev, int dm_idx, int dt_idx, in
     if (dm_idx < 0 || dm_idx >= p->ndm || dt_idx < 0 || dt_idx >= p->ndt) { set_error("trial index out of range"); return RF_ERR_STATE; }
     if (half_window < 0 || half_window > 32767) { set_error("half_window out of range"); return RF_ERR_ARG; }
     if (l_pix < -p->npix || l_pix >= p->npix || m_pix < -p->npix || m_pix >= p->npix) { set_error("pixel out of range"); return RF_ERR_ARG; }
+    if (int rc_d = check_device(p)) return rc_d;
     return rf::launch_cand_spectrum(p, vis_dev, dm_idx, dt_idx, t_idx, l_pix, m_pix, half_window, spec_dev,
                                     static_cast<cudaStream_t>(cuda_stream));
 }
@@ -274,6 +317,7 @@ int rf_inject(rf_plan* p, void* vis_dev, double amp, double l_pix, double m_pix,
         set_error("invalid source parameters");
         return RF_ERR_ARG;
     }
+    if (int rc_d = check_device(p)) return rc_d;
     return rf::launch_inject(p, vis_dev, amp, l_pix, m_pix, dm, width, t0, static_cast<cudaStream_t>(cuda_stream));
 }
 
@@ -283,6 +327,7 @@ int rf_search_periodic(rf_plan* p, const void* vis_dev, void* cuda_stream, rf_ca
         return RF_ERR_ARG;
     }
     if (reinterpret_cast<uintptr_t>(vis_dev) & 15) { set_error("vis_dev must be 16-byte aligned"); return RF_ERR_ARG; }
+    if (int rc_d = check_device(p)) return rc_d;
     return rf::launch_search_periodic(p, vis_dev, static_cast<cudaStream_t>(cuda_stream), out, -1, 0, nullptr, nullptr);
 }
 
@@ -297,6 +342,7 @@ int rf_debug_periodic_image(rf_plan* p, const void* vis_dev, int dm_idx, int k, 
     if (dm_idx < 0 || dm_idx >= p->ndm) { set_error("trial index out of range"); return RF_ERR_STATE; }
     const int nt = rf::periodic_nt(p, dm_idx);
     if (k < 1 || k > nt / 2) { set_error("fluctuation-frequency bin out of range"); return RF_ERR_STATE; }
+    if (int rc_d = check_device(p)) return rc_d;
     return rf::launch_search_periodic(p, vis_dev, static_cast<cudaStream_t>(cuda_stream), nullptr, dm_idx, k, power_dev,
                                       stats_dev);
 }
@@ -305,7 +351,7 @@ int rf_plan_get_counters(rf_plan* p, rf_counters* out) {
     if (!p || !out) { set_error("null pointer argument"); return RF_ERR_ARG; }
     int32_t c[4] = {0, 0, 0, 0};
     if (p->ws.counters) RF_CUDA_CHECK(cudaMemcpy(c, p->ws.counters, sizeof(c), cudaMemcpyDeviceToHost));
-    out->images = p->n_images;
+    out->images = c[1];               // counted by the kernels: one per finalised image of the last search
     out->vis_gridded = p->vis_gridded;
     out->n_kept = p->n_kept;
     out->n_dropped = p->n_dropped;

@@ -150,6 +150,13 @@ struct rf_plan {
     bool use_tree = true;            // image-domain boxcar tree for power-of-two dt (rf_plan_set_mode)
     bool meansub = false;            // search vis - mean_t(vis) (rf_plan_set_meansub)
     int user_batch = 0;
+    int device = 0;                  // CUDA device the plan was created on (checked by every entry point that launches)
+    // tuning knobs (rf_plan_set_tuning): none of them changes a result
+    bool tune_aux = true;            // widths off the tree ride the tree kernels on phase-decimated sums (B7)
+    int tune_dm_group = rf::kDmGroup;   // DM trials interleaved in time by the block order
+    int tune_feed_batch = 0;         // blocks per launch behind an upload (0 = one wave of row-pass CTAs)
+    int tune_tree_maxpix = 4096;     // largest npix searched by the boxcar-tree kernels
+    std::map<const void*, size_t> smem_attr;   // dynamic shared memory opted in per kernel, on this plan's device
     std::vector<double> freqs, uvw, dms;
     std::vector<int32_t> dts;
     std::vector<float> weights;      // [nchan]
@@ -200,6 +207,10 @@ int build_cell_table(rf_plan* p);             // device kernel (float64) -> d.ce
 int build_grid_lists(rf_plan* p);             // host binning of the cell table -> d.gen, d.tree
 int aux_pitch_of(const rf_plan* p, int dt);   // row pitch of the phase-decimated sum array of a width
 int build_image_list(rf_plan* p);             // (dm, dt, j) loop -> d.images (generic) + d.blocks (tree)
+size_t phase_sum_smem(int dt, int* jc_out);   // dynamic shared memory (and JC) of k_phase_sum for a width
+constexpr size_t kMaxDynSmem = 227 * 1024;    // opt-in limit per CTA on sm_100a
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) once per (plan = device, kernel); kernels are per-device objects
+int ensure_smem_attr(rf_plan* p, const void* kern, size_t smem);
 int tree_cols_per_group(int npix, int tb);
 void configure_tree(rf_plan* p);              // which dt values ride the boxcar tree    // columns per pass-1 CTA of the tree path
 // rf_prep.cu

@@ -21,9 +21,6 @@ struct SearchParams {
     const float* vis;               // complex64 [nint][nbl][nchan][npol] as floats
     const float2* mean_i;           // [nbl*nchan] Stokes-I sum of the time means, or null (no subtraction)
     const float2* visI;             // [nbl*nchan][tpitch] time-fastest Stokes-I sums (mean already removed), or null
-    const float2* visS;             // [n_slots][nbl*nchan][tpitch] sliding sums over dt of visI, or null
-    const int32_t* gen_slot;        // [ndt] slot of each width in visS, or -1
-    long long visS_stride;          // elements per slot
     int32_t tpitch;
     const int32_t* delay;           // [ndm][nchan]
     const GridEntry* entries;
@@ -167,53 +164,6 @@ __device__ __forceinline__ void gather_grid_visi(const SearchParams& p, float2* 
     }
 }
 
-// The gather from a sliding-sum array (one pre-summed sample per entry): the chunks of a warp are
-// independent until their commit, so U chunks are kept in flight (entries of the next U prefetched behind
-// the loads of the current ones) -- the loop is otherwise a chain of two dependent global loads per chunk.
-template <int PITCH>
-__device__ __forceinline__ void gather_grid_presummed(const SearchParams& p, float2* __restrict__ tile,
-                                                      const int* __restrict__ sdelay, int t_first,
-                                                      int c_beg, int c_end, int lane,
-                                                      const float2* __restrict__ arr) {
-    constexpr int U = 4;
-    GridEntry en[U];
-#pragma unroll
-    for (int u = 0; u < U; u++)
-        en[u] = (c_beg + u < c_end) ? p.entries[(size_t)(c_beg + u) * 32 + lane] : GridEntry{0u, 0u};
-    for (int ck = c_beg; ck < c_end; ck += U) {
-        GridEntry e[U];
-        float2 a[U];
-#pragma unroll
-        for (int u = 0; u < U; u++) e[u] = en[u];
-#pragma unroll
-        for (int u = 0; u < U; u++) {
-            a[u] = make_float2(0.f, 0.f);
-            if (e[u].w0 >> 31) a[u] = __ldg(arr + (size_t)(e[u].w0 & 0xffffffu) * p.tpitch + (t_first + sdelay[e[u].w1 & 0xfff]));
-        }
-#pragma unroll
-        for (int u = 0; u < U; u++)
-            en[u] = (ck + U + u < c_end) ? p.entries[(size_t)(ck + U + u) * 32 + lane] : GridEntry{0u, 0u};
-#pragma unroll
-        for (int u = 0; u < U; u++) {
-            float re = a[u].x, im = (e[u].w0 & (1u << 30)) ? -a[u].y : a[u].y;
-            const int dist = (e[u].w0 >> 24) & 31;
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                float r2 = __shfl_up_sync(0xffffffffu, re, d);
-                float i2 = __shfl_up_sync(0xffffffffu, im, d);
-                if (dist >= d) { re += r2; im += i2; }
-            }
-            if ((e[u].w0 >> 31) && (e[u].w0 & (1u << 29))) {
-                const int row = (e[u].w1 >> 12) & 0xfff, col = (e[u].w1 >> 24) & 0xf;
-                float2* dst = &tile[col * PITCH + fft_pad(row)];
-                float2 cur = *dst;
-                *dst = make_float2(cur.x + re, cur.y + im);
-            }
-            __syncwarp();
-        }
-    }
-}
-
 // ------------------------------------------------------------------------------------------
 // Pass 1.  grid = (n_img, ngroups): group-major launch order, so the heavy central column
 // groups start first (measured faster than image-major order); block = 256.  Dynamic smem:
@@ -243,10 +193,7 @@ __global__ void __launch_bounds__(kThreads) k_grid_colfft(const SearchParams p) 
         const int c_beg = p.warp_chunk[g * kWarpsPerCta + warp];
         const int c_end = p.warp_chunk[g * kWarpsPerCta + warp + 1];
         const float* base = p.vis + (long long)im.j * im.dt * p.row_floats;
-        const int vslot = p.visS != nullptr ? p.gen_slot[im.dt_idx] : -1;
-        // a width with a sliding-sum array reads ONE pre-summed sample per entry (sum of dt integrations)
-        if (vslot >= 0) gather_grid_presummed<PITCH>(p, tile, sdelay, im.j * im.dt, c_beg, c_end, lane, p.visS + vslot * p.visS_stride);
-        else if (p.visI != nullptr) gather_grid_visi<PITCH>(p, tile, sdelay, im.j * im.dt, c_beg, c_end, lane, im.dt, p.visI);
+        if (p.visI != nullptr) gather_grid_visi<PITCH>(p, tile, sdelay, im.j * im.dt, c_beg, c_end, lane, im.dt, p.visI);
         else switch (im.dt) {   // compile-time widths keep U x DT independent 16-byte loads in flight per lane
             case 1: gather_grid<NPOL, 1, 8, PITCH>(p, tile, sdelay, base, c_beg, c_end, lane, 1); break;
             case 2: gather_grid<NPOL, 2, 4, PITCH>(p, tile, sdelay, base, c_beg, c_end, lane, 2); break;
@@ -620,7 +567,9 @@ __global__ void __launch_bounds__(kThreads) k_rowfft_stats(const SearchParams p)
                 c.peak = peak; c.sigma = sigma; c.snr = snr;
                 if (overflow) atomicAdd(&p.counters[0], 1);
                 if (p.stats_out != nullptr && slot_a + which == 0) *p.stats_out = c;
-                if (p.cand_count != nullptr && snr >= p.threshold) {
+                if (p.cand_count != nullptr) atomicAdd(&p.counters[1], 1);   // images finalised (rf_counters.images)
+                // an all-zero image (sigma = 0) has snr := 0 and is never a candidate (reading A24)
+                if (p.cand_count != nullptr && sigma > 0.f && snr >= p.threshold) {
                     int idx = atomicAdd(p.cand_count, 1);
                     if (idx < p.cand_capacity) p.cand_items[idx] = c;
                 }

@@ -13,6 +13,18 @@
 
 namespace rf {
 
+// Kernel attributes are per-device state: every plan (created on one device, rf_plan::device) opts each kernel into
+// its dynamic shared memory itself, once per size increase.  Requests at or below the 48 KB default need no opt-in.
+int ensure_smem_attr(rf_plan* p, const void* kern, size_t smem) {
+    if (smem <= 48 * 1024) return RF_OK;
+    if (smem > kMaxDynSmem) { set_error("internal: kernel needs %zu bytes of shared memory (limit %zu)", smem, kMaxDynSmem); return RF_ERR_STATE; }
+    size_t& have = p->smem_attr[kern];
+    if (smem <= have) return RF_OK;
+    RF_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    have = smem;
+    return RF_OK;
+}
+
 namespace {
 
 template <int N> size_t smem_pass1(int nchan, int ncolgrp) {
@@ -27,39 +39,31 @@ template <int N> size_t smem_pass2(int nbins) {
 }
 
 template <int N, int NPOL, int NCOL>
-int launch_pass1(const SearchParams& sp, int nchan, cudaStream_t st) {
+int launch_pass1(rf_plan* p, const SearchParams& sp, int nchan, cudaStream_t st) {
     auto kern = k_grid_colfft<N, NPOL, NCOL>;
     const size_t smem = smem_pass1<N>(nchan, NCOL);
-    static size_t configured = 0;
-    if (smem > configured) {
-        RF_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = smem;
-    }
+    { const int rc_a = ensure_smem_attr(p, (const void*)kern, smem); if (rc_a != RF_OK) return rc_a; }
     kern<<<dim3(sp.n_img, sp.ngroups), kThreads, smem, st>>>(sp);
     RF_CUDA_CHECK(cudaGetLastError());
     return RF_OK;
 }
 
 template <int N, int NCOL>
-int launch_pass1_npol(const SearchParams& sp, int nchan, int npol, cudaStream_t st) {
+int launch_pass1_npol(rf_plan* p, const SearchParams& sp, int nchan, int npol, cudaStream_t st) {
     switch (npol) {
-        case 1: return launch_pass1<N, 1, NCOL>(sp, nchan, st);
-        case 2: return launch_pass1<N, 2, NCOL>(sp, nchan, st);
-        case 4: return launch_pass1<N, 4, NCOL>(sp, nchan, st);
+        case 1: return launch_pass1<N, 1, NCOL>(p, sp, nchan, st);
+        case 2: return launch_pass1<N, 2, NCOL>(p, sp, nchan, st);
+        case 4: return launch_pass1<N, 4, NCOL>(p, sp, nchan, st);
     }
     set_error("unsupported npol %d", npol);
     return RF_ERR_ARG;
 }
 
 template <int N>
-int launch_pass2(const SearchParams& sp, cudaStream_t st) {
+int launch_pass2(rf_plan* p, const SearchParams& sp, cudaStream_t st) {
     auto kern = k_rowfft_stats<N, exact_stats<N>()>;
     const size_t smem = smem_pass2<N>(sp.nbins);
-    static size_t configured = 0;
-    if (smem > configured) {
-        RF_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = smem;
-    }
+    { const int rc_a = ensure_smem_attr(p, (const void*)kern, smem); if (rc_a != RF_OK) return rc_a; }
     kern<<<dim3(sp.rsplit, (sp.n_img + 1) / 2), kThreads, smem, st>>>(sp);
     RF_CUDA_CHECK(cudaGetLastError());
     return RF_OK;
@@ -86,9 +90,9 @@ int launch_batch(rf_plan* p, const SearchParams& sp, cudaStream_t st) {
     switch (p->npix) {
 #define RF_CASE(N, NCOL)                                                                    \
     case N:                                                                                 \
-        if ((rc = launch_pass1_npol<N, NCOL>(sp, p->nchan, p->npol, st)) != RF_OK) return rc; \
+        if ((rc = launch_pass1_npol<N, NCOL>(p, sp, p->nchan, p->npol, st)) != RF_OK) return rc; \
         if ((rc = mark(p, st, 0)) != RF_OK) return rc;                                      \
-        if ((rc = launch_pass2<N>(sp, st)) != RF_OK) return rc;                             \
+        if ((rc = launch_pass2<N>(p, sp, st)) != RF_OK) return rc;                             \
         return mark(p, st, 1);
         RF_CASE(64, 16)
         RF_CASE(128, 16)
@@ -116,7 +120,16 @@ template <int N, int TB> size_t smem_tree2(int nbins, int cpad, int nthreads = k
     const size_t xb = g2 * fft_padded_size(N) * sizeof(float2);
     const size_t fin = (size_t)2 * nbins * sizeof(uint32_t);
     return std::max(xb, fin) + FftCfg<N>::TW_TOTAL * sizeof(float2) + g2 * cpad * sizeof(float4) +
-           (size_t)(N >= 2048 ? 2 * TB - 1 : TB) * nbins * sizeof(uint32_t) + 64 * 4 + (size_t)2 * kWarps2 * (2 * TB - 1) * 4;
+           (size_t)(N >= 2048 ? 2 * TB - 1 : TB) * nbins * sizeof(uint32_t) + 80 * 4 + (size_t)2 * kWarps2 * (2 * TB - 1) * 4;
+}
+
+// power variant of the row pass (periodicity search): 512 threads, one 32-bit histogram per pair = TB/2 images
+template <int N, int TB> size_t smem_tree2_power(int nbins, int cpad) {
+    const size_t g2 = kThreads2 / FftCfg<N>::TPF;
+    const size_t xb = g2 * fft_padded_size(N) * sizeof(float2);
+    const size_t fin = (size_t)2 * nbins * sizeof(uint32_t);
+    return std::max(xb, fin) + FftCfg<N>::TW_TOTAL * sizeof(float2) + g2 * cpad * sizeof(float4) +
+           (size_t)(TB / 2) * nbins * sizeof(uint32_t) + 64 * 4 + (size_t)2 * kWarps2 * TB * 4;
 }
 
 // event kinds: 0 = grid + column FFT (generic pass 1 / tree column FFT), 1 = row FFT + statistics,
@@ -137,23 +150,15 @@ int launch_tree(rf_plan* p, const TreeParams& tp, cudaStream_t st) {
         constexpr int NTH = N >= 4096 ? 512 : kThreads;   // two concurrent 4096-point transforms per CTA
         auto kern = k_tree_colfft<N, TB, NCOL, QH, NTH>;
         const size_t smem = smem_tree1<N>(QH * NCOL);
-        static size_t configured = 0;
-        if (smem > configured) {
-            RF_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            configured = smem;
-        }
+        { const int rc_a = ensure_smem_attr(p, (const void*)kern, smem); if (rc_a != RF_OK) return rc_a; }
         kern<<<dim3(tp.ngroups, tp.n_blk, TB / QH), NTH, smem, st>>>(tp);
         RF_CUDA_CHECK(cudaGetLastError());
         if ((rc = mark(p, st, 0)) != RF_OK) return rc;
     }
     if (tp.zero_row >= 0) {    // periodicity search: every pair is one complex image, searched in power
         auto kern = k_tree_rowfft_power<N, TB>;
-        const size_t smem = smem_tree2<N, TB>(tp.nbins, tp.cpad);
-        static size_t configured = 0;
-        if (smem > configured) {
-            RF_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            configured = smem;
-        }
+        const size_t smem = smem_tree2_power<N, TB>(tp.nbins, tp.cpad);
+        { const int rc_a = ensure_smem_attr(p, (const void*)kern, smem); if (rc_a != RF_OK) return rc_a; }
         kern<<<dim3(tp.n_blk), kThreads2, smem, st>>>(tp);
         RF_CUDA_CHECK(cudaGetLastError());
         return mark(p, st, 1);
@@ -162,11 +167,7 @@ int launch_tree(rf_plan* p, const TreeParams& tp, cudaStream_t st) {
         constexpr int NT2 = tree2_threads<N>();
         auto kern = k_tree_rowfft_stats<N, TB, NT2>;
         const size_t smem = smem_tree2<N, TB>(tp.nbins, tp.cpad, NT2);
-        static size_t configured = 0;
-        if (smem > configured) {
-            RF_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            configured = smem;
-        }
+        { const int rc_a = ensure_smem_attr(p, (const void*)kern, smem); if (rc_a != RF_OK) return rc_a; }
         kern<<<dim3(tp.n_blk), NT2, smem, st>>>(tp);
         RF_CUDA_CHECK(cudaGetLastError());
         if ((rc = mark(p, st, 1)) != RF_OK) return rc;
@@ -240,6 +241,33 @@ TreeParams tree_params(rf_plan* p) {
     tp.norm = p->n_kept > 0 ? (float)(1.0 / (2.0 * (double)p->n_kept * (double)p->npol)) : 0.f;
     tp.threshold = p->threshold;
     return tp;
+}
+
+// Widths off the tree (B7): the phase-decimated boxcar sums of width dts[k] from the Stokes-I array (once per segment) ...
+int launch_phase_sum(rf_plan* p, int k, cudaStream_t st) {
+    const int dt = p->dts[k], pitch = p->aux_pitch[k], nelem = p->nbl * p->nchan;
+    float2* arr = p->ws.visS + p->ws.aux_off[k];
+    int rc;
+    if ((rc = mark(p, st, -1)) != RF_OK) return rc;
+    int JC = 8;
+    const size_t psm = phase_sum_smem(dt, &JC);
+    if ((rc = ensure_smem_attr(p, (const void*)k_phase_sum, psm)) != RF_OK) return rc;
+    k_phase_sum<<<dim3(nelem, (pitch + JC - 1) / JC), 256, psm, st>>>(p->ws.visI, arr, dt, p->tpitch, pitch, nelem, JC);
+    RF_CUDA_CHECK(cudaGetLastError());
+    return mark(p, st, 2);
+}
+// ... and the parameters with which the unchanged tree kernels search that array: level 0 of the tree = the width itself
+TreeParams aux_tree_params(rf_plan* p, const TreeParams& tp, int k) {
+    const int dt = p->dts[k], pitch = p->aux_pitch[k], nelem = p->nbl * p->nchan;
+    TreeParams t2 = tp;
+    t2.entries = p->d.aux_entries[k];
+    t2.visI = p->ws.visS + p->ws.aux_off[k];
+    t2.dec = dt;
+    t2.phase_stride = (uint32_t)((size_t)(nelem + 1) * pitch);
+    t2.dt_idx[0] = k;
+    for (int l = 1; l < 4; l++) t2.dt_idx[l] = -1;
+    t2.norm = tp.norm / (float)dt;
+    return t2;
 }
 
 // Device buffers only ever grow (25 % headroom): the sizes follow the gridding lists, which change with every
@@ -447,7 +475,7 @@ int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out
             cudaGetDevice(&dev);
             cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
             small = std::min(small, sms) & ~1;
-            if (const char* e = getenv("RF_FEED_BATCH")) small = std::max(2, std::min(p->ws.blk_batch, atoi(e)) & ~1);
+            if (p->tune_feed_batch > 0) small = std::max(2, std::min(p->ws.blk_batch, p->tune_feed_batch) & ~1);
         }
         for (int64_t base = 0; base < p->n_blocks;) {
             int n = (int)std::min<int64_t>(p->ws.blk_batch, p->n_blocks - base);
@@ -465,30 +493,9 @@ int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out
         for (int k = 0; k < p->ndt; k++) {
             const int64_t nb2 = p->aux_first[k + 1] - p->aux_first[k];
             if (!p->aux_width[k] || nb2 == 0) continue;
-            const int dt = p->dts[k], pitch = p->aux_pitch[k], nelem = p->nbl * p->nchan;
-            float2* arr = p->ws.visS + p->ws.aux_off[k];
-            if ((rc = mark(p, st, -1)) != RF_OK) return rc;
-            const int JC = std::max(8, 2048 / dt);
-            const size_t psm = ((size_t)JC * dt + dt + (size_t)JC * dt + JC * dt / 32 + 2) * sizeof(float2);
-            if (psm > 48 * 1024) {    // very wide boxcars: beyond the default dynamic shared-memory window
-                static size_t configured = 0;
-                if (psm > configured) {
-                    RF_CUDA_CHECK(cudaFuncSetAttribute(k_phase_sum, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)psm));
-                    configured = psm;
-                }
-            }
-            k_phase_sum<<<dim3(nelem, (pitch + JC - 1) / JC), 256, psm, st>>>(p->ws.visI, arr, dt, p->tpitch, pitch, nelem, JC);
-            RF_CUDA_CHECK(cudaGetLastError());
-            if ((rc = mark(p, st, 2)) != RF_OK) return rc;
+            if ((rc = launch_phase_sum(p, k, st)) != RF_OK) return rc;
             p->last_launches += 1;
-            TreeParams t2 = tp;
-            t2.entries = p->d.aux_entries[k];
-            t2.visI = arr;
-            t2.dec = dt;
-            t2.phase_stride = (uint32_t)((size_t)(nelem + 1) * pitch);
-            t2.dt_idx[0] = k;
-            for (int l = 1; l < 4; l++) t2.dt_idx[l] = -1;
-            t2.norm = tp.norm / (float)dt;
+            TreeParams t2 = aux_tree_params(p, tp, k);
             for (int64_t base = 0; base < nb2; base += p->ws.blk_batch) {
                 t2.blocks = p->d.blocks2 + p->aux_first[k] + base;
                 t2.n_blk = (int)std::min<int64_t>(p->ws.blk_batch, nb2 - base);
@@ -541,6 +548,26 @@ int launch_debug_image(rf_plan* p, const void* vis, int dm_idx, int dt_idx, int 
         tp.cand_count = nullptr;
         return launch_tree_batch(p, tp, st);
     }
+    if (p->tree_tb > 0 && p->n_kept > 0 && p->aux_width[dt_idx]) {
+        // a width searched on its phase-decimated sums (B7): the same kernels as rf_search, image t_idx = level-0
+        // node t_idx % TB of block t_idx / TB of this (dm, width)
+        const int TB = p->tree_tb, tb = t_idx / TB;
+        const int nj = p->h_num_t[(size_t)dm_idx * p->ndt + dt_idx];
+        BlockDesc b[2] = {{dm_idx, tb & ~1, nj, 0}, {dm_idx, tb | 1, nj, 0}};
+        RF_CUDA_CHECK(cudaMemcpyAsync(p->ws.dbg_block, b, sizeof(b), cudaMemcpyHostToDevice, st));
+        RF_CUDA_CHECK(cudaStreamSynchronize(st));
+        if ((rc = launch_prep(p, vis, st)) != RF_OK) return rc;
+        if ((rc = launch_phase_sum(p, dt_idx, st)) != RF_OK) return rc;
+        TreeParams tp = aux_tree_params(p, tree_params(p), dt_idx);
+        tp.blocks = p->ws.dbg_block;
+        tp.n_blk = 2;
+        tp.dbg_slot = tb & 1;
+        tp.image_out = image_dev;
+        tp.stats_out = stats_dev;
+        tp.dbg_img = t_idx % TB;
+        tp.cand_count = nullptr;
+        return launch_tree_batch(p, tp, st);
+    }
     ImgDesc d{dm_idx, dt_idx, t_idx, p->dts[dt_idx]};
     RF_CUDA_CHECK(cudaMemcpyAsync(p->ws.dbg_desc, &d, sizeof(d), cudaMemcpyHostToDevice, st));
     RF_CUDA_CHECK(cudaStreamSynchronize(st));   // `d` lives on this stack frame (debug hook only)
@@ -578,11 +605,7 @@ int launch_time_fft(rf_plan* p, const int32_t* delay_dm, const float2* tw, float
     constexpr int G = kThreads / FftCfg<NT>::TPF;
     auto kern = k_time_fft<NT>;
     const size_t smem = ((size_t)G * fft_padded_size(NT) + FftCfg<NT>::TW_TOTAL) * sizeof(float2);
-    static size_t configured = 0;
-    if (smem > configured) {
-        RF_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = smem;
-    }
+    { const int rc_a = ensure_smem_attr(p, (const void*)kern, smem); if (rc_a != RF_OK) return rc_a; }
     const int nelem = p->nbl * p->nchan;
     kern<<<(nelem + G - 1) / G, kThreads, smem, st>>>(p->ws.visI, delay_dm, tw, slab, nelem, p->nchan, p->tpitch,
                                                        p->ws.slab_pitch);

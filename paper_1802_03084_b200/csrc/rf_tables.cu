@@ -298,10 +298,17 @@ int aux_pitch_of(const rf_plan* p, int dt) { return (((p->tpitch + dt - 1) / dt 
 
 // Which widths off the tree are searched by the tree kernels on phase-decimated sums (B7): every width > 1 while the
 // sum arrays fit kSlidingSumBudget (each is about the size of the Stokes-I array); the rest takes the per-image path.
+// Dynamic shared memory of k_phase_sum for a width: in [JC*dt + dt] | sums [JC*dt padded by 1/32] float2.
+size_t phase_sum_smem(int dt, int* jc_out) {
+    const int JC = std::max(8, 2048 / dt);
+    if (jc_out) *jc_out = JC;
+    return ((size_t)JC * dt + dt + (size_t)JC * dt + (size_t)JC * dt / 32 + 2) * sizeof(float2);
+}
+
 static void decide_aux_widths(rf_plan* p) {
     p->aux_width.assign(p->ndt, 0);
     p->aux_pitch.assign(p->ndt, 0);
-    if (p->tree_tb == 0 || getenv("RF_NO_AUX")) return;
+    if (p->tree_tb == 0 || !p->tune_aux) return;
     size_t bytes = 0;
     for (int k = 0; k < p->ndt; k++) {
         bool in_tree = false;
@@ -310,6 +317,7 @@ static void decide_aux_widths(rf_plan* p) {
         if (in_tree || dt <= 1 || dt >= p->nint) continue;
         const size_t need = (size_t)dt * ((size_t)p->nbl * p->nchan + 1) * aux_pitch_of(p, dt) * sizeof(float2);
         if (bytes + need > kSlidingSumBudget || need / sizeof(float2) >= (1ull << 32)) continue;
+        if (phase_sum_smem(dt, nullptr) > kMaxDynSmem) continue;     // very wide boxcars: per-image path
         bytes += need;
         p->aux_width[k] = 1;
         p->aux_pitch[k] = aux_pitch_of(p, dt);
@@ -322,12 +330,12 @@ void configure_tree(rf_plan* p) {
     // which dt values ride the image-domain boxcar tree (B3)
     p->tree_tb = 0;
     for (int l = 0; l < 4; l++) p->tree_dt_idx[l] = -1;
-    // every size from 256 up rides the tree (N >= 2048: 256-thread row-pass CTAs, see launch_tree); RF_TREE_MAXPIX
-    // lowers the limit for experiments
-    int tree_maxpix = 4096;
-    if (const char* e = getenv("RF_TREE_MAXPIX")) tree_maxpix = atoi(e);
-    if (p->use_tree && p->npix >= 256 && p->npix <= tree_maxpix) {
-        const int tb_max = 8;
+    // every size from 256 up rides the tree (N >= 2048: 256-thread row-pass CTAs, see launch_tree);
+    // rf_plan_set_tuning(RF_TUNE_TREE_MAXPIX) lowers the limit
+    if (p->use_tree && p->npix >= 256 && p->npix <= p->tune_tree_maxpix) {
+        // N >= 2048: the row pass keeps one 32-bit histogram per image, so TB stops at 4 there (launch_tree_batch);
+        // a width of 8 then rides the phase-decimated sums (B7) like any other width off the tree
+        const int tb_max = p->npix >= 2048 ? 4 : 8;
         for (int k = 0; k < p->ndt; k++) {
             const int dt = p->dts[k];
             for (int l = 0; l < 4; l++)
@@ -375,8 +383,7 @@ int build_image_list(rf_plan* p) {
     std::vector<int> order(p->ndm);
     for (int d = 0; d < p->ndm; d++) order[d] = d;
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return p->h_maxdelay[a] < p->h_maxdelay[b]; });
-    int dm_group = kDmGroup;
-    if (const char* e = getenv("RF_DMGROUP")) dm_group = std::max(1, atoi(e));
+    const int dm_group = std::max(1, p->tune_dm_group);
     // Image order of the per-image path: per width, DM groups, output integration j in the OUTER loop and
     // the DM trials of the group inside.  Concurrent CTAs of one column group (blockIdx.x = image) then read
     // the same (baseline, channel) rows at times a few integrations apart: the 32-byte sectors of the

@@ -184,9 +184,6 @@ __global__ void __launch_bounds__(kThreads, 4) k_tree_gather(const TreeParams p)
     asm volatile("" : "+l"(vbase));     // one register pointer: a sample's address is then a single 32 x 8 + 64-bit multiply-add
     float2* cs = p.cellsum + (size_t)(slot + h) * p.n_cells * TB + q;
     float2 acc = make_float2(0.f, 0.f);
-#ifdef RF_EXP_NOGATHER
-    if (p.nchan < 0)
-#endif
     for (int it = it_beg; it < it_end; it += U) {
         uint32_t e[U];
         float2 x[U];
@@ -302,9 +299,6 @@ __global__ void __launch_bounds__(NTH) k_tree_colfft(const TreeParams p) {
     {
         constexpr int G1 = NTH / C::TPF;
         const int grp = tid / C::TPF, t = tid % C::TPF;
-#ifdef RF_EXP_NOFFT
-        if (p.nchan < 0)
-#endif
         for (int f = grp; f < NF; f += G1) {
             float2* col = tile + f * PITCH;
             float2 v[16];
@@ -337,9 +331,6 @@ __global__ void __launch_bounds__(NTH) k_tree_colfft(const TreeParams p) {
         const int i = tid % SEG, pr = i / NCOL, c = i % NCOL;
         const float2* ta = tile + (2 * pr * NCOL + c) * PITCH;
         const float2* tb = ta + NCOL * PITCH;
-#ifdef RF_EXP_NOSTORE
-        if (p.nchan < 0)
-#endif
         for (int y = y0; y < N; y += NTH / SEG) {
             const float2 a = ta[fft_pad(y)], b = tb[fft_pad(y)];
             Hs[((size_t)y * (TB / 2) + q0 / 2 + pr) * p.cpad + g * NCOL + c] = make_float4(a.x, a.y, b.x, b.y);
@@ -386,9 +377,6 @@ __device__ __forceinline__ void tree_row_stats(const float (&x)[16], int img, in
 #pragma unroll
     for (int e = 0; e < 16; e++) {
         const int q = min(max(__float_as_int(__fmaf_rd(x[e], A, Bm)), kMagicBits), top);
-#ifdef RF_EXP_NOHIST
-        if (q == 12345678)
-#endif
         asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(hw + (uint32_t)q * 4u), "r"(inc) : "memory");
         m = fmaxf(m, x[e]);
     }
@@ -449,7 +437,8 @@ __global__ void __launch_bounds__(NT2, NT2 == 512 ? 1 : 2) k_tree_rowfft_stats(c
     float* sScale = sA + 16;                                                 // [16]
     float* sSig = sScale + 16;                                               // [16] sigma_rms per image
     int* sValid = reinterpret_cast<int*>(sSig + 16);                         // [16]
-    float* sBest = reinterpret_cast<float*>(sValid + 16);                    // [16 warps][NIMG]
+    int* sInr = sValid + 16;                                                 // [16] 1 = an image of the search loop
+    float* sBest = reinterpret_cast<float*>(sInr + 16);                      // [16 warps][NIMG]
     int* sBpos = reinterpret_cast<int*>(sBest + NWP * NIMG);             // [16 warps][NIMG]
     uint32_t* hun = reinterpret_cast<uint32_t*>(xbuf);                       // after the row loop
     uint32_t* cum = hun + p.nbins;
@@ -480,7 +469,9 @@ __global__ void __launch_bounds__(NT2, NT2 == 512 ? 1 : 2) k_tree_rowfft_stats(c
         float tot = 0.f;
         for (int part = 0; part < p.n_parts; part++) tot += p.sumsq[((size_t)slot * NIMG + tid) * p.n_parts + part];
         const float sig = sqrtf(tot) / (float)dt;                // rms of the image (Parseval)
-        const bool valid = p.dt_idx[l] >= 0 && (j + 1) * dt <= blk.nsearch && sig > 0.f;
+        const bool inr = p.dt_idx[l] >= 0 && (j + 1) * dt <= blk.nsearch;
+        const bool valid = inr && sig > 0.f;              // an all-zero image has snr := 0 and is never a candidate
+        sInr[tid] = inr ? 1 : 0;
         sValid[tid] = valid ? 1 : 0;
         sSig[tid] = sig;
         sScale[tid] = 1.f / (float)dt;
@@ -609,13 +600,19 @@ __global__ void __launch_bounds__(NT2, NT2 == 512 ? 1 : 2) k_tree_rowfft_stats(c
                 c.peak = peak; c.sigma = sigma; c.snr = snr;
                 if (overflow) atomicAdd(&p.counters[0], 1);
                 if (report_zero) *p.stats_out = c;
-                if (p.cand_count != nullptr && sValid[img] && snr >= p.threshold) {
+                if (p.cand_count != nullptr && sValid[img] && sigma > 0.f && snr >= p.threshold) {
                     int idx = atomicAdd(p.cand_count, 1);
                     if (idx < p.cand_capacity) p.cand_items[idx] = c;
                 }
             }
         }
         __syncthreads();
+    }
+    // images of the search loop this CTA has finalised (rf_counters.images is counted on the device)
+    if (tid == 0 && p.cand_count != nullptr) {
+        int n = 0;
+        for (int img = 0; img < NIMG; img++) n += sInr[img];
+        if (n) atomicAdd(&p.counters[1], n);
     }
 }
 
@@ -714,6 +711,7 @@ __global__ void __launch_bounds__(kThreads2, 1) k_tree_rowfft_power(const TreePa
             for (int part = 0; part < p.n_parts; part++) tot += p.sumsq[((size_t)slot * NNODE + 2 * tid + h) * p.n_parts + part];
         const int k = 1 + blk.tb * NIMG + tid;         // fluctuation-frequency bin of this image
         const bool valid = k <= blk.nsearch / 2 && tot > 0.f;      // nsearch = NT of this DM
+        if (k <= blk.nsearch / 2 && p.cand_count != nullptr) atomicAdd(&p.counters[1], 1);   // frequency images searched
         sValid[2 * tid] = valid ? 1 : 0;
         sMean[2 * tid] = tot;
         sA[2 * tid] = valid ? (float)p.nbins / (kPowerRange * tot) : 0.f;
@@ -813,7 +811,7 @@ __global__ void __launch_bounds__(kThreads2, 1) k_tree_rowfft_power(const TreePa
             c.peak = peak; c.sigma = sigma; c.snr = snr;
             if (overflow) atomicAdd(&p.counters[0], 1);
             if (report_zero) *p.stats_out = c;
-            if (p.cand_count != nullptr && sValid[si] && snr >= p.threshold) {
+            if (p.cand_count != nullptr && sValid[si] && sigma > 0.f && snr >= p.threshold) {
                 int idx = atomicAdd(p.cand_count, 1);
                 if (idx < p.cand_capacity) p.cand_items[idx] = c;
             }

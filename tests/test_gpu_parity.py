@@ -5,6 +5,7 @@ import numpy as np
 import pytest
 
 import oracle as O
+import oracle_pool as OP
 import workloads as W
 import workloads.generate  # noqa: F401
 
@@ -142,10 +143,103 @@ def _transient_keys(cfg, delays, dms, max_keys=12):
     return keys[:max_keys]
 
 
-@pytest.mark.parametrize("name,nsample", [("lband", 10), ("sband", 3), ("hires", 1)])
-def test_full_size_sampled_parity(name, nsample):
-    """BASELINE.json configs 2-4 at full size, in the launch configuration bench.py times:
-    whole rf_search, then sampled images (random + at the injected transients) against the oracle."""
+def _check_list_against_stats(gpu, stats, cfg, thr):
+    """The WHOLE rf_search list against per-image oracle statistics: for every key the oracle evaluated, membership
+    (away from the threshold, A11), S/N <= 1e-3, peak <= 1e-4, sigma <= 1e-3, peak pixel (A20)."""
+    g = {(int(c["dm_idx"]), int(c["dt_idx"]), int(c["t_idx"])): c for c in gpu}
+    assert len(g) == len(gpu), "duplicate candidate keys"
+    worst, n_in, n_near = 0.0, 0, 0
+    for key, st in stats.items():
+        peak, y, x, sigma, snr = st[:5]
+        near = abs(snr - thr) <= NEAR_THR * thr
+        n_near += near
+        if not near:
+            assert (key in g) == (sigma > 0.0 and snr >= thr), (key, snr)
+        if key in g:
+            c = g[key]
+            n_in += 1
+            dev = abs(float(c["snr"]) - snr) / snr
+            worst = max(worst, dev)
+            assert dev <= SNR_TOL, (key, float(c["snr"]), snr)
+            assert abs(float(c["sigma"]) - sigma) <= SNR_TOL * sigma, key
+            assert abs(float(c["peak"]) - peak) <= 1e-4 * abs(peak) + 1e-7, key
+            assert OP.peak_pixel_ok(int(c["l_pix"]), int(c["m_pix"]), st, cfg.npix), (key, st)
+    return g, worst, n_in, n_near
+
+
+def test_lband_full_parity():
+    """BASELINE.json configs[1] IN FULL ("C2 ... run in full"): the statistics of all 85,404
+    (dm, dt, j) images from the float64 oracle on the host cores, then the whole rf_search candidate list
+    against them -- key set equal away from 2e-3 thr, S/N, sigma, peak and peak pixel of every candidate.
+    Method: thresholding each image; loops of Fig. 2."""
+    torch = _torch()
+    cfg = W.get_config("lband")
+    plan, f, uvw, cell = _plan_for(cfg)
+    dms = W.dm_list(cfg)
+    vis = W.make_segment(cfg)
+    dvis = torch.from_numpy(vis).cuda()
+    gpu, n = plan.search(dvis, capacity=1 << 18)
+    ctr = plan.get_counters()
+    delays = O.delay_table(f, dms, cfg.inttime_s)
+    keys = OP.all_keys(delays, cfg.nint, cfg.dt_list)
+    assert len(keys) == 85404                                       # SURVEY.md section 8 table
+    assert ctr["images"] == len(keys), "device-counted images"      # one atomic count per finalised image
+    assert n == len(gpu) and ctr["stats_overflow"] == 0
+    stats = OP.oracle_stats(vis, f, uvw, cfg.inttime_s, cfg.npix, cell, dms, cfg.dt_list, keys)
+    assert len(stats) == len(keys)
+    g, worst, n_in, n_near = _check_list_against_stats(gpu, stats, cfg, cfg.threshold)
+    assert set(g) <= set(stats)                                     # no candidate outside the loop
+    n_or = sum(1 for st in stats.values() if st[3] > 0 and st[4] >= cfg.threshold)
+    assert abs(len(g) - n_or) <= n_near
+    print(f"L-band full parity: {len(keys)} images, {len(g)} GPU candidates / {n_or} oracle, {n_near} within "
+          f"2e-3 of the threshold, worst relative S/N deviation {worst:.2e}")
+    # pixel parity through the debug hook: at the injected transients and on images of every width
+    iu, iv, keep = O.cell_table(uvw, f, cfg.npix, cell)
+    for (d, k, j) in _transient_keys(cfg, delays, dms, 10) + _stratified_keys(cfg, delays, 3, 7):
+        ref = O.search_image(vis, delays, iu, iv, keep, cfg.npix, d, cfg.dt_list[k], j)
+        img, st = plan.debug_image(dvis, d, k, j)
+        assert np.abs(img - ref).max() <= PIX_TOL * np.sqrt((ref ** 2).mean()), (d, k, j)
+        assert abs(float(st["snr"]) - stats[(d, k, j)][4]) <= SNR_TOL * stats[(d, k, j)][4], (d, k, j)
+    plan.destroy()
+
+
+def _stratified_keys(cfg, delays, per_dt, seed):
+    """per_dt images per width, drawn uniformly over (dm, j) of that width."""
+    rng = np.random.default_rng(seed)
+    keys = set()
+    for k, dt in enumerate(cfg.dt_list):
+        got = set()
+        while len(got) < per_dt:
+            d = int(rng.integers(cfg.ndm))
+            nj = O.n_images(cfg.nint, int(delays[d].max()), dt)
+            if nj > 0:
+                got.add((d, k, int(rng.integers(nj))))
+        keys |= got
+    return sorted(keys)
+
+
+def _neighbourhood_keys(cfg, delays, dms, ddm=2, dt_native=16):
+    """Every image within +-ddm DM trials / +-dt_native native integrations of each injected transient
+    (SURVEY.md 8(d)), for every width."""
+    keys = set()
+    for src in W.transients(cfg):
+        d0 = int(np.argmin(np.abs(dms - src.dm)))
+        for d in range(max(0, d0 - ddm), min(cfg.ndm, d0 + ddm + 1)):
+            md = int(delays[d].max())
+            for k, dt in enumerate(cfg.dt_list):
+                nj = O.n_images(cfg.nint, md, dt)
+                for j in range(max(0, (src.t0 - dt_native) // dt), min(nj, (src.t0 + dt_native) // dt + 1)):
+                    keys.add((d, k, j))
+    return sorted(keys)
+
+
+@pytest.mark.parametrize("name,per_dt,npixel", [("sband", 52, 10), ("hires", 32, 4)])
+def test_full_size_stratified_parity(name, per_dt, npixel):
+    """BASELINE.json configs[2], [3] at full size, in the launch configuration bench.py times: whole rf_search, then
+    >= 256 (S-band: 52 per width x 5) / >= 32 per width (hi-res) images drawn uniformly PER WIDTH plus every image
+    within +-2 DM trials / +-16 native integrations of each injected transient: S/N and list
+    membership on all of them, pixels on a subset.  Widths off the boxcar tree (S-band dt = 16) go through the same
+    phase-decimated path in rf_debug_image as in rf_search (B7)."""
     torch = _torch()
     cfg = W.get_config(name)
     w = W.chan_weights(cfg) if cfg.n_flagged else None
@@ -153,34 +247,36 @@ def test_full_size_sampled_parity(name, nsample):
     dms = W.dm_list(cfg)
     vis = W.make_segment(cfg)
     dvis = torch.from_numpy(vis).cuda()
-    gpu, n = plan.search(dvis, capacity=1 << 18)
+    gpu, n = plan.search(dvis, capacity=1 << 19)
     ctr = plan.get_counters()
-    assert ctr["images"] == plan.num_images() and n == len(gpu)
-    assert ctr["stats_overflow"] == 0
-    g = {(int(c["dm_idx"]), int(c["dt_idx"]), int(c["t_idx"])): c for c in gpu}
-    assert len(g) == len(gpu)
     delays = O.delay_table(f, dms, cfg.inttime_s)
+    total = sum(O.n_images(cfg.nint, int(delays[d].max()), dt) for d in range(cfg.ndm) for dt in cfg.dt_list)
+    assert ctr["images"] == total and n == len(gpu)                # device-counted images vs the oracle's loop
+    assert ctr["stats_overflow"] == 0
+    uniform = _stratified_keys(cfg, delays, per_dt, 7)
+    near = _neighbourhood_keys(cfg, delays, dms)
+    keys = sorted(set(uniform) | set(near))
+    stats = OP.oracle_stats(vis, f, uvw, cfg.inttime_s, cfg.npix, cell, dms, cfg.dt_list, keys, chan_weights=w,
+                            max_procs=16 if cfg.npix <= 1024 else 8)
+    g, worst, n_in, n_near = _check_list_against_stats(gpu, stats, cfg, cfg.threshold)
+    assert n_in >= len(W.transients(cfg)), "injected transients not recovered"
+    for c in gpu:                                                   # list-wide properties
+        k = int(c["dt_idx"])
+        assert 0 <= int(c["dm_idx"]) < cfg.ndm and 0 <= k < len(cfg.dt_list)
+        assert 0 <= int(c["t_idx"]) < O.n_images(cfg.nint, int(delays[int(c["dm_idx"])].max()), cfg.dt_list[k])
+        assert float(c["sigma"]) > 0 and float(c["snr"]) >= cfg.threshold
+    print(f"{name}: {len(keys)} oracle images ({len(uniform)} uniform, {len(near)} near transients), {n_in} of them "
+          f"candidates, {n_near} within 2e-3 of the threshold, worst relative S/N deviation {worst:.2e}")
+    # pixels and per-image statistics through the debug hook: one image per width at a transient + random ones
     iu, iv, keep = O.cell_table(uvw, f, cfg.npix, cell, w)
-    keys = _transient_keys(cfg, delays, dms, 3 if name != "lband" else 10) + _sample_keys(cfg, delays, nsample, 7)
-    n_w = int(keep.sum())
-    found = 0
-    for (d, k, j) in keys:
-        s = O.dedisperse_resample(vis, delays[d], cfg.dt_list[k], j)
-        ref = O.image_from_grid(O.grid_visibilities(s, iu, iv, keep, cfg.npix), n_w)
-        peak, y, x, sigma, snr = O.image_stats(ref)
+    src = W.transients(cfg)[0]
+    d0 = int(np.argmin(np.abs(dms - src.dm)))
+    sub = [(d0, k, src.t0 // dt) for k, dt in enumerate(cfg.dt_list)] + uniform[:: max(1, len(uniform) // npixel)][:npixel]
+    for (d, k, j) in sub:
+        ref = O.search_image(vis, delays, iu, iv, keep, cfg.npix, d, cfg.dt_list[k], j)
         img, st = plan.debug_image(dvis, d, k, j)
-        rms = np.sqrt((ref ** 2).mean())
-        assert np.abs(img - ref).max() <= PIX_TOL * rms, (d, k, j)
-        assert abs(float(st["snr"]) - snr) <= SNR_TOL * snr, (d, k, j)
-        in_list = (d, k, j) in g
-        if abs(snr - cfg.threshold) > NEAR_THR * cfg.threshold:
-            assert in_list == (snr >= cfg.threshold), (d, k, j, snr)
-        if in_list:
-            found += 1
-            c = g[(d, k, j)]
-            assert abs(float(c["snr"]) - snr) <= SNR_TOL * snr
-            assert (int(c["l_pix"]) % cfg.npix, int(c["m_pix"]) % cfg.npix) == (x, y)
-    assert found >= 1, "no injected transient was recovered"
+        assert np.abs(img - ref).max() <= PIX_TOL * np.sqrt((ref ** 2).mean()), (d, k, j)
+        assert abs(float(st["snr"]) - stats[(d, k, j)][4]) <= SNR_TOL * stats[(d, k, j)][4], (d, k, j)
     plan.destroy()
 
 
@@ -206,7 +302,7 @@ def test_streaming_segments():
         vis = W.make_segment(cfg, seg)
         dvis = torch.from_numpy(vis).cuda()
         gpu, n = plan.search(dvis, capacity=1 << 17)
-        assert n == len(gpu) and plan.get_counters()["images"] == 48000
+        assert n == len(gpu) and plan.get_counters()["images"] == 48000         # counted on the device
         for k, dt in enumerate(cfg.dt_list):
             sel = gpu[gpu["dt_idx"] == k]
             assert (sel["t_idx"] < cfg.stride_int // dt).all()

@@ -168,3 +168,29 @@ def test_lband_full_size_sampled():
                 assert (dm_idx, k) not in g
     assert found_harmonic                                            # the pulse train is seen at its DM and pixel
     plan.destroy()
+
+
+def test_periodic_npix_2048_tb4():
+    """The power variant of the row pass at npix 2048 with TB = 4 (512 threads, TB/2 32-bit histograms of 4096
+    bins): its shared memory must fit the 227 KB opt-in limit (sized per power image, not per tree node)."""
+    import torch
+    import paper_1802_03084_b200 as R
+    cfg = W.get_config("tiny")
+    npix, nint, dts = 2048, 70, (1, 2, 4)
+    f, uvw = W.channel_freqs_hz(cfg), W.baseline_uvw_m(cfg)
+    cell = W.default_cell_rad(cfg, uvw) * 64 / npix * 0.8
+    dms = np.array([0.0, 20.0])
+    vis = _rand_vis((nint, cfg.nbl, cfg.nchan, 2), 2050)
+    vis = _pulse_train(vis, f, uvw, cfg.inttime_s, cell, 0.5, 200, -310, 20.0, 8, 3)
+    plan = R.Plan(f, uvw, 2, nint, cfg.inttime_s, npix, cell, dms, dts, 0.0)
+    d = torch.from_numpy(vis).cuda()
+    gpu, n = plan.search_periodic(d, capacity=1 << 10)
+    assert n == len(gpu) == 64 == plan.get_counters()["images"]      # 2 trials x NT/2 = 32 frequency images
+    keys = [(0, 1), (1, 8), (1, 32), (0, 17)]
+    ref, stats = O.periodicity_search(vis, f, uvw, cfg.inttime_s, npix, cell, dms, 0.0, keys=keys, return_all_stats=True)
+    g = {(int(c["dm_idx"]), int(c["t_idx"])): c for c in gpu}
+    for key in keys:
+        amp, y, x, sigma, snr = stats[key]
+        assert abs(float(g[key]["snr"]) - snr) <= SNR_TOL * snr, key
+        assert (int(g[key]["l_pix"]) % npix, int(g[key]["m_pix"]) % npix) == (x, y), key
+    plan.destroy()
