@@ -165,7 +165,9 @@ int launch_tree(rf_plan* p, const TreeParams& tp, cudaStream_t st) {
     }
     {
         constexpr int NT2 = tree2_threads<N>();
-        auto kern = k_tree_rowfft_stats<N, TB, NT2>;
+        // half planes within 6/16 of the row (always, with the default cell: |u| <= N/3, A13) take the pruned transform
+        const bool zm = tp.ncol <= 6 * FftCfg<N>::TPF;
+        auto kern = zm ? k_tree_rowfft_stats<N, TB, NT2, true> : k_tree_rowfft_stats<N, TB, NT2, false>;
         const size_t smem = smem_tree2<N, TB>(tp.nbins, tp.cpad, NT2);
         { const int rc_a = ensure_smem_attr(p, (const void*)kern, smem); if (rc_a != RF_OK) return rc_a; }
         kern<<<dim3(tp.n_blk), NT2, smem, st>>>(tp);

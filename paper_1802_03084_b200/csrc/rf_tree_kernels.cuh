@@ -342,15 +342,18 @@ __global__ void __launch_bounds__(NTH) k_tree_colfft(const TreeParams p) {
 // Tree pass 2.  grid = (n_blk); block = 256; one CTA = all rows of one block.  Dynamic smem:
 //   xbuf [G2][XB] float2 (reused after the row loop for the unpacked histogram + prefix sums)
 //   | tw | hist [NW][nbins] u32, two images per word (16 bits each) | per-image parameters
+// bins per unit of the saturated coordinate y in [0, 1]: y = 1 must still land in bin nbins - 1
+__host__ __device__ __forceinline__ float hist_scale(int nbins) { return (float)nbins - 0.015625f; }
+
 template <int TPF>
 struct TreeStatsCtx {
     uint32_t* hist;
-    const float* sA;        // bin = x * A + B
+    const float* sA;        // bin = floor(S * sat(x * A + B)): A = 1 / (histogram range in units of x)
     const float* sScale;    // pixel = x * scale
     const int* sValid;
     float* sBest;           // [warp][NIMG]
     int* sBpos;
-    float B;
+    float B, S;             // B = 0.5 (range centred on 0) or 0 (range starts at 0); S = hist_scale(nbins)
     int nbins, nimg;
     bool wide;              // one 32-bit counter per bin and image (N >= 2048) instead of two packed 16-bit ones
 };
@@ -365,18 +368,18 @@ __device__ __forceinline__ void tree_row_stats(const float (&x)[16], int img, in
     uint32_t hw = (uint32_t)__cvta_generic_to_shared(cx.hist) + (uint32_t)((cx.wide ? img : (img >> 1)) * cx.nbins) * 4u;
     asm volatile("" : "+r"(hw));          // keep the sum in a register (the compiler re-forms it per pixel otherwise)
     const uint32_t inc = (!cx.wide && (img & 1)) ? 65536u : 1u;
-    // bin = clamp(floor(x * A + B), 0, nbins - 1) without a float -> int conversion: one FMA rounded DOWN onto
-    // 1.5 * 2^23 (ulp 1) leaves floor(x * A + B) in the low mantissa bits; B = nbins / 2 is an integer, so the addend
-    // is exact.  As SIGNED integers the bit patterns are ordered like the values (anything below -2^22 bins, incl.
-    // negative floats, clamps to bin 0; +inf clamps to the top), so one 3-input min/max clamps both ends.
+    // bin = floor(S * clamp(x * A + B, 0, 1)) with S = nbins - 2^-6, in two FMA-pipe instructions and no integer
+    // clamp: FFMA.SAT maps the histogram range onto [0, 1] (NaN -> 0, +-inf -> the end bins), then one FMA rounded
+    // DOWN onto 1.5 * 2^23 (ulp 1) leaves floor(y * S) <= nbins - 1 in the low mantissa bits (no F2I: that runs on
+    // the quarter-rate XU pipe).  Per pixel and image: FFMA.SAT, FFMA.RM, LEA, ATOMS and a third of an FMNMX3.
     constexpr int kMagicBits = 0x4B400000;                  // 12582912.0f
-    const float Bm = cx.B + 12582912.0f;
-    const int top = kMagicBits + cx.nbins - 1;
+    const float S = cx.S;
     hw -= (uint32_t)kMagicBits * 4u;                        // wraps; undone by the scaled add below
     float m = x[0];
 #pragma unroll
     for (int e = 0; e < 16; e++) {
-        const int q = min(max(__float_as_int(__fmaf_rd(x[e], A, Bm)), kMagicBits), top);
+        const float yv = __saturatef(fmaf(x[e], A, cx.B));
+        const int q = __float_as_int(__fmaf_rd(yv, S, 12582912.0f));
         asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(hw + (uint32_t)q * 4u), "r"(inc) : "memory");
         m = fmaxf(m, x[e]);
     }
@@ -404,21 +407,42 @@ __device__ __forceinline__ void tree_row_stats(const float (&x)[16], int img, in
     }
 }
 
-// 16-byte asynchronous global -> shared copy (LDGSTS): no register staging, no scoreboard wait
-__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
-    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gsrc) : "memory");
+// ---- bulk asynchronous copy (TMA, 1-D) completed on an mbarrier: one elected thread moves a whole contiguous
+// (row, pair) of the half plane (ncol x 16 bytes) global -> shared; no per-thread copy instructions, no register
+// staging, the consumers sleep on the barrier's phase bit (SASS: UBLKCP + SYNCS).
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void mbar_fence_init() {       // make the initialised barriers visible to the async proxy
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_copy_g2s(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(smem_dst)), "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    uint32_t done;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    } while (!done);
+}
+constexpr int kMaxRowGroups = 32;       // transform groups per row-pass CTA (one mbarrier each)
 
 constexpr int kThreads2 = 512;          // tree pass 2: one CTA of 16 warps per SM
 constexpr int kWarps2 = kThreads2 / 32;
 
 // NT2 = threads per CTA: 512 (one CTA per SM) up to N = 1024; 256 for N >= 2048, where one transform already
 // needs 128 or 256 threads and two or three smaller CTAs per SM hide its barriers better than one large one.
-template <int N, int TB, int NT2>
-__global__ void __launch_bounds__(NT2, NT2 == 512 ? 1 : 2) k_tree_rowfft_stats(const TreeParams p) {
+// ZM: the half plane occupies at most 6 N/16 columns (ncol <= 6 TPF; always true with the default cell, A13), so
+// elements 6 TPF .. 10 TPF - 1 of every row spectrum are zero: not staged into registers, pruned from the first stage.
+template <int N, int TB, int NT2, bool ZM>
+__global__ void __launch_bounds__(NT2, N >= 2048 ? 2 : 1) k_tree_rowfft_stats(const TreeParams p) {
     constexpr int NWP = NT2 / 32;
     using C = FftCfg<N>;
     constexpr int G2 = NT2 / C::TPF;
@@ -450,13 +474,20 @@ __global__ void __launch_bounds__(NT2, NT2 == 512 ? 1 : 2) k_tree_rowfft_stats(c
     const int grp = tid / C::TPF, t = tid % C::TPF;
     float4* sg = stg + (size_t)grp * p.cpad;
 
-    // stage (row y, pair p2): ncol contiguous 16-byte (H_a, H_b) entries, copied asynchronously
+    __shared__ __align__(8) uint64_t mbar[kMaxRowGroups];
+    // stage (row y, pair p2): ncol contiguous 16-byte (H_a, H_b) entries = ONE bulk copy issued by the group's first thread
     auto stage = [&](int y, int p2) {
         const float4* src = reinterpret_cast<const float4*>(Hblk + ((size_t)y * (TB / 2) + p2) * p.cpad * 2);
-        for (int c = t; c < p.ncol; c += C::TPF) cp_async16(sg + c, src + c);
-        cp_async_commit();
+        if (t == 0) {
+            mbar_arrive_expect_tx(&mbar[grp], (uint32_t)p.ncol * 16u);
+            bulk_copy_g2s(sg, src, (uint32_t)p.ncol * 16u, &mbar[grp]);
+        }
     };
+    if (tid < kMaxRowGroups) mbar_init(&mbar[tid], 1);
+    mbar_fence_init();
+    __syncthreads();
     stage(grp, 0);
+    uint32_t phase = 0;
 
     for (int i = tid; i < NW * p.nbins; i += NT2) hist[i] = 0u;
     load_twiddles<N>(tw, p.twiddles, tid, NT2);
@@ -475,11 +506,11 @@ __global__ void __launch_bounds__(NT2, NT2 == 512 ? 1 : 2) k_tree_rowfft_stats(c
         sValid[tid] = valid ? 1 : 0;
         sSig[tid] = sig;
         sScale[tid] = 1.f / (float)dt;
-        sA[tid] = valid ? (float)p.nbins / (2.f * kHistRange * sig) / (float)dt : 0.f;
+        sA[tid] = valid ? 1.f / (2.f * kHistRange * sig) / (float)dt : 0.f;     // x is the SUM of dt integrations
     }
     __syncthreads();
 
-    TreeStatsCtx<C::TPF> cx{hist, sA, sScale, sValid, sBest, sBpos, 0.5f * (float)p.nbins, p.nbins, NIMG, WIDE};
+    TreeStatsCtx<C::TPF> cx{hist, sA, sScale, sValid, sBest, sBpos, 0.5f, hist_scale(p.nbins), p.nbins, NIMG, WIDE};
     float2* xb = xbuf + grp * XB;
     const bool dbg = p.image_out != nullptr && slot == p.dbg_slot;
 
@@ -488,10 +519,11 @@ __global__ void __launch_bounds__(NT2, NT2 == 512 ? 1 : 2) k_tree_rowfft_stats(c
 #pragma unroll 1
         for (int p2 = 0; p2 < TB / 2; p2++) {
             float2 v[16];
-            cp_async_wait_all();
-            fft_group_sync<C::TPF>(1 + grp);                     // every lane's copies have landed
+            mbar_wait(&mbar[grp], phase);                        // the (row, pair) has landed
+            phase ^= 1u;
 #pragma unroll
             for (int e = 0; e < 16; e++) {
+                if (ZM && e >= 6 && e <= 9) { v[e] = make_float2(0.f, 0.f); continue; }
                 const int c = t + C::TPF * e;
                 const int cc = (e < 8) ? c : N - c;
                 float4 h = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -506,7 +538,7 @@ __global__ void __launch_bounds__(NT2, NT2 == 512 ? 1 : 2) k_tree_rowfft_stats(c
                 const int ny = (p2 + 1 == TB / 2) ? y + G2 : y;
                 if (ny < N) stage(ny, np2);
             }
-            fft_inverse<N>(v, xb, tw, t, 1 + grp);
+            fft_inverse<N, ZM>(v, xb, tw, t, 1 + grp);
             float a[16], s2[16];
 #pragma unroll
             for (int e = 0; e < 16; e++) a[e] = v[e].x;
@@ -551,9 +583,10 @@ __global__ void __launch_bounds__(NT2, NT2 == 512 ? 1 : 2) k_tree_rowfft_stats(c
         if (!sValid[img] && !report_zero) continue;            // block-uniform
         const uint32_t* hw = hist + (WIDE ? img : (img >> 1)) * p.nbins;
         const int sh = WIDE ? 0 : (img & 1) * 16;
-        const int per = p.nbins / NT2;
+        const int per = (p.nbins + NT2 - 1) / NT2;                 // bins [tid * per, ...) of this thread (none past nbins)
+        const int nmine = max(0, min(per, p.nbins - tid * per));
         uint32_t local = 0;
-        for (int i = 0; i < per; i++) {
+        for (int i = 0; i < nmine; i++) {
             const uint32_t c = WIDE ? hw[tid * per + i] : (hw[tid * per + i] >> sh) & 0xffffu;
             hun[tid * per + i] = c;
             local += c;
@@ -569,7 +602,7 @@ __global__ void __launch_bounds__(NT2, NT2 == 512 ? 1 : 2) k_tree_rowfft_stats(c
         __syncthreads();
         uint32_t base = inc - local, total = 0;
         for (int w = 0; w < NWP; w++) { if (w < warp) base += wtot[w]; total += wtot[w]; }
-        for (int i = 0; i < per; i++) { cum[tid * per + i] = base; base += hun[tid * per + i]; }
+        for (int i = 0; i < nmine; i++) { cum[tid * per + i] = base; base += hun[tid * per + i]; }
         __syncthreads();
         if (warp == 0) {
             int overflow = 0;
@@ -577,7 +610,7 @@ __global__ void __launch_bounds__(NT2, NT2 == 512 ? 1 : 2) k_tree_rowfft_stats(c
             const float sig_rms = sSig[img];
             if (sValid[img]) {
                 if (total != (uint32_t)N * (uint32_t)N) overflow = 1;   // a 16-bit counter wrapped
-                HistView hv{hun, cum, p.nbins, -kHistRange * sig_rms, (float)p.nbins / (2.f * kHistRange * sig_rms)};
+                HistView hv{hun, cum, p.nbins, -kHistRange * sig_rms, hist_scale(p.nbins) / (2.f * kHistRange * sig_rms)};
                 sigma = robust_sigma_from_hist(hv, (float)N * (float)N, lane, &overflow);
             }
             if (lane == 0) {
@@ -694,12 +727,19 @@ __global__ void __launch_bounds__(kThreads2, 1) k_tree_rowfft_power(const TreePa
     const float2* Hblk = p.Ht + (size_t)slot * N * p.cpad * TB;
     const int grp = tid / C::TPF, t = tid % C::TPF;
     float4* sg = stg + (size_t)grp * p.cpad;
+    __shared__ __align__(8) uint64_t mbar[kMaxRowGroups];
     auto stage = [&](int y, int p2) {
         const float4* src = reinterpret_cast<const float4*>(Hblk + ((size_t)y * (TB / 2) + p2) * p.cpad * 2);
-        for (int c = t; c < p.ncol; c += C::TPF) cp_async16(sg + c, src + c);
-        cp_async_commit();
+        if (t == 0) {
+            mbar_arrive_expect_tx(&mbar[grp], (uint32_t)p.ncol * 16u);
+            bulk_copy_g2s(sg, src, (uint32_t)p.ncol * 16u, &mbar[grp]);
+        }
     };
+    if (tid < kMaxRowGroups) mbar_init(&mbar[tid], 1);
+    mbar_fence_init();
+    __syncthreads();
     stage(grp, 0);
+    uint32_t phase = 0;
     for (int i = tid; i < NIMG * p.nbins; i += kThreads2) hist[i] = 0u;
     load_twiddles<N>(tw, p.twiddles, tid, kThreads2);
     for (int i = tid; i < kWarps2 * NSL; i += kThreads2) { sBest[i] = -CUDART_INF_F; sBpos[i] = 0; }
@@ -714,19 +754,19 @@ __global__ void __launch_bounds__(kThreads2, 1) k_tree_rowfft_power(const TreePa
         if (k <= blk.nsearch / 2 && p.cand_count != nullptr) atomicAdd(&p.counters[1], 1);   // frequency images searched
         sValid[2 * tid] = valid ? 1 : 0;
         sMean[2 * tid] = tot;
-        sA[2 * tid] = valid ? (float)p.nbins / (kPowerRange * tot) : 0.f;
+        sA[2 * tid] = valid ? 1.f / (kPowerRange * tot) : 0.f;
     }
     __syncthreads();
 
-    TreeStatsCtx<C::TPF> cx{hist, sA, sScale, sValid, sBest, sBpos, 0.f, p.nbins, NSL, false};
+    TreeStatsCtx<C::TPF> cx{hist, sA, sScale, sValid, sBest, sBpos, 0.f, hist_scale(p.nbins), p.nbins, NSL, false};
     float2* xb = xbuf + grp * XB;
     const bool dbg = p.image_out != nullptr && slot == p.dbg_slot;
     for (int y = grp; y < N; y += G2) {
 #pragma unroll 1
         for (int p2 = 0; p2 < TB / 2; p2++) {
             float2 v[16];
-            cp_async_wait_all();
-            fft_group_sync<C::TPF>(1 + grp);
+            mbar_wait(&mbar[grp], phase);
+            phase ^= 1u;
 #pragma unroll
             for (int e = 0; e < 16; e++) {
                 const int c = t + C::TPF * e;
@@ -789,7 +829,7 @@ __global__ void __launch_bounds__(kThreads2, 1) k_tree_rowfft_power(const TreePa
                     if ((float)cum[mid] <= target) lo_b = mid; else hi_b = mid - 1;
                 }
                 const float hb = (float)hun[lo_b];
-                const float w = kPowerRange * sMean[si] / (float)p.nbins;
+                const float w = kPowerRange * sMean[si] / hist_scale(p.nbins);
                 const float med = ((float)lo_b + (hb > 0.f ? (target - (float)cum[lo_b]) / hb : 0.5f)) * w;
                 if (lo_b == p.nbins - 1) overflow = 1;           // median beyond the histogram range
                 sigma = sqrtf(med / 0.6931471805599453f);
