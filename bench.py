@@ -86,17 +86,47 @@ def _setup(cfg, segment=0):
 
 def _alg_bytes(cfg, plan):
     """A_img = 16 N_bl N_chan,w dt + 16 N_pix^2 per image, split per kernel kind
-    (rf_plan_get_kernel_times): the visibility read belongs to the kernel that gathers (kind 3 for the
-    widths on the boxcar tree, kind 0 for the per-image path), the hand-off write (8 N^2) to the column
-    FFT (kind 0), the hand-off read (8 N^2) to the row FFT + statistics (kind 1)."""
+    (rf_plan_get_kernel_times): the visibility read belongs to the kernel that gathers (kind 3 `k_tree_gather` for every
+    width of a plan on the boxcar-tree kernels, npix >= 256: the widths on the tree and, through their phase-decimated
+    sums, the widths off it; kind 0 `k_grid_colfft` for npix < 256), the hand-off write (8 N^2) to the column FFT
+    (kind 0), the hand-off read (8 N^2) to the row FFT + statistics (kind 1)."""
     c = plan.get_counters()
-    images = c["images"]
-    tree = [k for k, dt in enumerate(cfg.dt_list) if dt in (1, 2, 4, 8) and 256 <= cfg.npix <= 1024]
-    vis_tree = sum(16.0 * plan.num_t(d, k) * cfg.dt_list[k] * c["n_kept"] for d in range(cfg.ndm) for k in tree)
+    images = plan.num_images()
     vis_bytes = 16.0 * c["vis_gridded"]                     # 16 B per (bl, ch) pol pair per native sample
+    vis_tree = vis_bytes if cfg.npix >= 256 else 0.0
     hand = 8.0 * cfg.npix * cfg.npix * images
     return {"total": vis_bytes + 2 * hand, "kind": [vis_bytes - vis_tree + hand, hand, 0.0, vis_tree],
-            "images": images, "vis_gridded": c["vis_gridded"]}
+            "images": images, "images_device_counted": c["images"], "vis_gridded": c["vis_gridded"]}
+
+
+FP32_LANES_PER_SM, N_SM = 128, 148          # B200: fp32 FMA peak = SMs x lanes x 2 flop x SM clock (B200_PROFILING.md)
+
+
+def _fft_rate(cfg, plan, k_ms, sm_mhz):
+    """Secondary evidence of SURVEY.md 8(d): FFT rate under the 5 N log2 N convention, counting only the transforms
+    the kernels actually run (rf_plan_fft_work), per pass against the time of the kernel that holds it, and against
+    the fp32 FMA peak at the SM clock seen during the run.  The 2-D FFT is the paper's dominant stage."""
+    n_col, n_row = plan.fft_work()
+    per = 5.0 * cfg.npix * np.log2(cfg.npix)
+    peak = N_SM * FP32_LANES_PER_SM * 2 * (sm_mhz or 1965) * 1e6 / 1e12
+    col = n_col * per / (k_ms[0] * 1e-3) / 1e12 if k_ms[0] > 0 else 0.0
+    row = n_row * per / (k_ms[1] * 1e-3) / 1e12 if k_ms[1] > 0 else 0.0
+    tot = (n_col + n_row) * per / ((k_ms[0] + k_ms[1]) * 1e-3) / 1e12 if k_ms[0] + k_ms[1] > 0 else 0.0
+    return {"convention": "5 N log2 N per N-point complex transform actually run", "column_transforms": n_col,
+            "row_pair_transforms": n_row, "flop_per_step": (n_col + n_row) * per, "column_pass_tflops": col,
+            "row_pass_tflops": row, "both_passes_tflops": tot, "fp32_peak_tflops": peak, "frac_of_fp32_peak": tot / peak,
+            "note": "the row-pass kernel also holds the statistics, the column-pass kernel the scatter and the hand-off store"}
+
+
+def _cpu_model():
+    try:
+        with open("/proc/cpuinfo") as fh:
+            for line in fh:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
 
 
 KIND_NAMES = ["column FFT kernels (k_tree_colfft; k_grid_colfft on the per-image path)",
@@ -109,20 +139,31 @@ def _roofline(alg, k_ms, k_n, ms_per_step, traffic=None):
     peak, peak_src = _peaks()
     dom = max((0, 1, 3), key=lambda k: k_ms[k])
     per_launch_bytes = alg["kind"][dom] / max(1, k_n[dom])
-    achieved = per_launch_bytes / (k_ms[dom] / max(1, k_n[dom]) * 1e-3) / 1e9
+    per_launch_s = k_ms[dom] / max(1, k_n[dom]) * 1e-3
+    achieved = per_launch_bytes / per_launch_s / 1e9
     path_gbs = alg["total"] / (ms_per_step * 1e-3) / 1e9
     names = ["pass1", "pass2", "prep", "gather"]
-    return {"bound": "hbm", "kernel": KIND_NAMES[dom], "achieved": achieved, "peak": peak, "unit": "GB/s",
-            "frac": achieved / peak, "traffic": traffic[dom] if traffic else None, "peak_source": peak_src,
-            "alg_bytes_per_launch": per_launch_bytes,
-            "kernel_ms_per_step": {n: k_ms[i] for i, n in enumerate(names)},
-            "kernel_launches_per_step": {n: k_n[i] for i, n in enumerate(names)},
-            "kernel_alg_gbs": {n: (alg["kind"][i] / (k_ms[i] * 1e-3) / 1e9 if k_ms[i] > 0 else 0.0)
-                               for i, n in enumerate(names)},
-            "path": {"alg_bytes_per_step": alg["total"], "achieved": path_gbs, "frac": path_gbs / peak,
-                     **_own_bytes(traffic, k_n, ms_per_step, peak)},
-            # what ncu says actually limits each kernel (the model bytes above are not what this design moves)
-            **({"limiters_ncu": traffic["limiters"]} if traffic and traffic.get("limiters") else {})}
+    out = {"bound": "hbm", "kernel": KIND_NAMES[dom], "achieved": achieved, "peak": peak, "unit": "GB/s",
+           "frac": achieved / peak, "traffic": traffic[dom] if traffic else None, "peak_source": peak_src,
+           "alg_bytes_per_launch": per_launch_bytes,
+           "kernel_ms_per_step": {n: k_ms[i] for i, n in enumerate(names)},
+           "kernel_launches_per_step": {n: k_n[i] for i, n in enumerate(names)},
+           "kernel_alg_gbs": {n: (alg["kind"][i] / (k_ms[i] * 1e-3) / 1e9 if k_ms[i] > 0 else 0.0)
+                              for i, n in enumerate(names)},
+           "path": {"alg_bytes_per_step": alg["total"], "achieved": path_gbs, "frac": path_gbs / peak,
+                    **_own_bytes(traffic, k_n, ms_per_step, peak)}}
+    if traffic and traffic.get(dom) is not None:
+        # the dominant kernel on the bytes it REALLY moves (ncu dram__bytes per launch / its live event time): the model
+        # fraction above exceeds 1 because this design avoids most of the model's bytes
+        own = traffic[dom] / per_launch_s / 1e9
+        out["own_bytes"] = {"achieved": own, "frac_own": own / peak,
+                            "note": "ncu DRAM bytes per launch / live CUDA-event time per launch / measured HBM peak"}
+        out["frac_own"] = own / peak
+        out["traffic_commit"] = traffic.get("commit")
+        out["traffic_source"] = traffic.get("source")
+    if traffic and traffic.get("limiters"):
+        out["limiters_ncu"] = traffic["limiters"]     # what ncu says actually limits each kernel
+    return out
 
 
 def _own_bytes(traffic, k_n, ms_per_step, peak):
@@ -219,22 +260,46 @@ def _ensure_built(local_rank: int) -> None:
         time.sleep(1.0)
 
 
-def run_ours(args, cfg):
-    import torch
-    import torch.distributed as dist
+class Ctx:
+    """Process-wide CUDA / torch.distributed state of one bench.py run."""
 
+    def __init__(self):
+        import torch
+        import torch.distributed as dist
+        self.torch, self.dist = torch, dist
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.local = int(os.environ.get("LOCAL_RANK", "0"))
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+        _ensure_built(self.local)
+        torch.cuda.set_device(self.local)
+        if self.world > 1:
+            dist.init_process_group("nccl", device_id=torch.device("cuda", self.local))
+        self.dev = torch.device("cuda", self.local)
+
+    def close(self):
+        if self.world > 1:
+            self.dist.destroy_process_group()
+
+
+def _traffic(cfg, args):
+    """ncu DRAM bytes per launch of the three tree kernels in this launch configuration: numbers only a profiler run
+    can provide, read from the committed capture (profiles/), which names the commit it was taken at."""
+    tpath = os.path.join(ROOT, "profiles", f"r2_traffic_{cfg.name}.json.txt")
+    if args.batch or args.tune or not os.path.exists(tpath):
+        return None
+    with open(tpath) as fh:
+        tj = json.load(fh)
+    return {0: tj.get("pass1_dram_bytes_per_launch"), 1: tj.get("pass2_dram_bytes_per_launch"),
+            3: tj.get("gather_dram_bytes_per_launch"), "limiters": tj.get("limiters"), "commit": tj.get("commit"),
+            "source": tj.get("source")}
+
+
+def measure(args, cfg, ctx):
+    """One config, device-resident and end to end; returns the JSON line as a dict on rank 0 (None elsewhere)."""
     import paper_1802_03084_b200 as R
-
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
-    _ensure_built(local)
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    dev = torch.device("cuda", local)
+    torch, dist, world, rank, local, dev = ctx.torch, ctx.dist, ctx.world, ctx.rank, ctx.local, ctx.dev
 
     f, uvw, dms, cell = _setup(cfg)
     # segment round-robin (PAPER.md:108): rank r searches the r-th consecutive segment of the observation
@@ -250,6 +315,8 @@ def run_ours(args, cfg):
         plan.set_batch(args.batch)
     if args.meansub:
         plan.set_meansub(True)
+    for knob, val in args.tune:
+        plan.set_tuning(knob, val)
     capacity = 1 << 17
     stream = torch.cuda.current_stream(dev)
     items = torch.empty(capacity * 32, dtype=torch.uint8, device=dev)
@@ -322,26 +389,26 @@ def run_ours(args, cfg):
 
     alg = _alg_bytes(cfg, plan)
     images = alg["images"]
+    if alg["images_device_counted"] != images:
+        raise SystemExit(f"the kernels finalised {alg['images_device_counted']} images, the plan lists {images}")
     ms_per_step = total_ms / args.steps
     value = world * images / (ms_per_step * 1e-3)
     e2e_value = world * images / (e2e_ms / args.steps * 1e-3)
 
+    line = None
     if rank == 0:
-        traffic = None
-        tpath = os.path.join(ROOT, "profiles", "r1_traffic_lband.json.txt")
-        if cfg.name == "lband" and not args.batch and os.path.exists(tpath):
-            with open(tpath) as fh:       # one ncu --set full capture of this launch configuration
-                tj = json.load(fh)
-            traffic = {0: tj.get("pass1_dram_bytes_per_launch"), 1: tj.get("pass2_dram_bytes_per_launch"),
-                       3: tj.get("gather_dram_bytes_per_launch"), "limiters": tj.get("limiters")}
+        label = (f"{cfg.name}: BASELINE.json configs[{cfg.index}] ({cfg.nant} antennas, {cfg.nchan} ch, {cfg.nint} x "
+                 f"{cfg.inttime_s * 1e3:g} ms, {cfg.ndm} DM x dt {list(cfg.dt_list)}, npix {cfg.npix})")
+        roof = _roofline(alg, k_ms, k_n, ms_per_step, _traffic(cfg, args))
+        roof["fft"] = _fft_rate(cfg, plan, k_ms, clocks.get("sm_mhz"))
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": f"{cfg.name}: BASELINE.json configs[{cfg.index}] ({cfg.nant} antennas, "
-                                   f"{cfg.nchan} ch, {cfg.nint} x {cfg.inttime_s * 1e3:g} ms, {cfg.ndm} DM x dt "
-                                   f"{list(cfg.dt_list)}, npix {cfg.npix})",
-                       "images_per_step": images, "gvis_per_s": world * alg["vis_gridded"] / (ms_per_step * 1e-3) / 1e9,
+            "config": {"workload": label,
+                       "images_per_step": images, "images_counted_on_device": alg["images_device_counted"],
+                       "gvis_per_s": world * alg["vis_gridded"] / (ms_per_step * 1e-3) / 1e9,
+                       "input_mvis_per_s": world * cfg.nint * cfg.nbl * cfg.nchan * cfg.npol / (ms_per_step * 1e-3) / 1e6,
                        "l2_policy": f"input segment {vis.nbytes / 1e9:.2f} GB is larger than L2 (126 MB); no flush",
                        "candidates": n_cands, "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
                        "prep": "mean-visibility subtraction fused into the readers" if args.meansub else "none"},
@@ -349,17 +416,18 @@ def run_ours(args, cfg):
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(vis.nbytes),
                     "d2h_bytes_per_step": int(4 + min(n_e2e, capacity) * 32)},
             "gpu_launches": int(launches) * args.steps,
-            "roofline": _roofline(alg, k_ms, k_n, ms_per_step, traffic),
+            "roofline": roof,
         }
         if periodic is not None:
             line["periodic"] = periodic
         if world == 1 and not args.no_cpu_baseline:
             v, cores, sample = oracle_throughput(cfg, vis, args.ref_images)
-            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
-        print(json.dumps(line), flush=True)
-    if world > 1:
-        dist.destroy_process_group()
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                                    "cpu": _cpu_model()}
     plan.destroy()
+    del dvis, hvis, items, count
+    torch.cuda.empty_cache()
+    return line
 
 
 def _stream_host_rows(cfg, nseg, torch):
@@ -395,7 +463,6 @@ def run_stream(args, cfg):
         raise SystemExit("--config stream is a single-GPU measurement (replicas: run one per GPU)")
     dev = torch.device("cuda", 0)
     torch.cuda.set_device(dev)
-    _ensure_built(0)
     nseg_cfg = cfg.n_segments
     n_warm, n_timed = args.warmup, args.steps
     n_total = n_warm + n_timed
@@ -408,7 +475,7 @@ def run_stream(args, cfg):
     overlap = cfg.nint - cfg.stride_int
 
     main, side = torch.cuda.Stream(dev), torch.cuda.Stream(dev)
-    capacity = 1 << 17
+    capacity = 1 << 19 if cfg.name == "stream1ms" else 1 << 17
     plans, bufs, items, counts, h_items, h_counts = [], [], [], [], [], []
     for b in range(2):
         pl = R.Plan(f, geo[0][0], cfg.npol, cfg.nint, cfg.inttime_s, cfg.npix, geo[0][1], dms, cfg.dt_list, cfg.threshold)
@@ -482,32 +549,61 @@ def run_stream(args, cfg):
     k_ms, k_n = plans[b].get_kernel_times()
     launches = plans[b].get_counters()["kernel_launches"]
     alg = _alg_bytes(cfg, plans[b])
+    if alg["images_device_counted"] != images:
+        raise SystemExit(f"the kernels finalised {alg['images_device_counted']} images, the plan lists {images}")
     ms_per_step = dev_ms / n_timed
     data_s = cfg.stride_int * cfg.inttime_s
     new_bytes = cfg.stride_int * cfg.nbl * cfg.nchan * cfg.npol * 8
+    if cfg.name == "stream1ms":
+        label = (f"stream1ms: the paper's GOAL workload (PAPER.md:94, Table 1 row L, PAPER.md:180: 1 ms sampling, 1.4 GB/s) on "
+                 f"the BASELINE.json configs[4] array and trial grid ({cfg.nant} antennas, {cfg.nchan} ch, segments of {cfg.nint} x 1 ms "
+                 f"with stride {cfg.stride_int} = 2.0 s, overlap = the DM 1000 sweep, {cfg.ndm} DM x dt {list(cfg.dt_list)}, npix "
+                 f"{cfg.npix}); a step = one segment, pipelined")
+    else:
+        label = (f"stream: BASELINE.json configs[4] ({cfg.nant} antennas, {cfg.nchan} ch, segments of {cfg.nint} x "
+                 f"{cfg.inttime_s * 1e3:g} ms with stride {cfg.stride_int}, {cfg.ndm} DM x dt {list(cfg.dt_list)}, npix {cfg.npix}); "
+                 f"a step = one segment, pipelined")
+    roof = _roofline(alg, k_ms, k_n, ms_per_step)
+    roof["fft"] = _fft_rate(cfg, plans[b], k_ms, clocks.get("sm_mhz"))
     line = {
         "metric": METRIC, "value": images / (ms_per_step * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": n_timed,
         "warmup": n_warm, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"stream: BASELINE.json configs[4] ({cfg.nant} antennas, {cfg.nchan} ch, segments of "
-                               f"{cfg.nint} x {cfg.inttime_s * 1e3:g} ms with stride {cfg.stride_int}, {cfg.ndm} DM x dt "
-                               f"{list(cfg.dt_list)}, npix {cfg.npix}); a step = one segment, pipelined",
-                   "images_per_step": images, "realtime_factor": data_s / (ms_per_step * 1e-3),
+        "config": {"workload": label,
+                   "images_per_step": images, "images_counted_on_device": alg["images_device_counted"],
+                   "realtime_factor": data_s / (ms_per_step * 1e-3),
                    "realtime_factor_wall": data_s * n_timed / (wall_ms * 1e-3),
-                   "data_seconds_per_step": data_s, "candidates_last_segment": n_last, "candidates_read_on_host": found[0],
+                   "data_seconds_per_step": data_s, "input_rate_gbs": new_bytes / data_s / 1e9,
+                   "h2d_gbs_sustained": new_bytes * n_timed / (wall_ms * 1e-3) / 1e9,
+                   "candidates_last_segment": n_last, "candidates_read_on_host": found[0],
                    "gvis_per_s": alg["vis_gridded"] / (ms_per_step * 1e-3) / 1e9,
-                   "l2_policy": "each segment's 1.47 GB buffer is larger than L2 (126 MB); no flush",
+                   "l2_policy": f"each segment's {bufs[0].numel() * 8 / 1e9:.2f} GB buffer is larger than L2 (126 MB); no flush",
                    "overlap": "H2D of the next segment's new integrations on a side stream; table rebuild on the host",
-                   "parallelism": "single GPU"},
+                   "parallelism": "single GPU; on more GPUs the split is by segment (replicas, PAPER.md:108), unmeasured on hardware"},
         "clocks": clocks,
         "e2e": {"value": images * n_timed / (wall_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(new_bytes),
                 "d2h_bytes_per_step": int(4 + capacity * 32)},
         "gpu_launches": int(launches) * n_timed,
-        "roofline": _roofline(alg, k_ms, k_n, ms_per_step),
+        "roofline": roof,
     }
-    print(json.dumps(line), flush=True)
     for pl in plans:
         pl.destroy()
+    del bufs, items, counts, first, new
+    torch.cuda.empty_cache()
+    return line
+
+
+def _brief(line):
+    """The part of another config's line that the default run carries as a sub-object."""
+    keep = ("value", "unit", "steps", "warmup", "ms_per_step", "clocks", "gpu_launches")
+    out = {k: line[k] for k in keep if k in line}
+    out["config"] = line["config"]
+    out["e2e"] = line["e2e"]
+    r = line["roofline"]
+    out["roofline"] = {"kernel_ms_per_step": r["kernel_ms_per_step"], "path_frac": r["path"]["frac"],
+                       "fft_both_passes_tflops": r["fft"]["both_passes_tflops"],
+                       "fft_frac_of_fp32_peak": r["fft"]["frac_of_fp32_peak"]}
+    return out
 
 
 def main():
@@ -516,22 +612,46 @@ def main():
     ap.add_argument("--steps", type=int, default=None, help="timed steps (default 5; 32 segments for --config stream)")
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="lband", choices=sorted(W.CONFIGS))
+    ap.add_argument("--config", default=None, choices=sorted(W.CONFIGS),
+                    help="default: lband (BASELINE.json configs[1]) plus hi-res and streaming as sub-objects")
+    ap.add_argument("--no-extra", action="store_true", help="default run without the hi-res / streaming sub-objects")
     ap.add_argument("--batch", type=int, default=0, help="images per batch (0 = library default)")
     ap.add_argument("--ref-images", type=int, default=512, help="oracle sample size per timing")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--periodic", action="store_true", help="also time rf_search_periodic (8f-3) on the same segment")
     ap.add_argument("--meansub", action="store_true", help="also run the prep stage (mean-visibility subtraction, 8f-1)")
+    ap.add_argument("--tune", action="append", default=[], metavar="KNOB=VALUE",
+                    help="rf_plan_set_tuning(knob, value) before the run (experiments; results do not change)")
     args = ap.parse_args()
-    cfg = W.get_config(args.config)
+    args.tune = [tuple(int(x) for x in t.split("=")) for t in args.tune]
+    default_run = args.config is None
+    cfg = W.get_config(args.config or "lband")
     if args.steps is None:
         args.steps = cfg.n_segments if cfg.n_segments > 1 else 5
     if args.impl == "reference":
         run_reference(args, cfg)
-    elif cfg.n_segments > 1:
-        run_stream(args, cfg)
+        return
+    ctx = Ctx()
+    if cfg.n_segments > 1:
+        line = run_stream(args, cfg)
     else:
-        run_ours(args, cfg)
+        line = measure(args, cfg, ctx)
+    if default_run and ctx.world == 1 and line is not None and not args.no_extra:
+        # the other BASELINE.json configs the metric names, as sub-objects with their own clocks: hi-res (configs[3])
+        # and the streaming real-time factor (configs[4]).  S-band (configs[2]) is left to `--config sband`: its
+        # 11.8 GB segment takes minutes to generate on the host.
+        import copy
+        extra = {}
+        a = copy.copy(args)
+        a.steps, a.warmup, a.no_cpu_baseline, a.periodic = 3, 3, True, False
+        extra["hires"] = _brief(measure(a, W.get_config("hires"), ctx))
+        a = copy.copy(args)
+        a.steps, a.warmup = W.get_config("stream").n_segments, 3
+        extra["stream"] = _brief(run_stream(a, W.get_config("stream")))
+        line["other_configs"] = extra
+    if line is not None:
+        print(json.dumps(line), flush=True)
+    ctx.close()
 
 
 if __name__ == "__main__":

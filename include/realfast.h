@@ -124,6 +124,12 @@ int rf_plan_get_tables(rf_plan* plan, int32_t* delay_host, int32_t* cell_host, u
 int64_t rf_plan_num_images(const rf_plan* plan);
 int     rf_plan_num_t(const rf_plan* plan, int dm_idx, int dt_idx);
 
+/* Work accounting for the FFT rate (SURVEY.md 8(d) "secondary evidence"; the 2-D FFT is the paper's dominant
+ * stage): the number of npix-point complex transforms ONE rf_search of this plan runs --
+ * column pass (one per occupied-half-plane column, padded, per gridded integration) and row pass (one per image
+ * row and PAIR of images: two real images share a complex transform).  Either pointer may be NULL.   */
+int rf_plan_fft_work(const rf_plan* plan, int64_t* col_transforms, int64_t* row_transforms);
+
 /* Pixel-parity hook: write the float32 image [npix][npix] (row y, column x, no
  * fftshift) of one (dm_idx, dt_idx, t_idx) to DEVICE memory, and optionally its
  * statistics (peak, sigma, snr as the search computes them) to a device rf_cand.
@@ -151,6 +157,7 @@ int rf_plan_set_batch(rf_plan* plan, int images_per_batch);
 #define RF_TUNE_DM_GROUP    2
 #define RF_TUNE_FEED_BATCH  3
 #define RF_TUNE_TREE_MAXPIX 4
+#define RF_TUNE_GATHER_ORDER 5  /* gather grid order: 1 (default) block pairs fastest, 0 cell ranges fastest      */
 int rf_plan_set_tuning(rf_plan* plan, int knob, int value);
 
 /* End-to-end convenience entry with HOST buffers: copies the segment host->device into a

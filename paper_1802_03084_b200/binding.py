@@ -23,8 +23,10 @@ EXPORTS = [
     "rf_search_host", "rf_plan_set_profiling", "rf_plan_get_kernel_times", "rf_plan_set_mode",
     "rf_plan_set_meansub", "rf_prep_meansub", "rf_cand_spectrum", "rf_inject",
     "rf_search_periodic", "rf_plan_periodic_nt", "rf_debug_periodic_image", "rf_plan_set_tuning",
+    "rf_plan_fft_work",
 ]
 RF_TUNE_AUX_WIDTHS, RF_TUNE_DM_GROUP, RF_TUNE_FEED_BATCH, RF_TUNE_TREE_MAXPIX = 1, 2, 3, 4
+RF_TUNE_GATHER_ORDER = 5
 
 # numpy view of rf_cand (32 bytes)
 CAND_DTYPE = np.dtype([("dm_idx", "<i4"), ("dt_idx", "<i4"), ("t_idx", "<i4"), ("l_pix", "<i4"),
@@ -73,6 +75,7 @@ def load_library() -> C.CDLL:
     lib.rf_plan_num_images.argtypes = [vp]
     lib.rf_plan_num_images.restype = C.c_int64
     lib.rf_plan_num_t.argtypes = [vp, C.c_int, C.c_int]
+    lib.rf_plan_fft_work.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     lib.rf_debug_image.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, vp, vp, vp]
     lib.rf_plan_get_counters.argtypes = [vp, C.POINTER(_Counters)]
     lib.rf_last_error.restype = C.c_char_p
@@ -170,6 +173,12 @@ class Plan:
 
     def num_t(self, dm_idx: int, dt_idx: int) -> int:
         return int(self._lib.rf_plan_num_t(self._h, dm_idx, dt_idx))
+
+    def fft_work(self):
+        """rf_plan_fft_work: (column transforms, row pair transforms) of npix points per rf_search."""
+        a, b = C.c_int64(0), C.c_int64(0)
+        _check(self._lib.rf_plan_fft_work(self._h, C.byref(a), C.byref(b)))
+        return a.value, b.value
 
     def get_counters(self) -> dict:
         c = _Counters()

@@ -47,7 +47,7 @@ void free_tables(rf_plan* p) {
     rf::DeviceTables& d = p->d;
     cudaFree(d.delay); cudaFree(d.cell); cudaFree(d.keep); cudaFree(d.gen.entries); cudaFree(d.gen.warp_chunk);
     cudaFree(d.tree.entries); cudaFree(d.tree.cells); cudaFree(d.tree.stream_iter); cudaFree(d.tree.stream_cell); cudaFree(d.tree.group_cell); cudaFree(d.blocks); cudaFree(d.blocks2);
-    for (uint2* e : d.aux_entries) cudaFree(e); cudaFree(d.images); cudaFree(d.freqs); cudaFree(d.uvw); cudaFree(d.dms); cudaFree(d.weights); cudaFree(d.twiddles);
+    for (uint2* e : d.aux_entries) cudaFree(e); cudaFree(d.images); cudaFree(d.freqs); cudaFree(d.uvw); cudaFree(d.dms); cudaFree(d.weights); cudaFree(d.twiddles); cudaFree(d.twp);
     p->dev_cap.clear();
     d = rf::DeviceTables{};
 }
@@ -267,6 +267,9 @@ int rf_plan_set_tuning(rf_plan* p, int knob, int value) {
             if (value < 0) { set_error("tree maxpix must be >= 0"); return RF_ERR_ARG; }
             p->tune_tree_maxpix = value;
             break;
+        case RF_TUNE_GATHER_ORDER:
+            p->tune_gather_order = value != 0;
+            return RF_OK;
         default: set_error("unknown tuning knob %d", knob); return RF_ERR_ARG;
     }
     rf::configure_tree(p);
@@ -282,6 +285,13 @@ int rf_plan_get_tables(rf_plan* p, int32_t* delay_host, int32_t* cell_host, uint
 }
 
 int64_t rf_plan_num_images(const rf_plan* p) { return p ? p->n_images : 0; }
+
+int rf_plan_fft_work(const rf_plan* p, int64_t* col_transforms, int64_t* row_transforms) {
+    if (!p) { set_error("null plan"); return RF_ERR_ARG; }
+    if (col_transforms) *col_transforms = p->n_col_fft;
+    if (row_transforms) *row_transforms = p->n_row_fft;
+    return RF_OK;
+}
 
 int rf_plan_num_t(const rf_plan* p, int dm_idx, int dt_idx) {
     if (!p || dm_idx < 0 || dm_idx >= p->ndm || dt_idx < 0 || dt_idx >= p->ndt) return RF_ERR_ARG;

@@ -26,6 +26,8 @@ __device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(
 // multiply by +i
 __device__ __forceinline__ float2 cmuli(float2 a) { return make_float2(-a.y, a.x); }
 
+constexpr int kTwpPitch = 15;                // row pitch of the stage-2 twiddle-power table [16][15] (odd: conflict-free)
+constexpr int kTwpSize = 16 * kTwpPitch;
 __host__ __device__ constexpr int fft_pad(int i) { return i + (i >> 4); }
 __host__ __device__ constexpr int fft_padded_size(int n) { return n + (n >> 4); }
 
@@ -170,9 +172,9 @@ template <int TPF> __device__ __forceinline__ void fft_group_sync(int bar_id) {
 // P = 16 or 256: r*P is a multiple of 16), so one padded base per butterfly plus a
 // compile-time stride replaces a shift and two adds per access:
 //   fft_pad(base + r*P) = fft_pad(base) + r * (P == 1 ? 1 : P + P/16).
-template <int N, int R, int P, bool LAST, bool ZMID = false>
+template <int N, int R, int P, bool LAST, bool ZMID = false, bool TWP = false>
 __device__ __forceinline__ void fft_stage(float2 (&v)[16], float2* __restrict__ sm,
-                                          const float2* __restrict__ tw, int tid) {
+                                          const float2* __restrict__ tw, int tid, const float2* __restrict__ twp = nullptr) {
     constexpr int TPF = N / 16, M = 16 / R;
     constexpr int STRIDE = (P == 1) ? 1 : P + P / 16;
 #pragma unroll
@@ -182,7 +184,13 @@ __device__ __forceinline__ void fft_stage(float2 (&v)[16], float2* __restrict__ 
         for (int t = 0; t < R; t++) u[t] = v[m + t * M];
         const int b = tid + m * TPF;
         const int k = b & (P - 1);
-        if (P > 1) apply_twiddle_powers<R>(u, tw[k]);
+        if constexpr (TWP && P == 16 && R == 16) {
+            // the 15 powers W^(k t) of this thread's k = tid & 15 come from a [16][15] table (conflict-free: odd row
+            // pitch) instead of 14 complex multiplications per transform
+            const float2* w = twp + k * kTwpPitch;
+#pragma unroll
+            for (int t = 1; t < R; t++) u[t] = cmul(u[t], w[t - 1]);
+        } else if (P > 1) apply_twiddle_powers<R>(u, tw[k]);
         if constexpr (ZMID && P == 1 && R == 16) bfly16_zmid(u); else bfly<R>(u);
         if (LAST) {
 #pragma unroll
@@ -229,20 +237,67 @@ __device__ __forceinline__ void fft_unload(const float2 (&v)[16], float2* __rest
 // The caller guarantees that nobody still reads `sm` from a previous use (the function
 // starts with a group barrier) -- on return `sm` may still be read by slower lanes, so
 // the next user must barrier too (this function does).
+// N = 512 (one warp per transform): the radix-2 third stage pairs element j of the first half with j + 256 of the
+// second.  After the radix-16 second stage lane l holds X2[256 (l >> 4) + (l & 15) + 16 r], r = 0..15, so the partner
+// of every value sits in lane l ^ 16, same r: the second shared-memory exchange (16 STS.64 + 16 LDS.64 + 8 twiddle
+// loads = 80 of the ~440 shared-memory wavefronts of a row transform) becomes 16 SHFL.  Lanes 0..15 finish the
+// butterflies of even r (j = l + 32 e), lanes 16..31 those of odd r (same formula), which is the natural output layout
+// v[e] <-> l + 32 e.  The twiddle W512^(l + 32 e) = W512^l * W16^e: one table value per lane and compile-time constants.
+__device__ __forceinline__ void fft512_last_stage_shfl(float2 (&v)[16], const float2 wl, int lane) {
+    const float c1 = 0.92387953251128675613f, s1 = 0.38268343236508977173f, h = 0.70710678118654752440f;
+    const bool lo = lane < 16;
+    float2 out[16];
+#pragma unroll
+    for (int e = 0; e < 8; e++) {
+        const float2 ev = v[2 * e], od = v[2 * e + 1];
+        const float2 send = lo ? od : ev;
+        float2 recv;
+        recv.x = __shfl_xor_sync(0xffffffffu, send.x, 16);
+        recv.y = __shfl_xor_sync(0xffffffffu, send.y, 16);
+        const float2 a = lo ? ev : recv;
+        float2 b = cmul(lo ? recv : od, wl);
+        switch (e) {                                   // b *= exp(2 pi i e / 16)
+            case 1: b = cmul(b, make_float2(c1, s1)); break;
+            case 2: b = make_float2(h * (b.x - b.y), h * (b.x + b.y)); break;
+            case 3: b = cmul(b, make_float2(s1, c1)); break;
+            case 4: b = cmuli(b); break;
+            case 5: b = cmul(b, make_float2(-s1, c1)); break;
+            case 6: b = make_float2(-h * (b.x + b.y), h * (b.x - b.y)); break;
+            case 7: b = cmul(b, make_float2(-c1, s1)); break;
+            default: break;
+        }
+        out[e] = cadd(a, b);
+        out[e + 8] = csub(a, b);
+    }
+#pragma unroll
+    for (int e = 0; e < 16; e++) v[e] = out[e];
+}
+
 // ZMID: v[6..9] (elements 6 TPF .. 10 TPF - 1) are zero and are not read.
-template <int N, bool ZMID = false>
+template <int N, bool ZMID = false, bool TWP = false>
 __device__ __forceinline__ void fft_inverse(float2 (&v)[16], float2* __restrict__ sm,
-                                            const float2* __restrict__ tw, int tid, int bar_id) {
+                                            const float2* __restrict__ tw, int tid, int bar_id,
+                                            const float2* __restrict__ twp = nullptr) {
     using C = FftCfg<N>;
     fft_group_sync<C::TPF>(bar_id);
     fft_stage<N, C::R1, 1, false, ZMID>(v, sm, tw, tid);
     fft_group_sync<C::TPF>(bar_id);
     fft_reload<N>(v, sm, tid);
-    if (C::NSTAGE == 2) {
-        fft_stage<N, C::R2, C::R1, true>(v, sm, tw, tid);
+#ifndef RF_X_NOSHFL
+#define RF_X_SHFL512 true
+#else
+#define RF_X_SHFL512 false
+#endif
+    if constexpr (N == 512 && RF_X_SHFL512) {
+        // second stage in registers (one butterfly per lane, k = lane & 15), third stage by shuffles
+        apply_twiddle_powers<16>(v, tw[tid & 15]);
+        bfly<16>(v);
+        fft512_last_stage_shfl(v, tw[C::TW2 + tid], tid);
+    } else if (C::NSTAGE == 2) {
+        fft_stage<N, C::R2, C::R1, true, false, TWP>(v, sm, tw, tid, twp);
     } else {
         fft_group_sync<C::TPF>(bar_id);
-        fft_stage<N, C::R2, C::R1, false>(v, sm, tw, tid);
+        fft_stage<N, C::R2, C::R1, false, false, TWP>(v, sm, tw, tid, twp);
         fft_group_sync<C::TPF>(bar_id);
         fft_reload<N>(v, sm, tid);
         fft_stage<N, (C::R3 > 1 ? C::R3 : 2), C::R1 * C::R2, true>(v, sm, tw + C::TW2, tid);
@@ -254,6 +309,16 @@ __device__ __forceinline__ void fft_inverse(float2 (&v)[16], float2* __restrict_
 template <int N>
 __device__ __forceinline__ void load_twiddles(float2* tw, const float2* __restrict__ gtw, int tid, int nthreads) {
     for (int i = tid; i < FftCfg<N>::TW_TOTAL; i += nthreads) tw[i] = gtw[i];
+}
+
+// stage-2 twiddle powers of the sizes with R2 = 16 (n >= 256): out[k * 15 + t - 1] = exp(+2 pi i k t / 256), t = 1..15
+inline void host_twiddle_powers(float2* out /* kTwpSize entries */) {
+    const double two_pi = 6.283185307179586476925286766559;
+    for (int k = 0; k < 16; k++)
+        for (int t = 1; t < 16; t++) {
+            const double a = two_pi * (double)(k * t) / 256.0;
+            out[k * kTwpPitch + t - 1] = make_float2((float)cos(a), (float)sin(a));
+        }
 }
 
 inline void host_twiddles(int n, float2* out /* 16 + 256 entries */) {

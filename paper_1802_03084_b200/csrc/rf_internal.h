@@ -101,6 +101,7 @@ struct DeviceTables {
     double* dms = nullptr;           // [ndm]
     float* weights = nullptr;        // [nchan]
     float2* twiddles = nullptr;      // [16 + 256] FFT stage twiddles
+    float2* twp = nullptr;           // [16][15] stage-2 twiddle powers
 };
 
 struct Workspace {
@@ -156,6 +157,7 @@ struct rf_plan {
     int tune_dm_group = rf::kDmGroup;   // DM trials interleaved in time by the block order
     int tune_feed_batch = 0;         // blocks per launch behind an upload (0 = one wave of row-pass CTAs)
     int tune_tree_maxpix = 4096;     // largest npix searched by the boxcar-tree kernels
+    int tune_gather_order = 1;       // 1 = gather grid runs over block pairs fastest (cell-range major), 0 = cell ranges fastest
     std::map<const void*, size_t> smem_attr;   // dynamic shared memory opted in per kernel, on this plan's device
     std::vector<double> freqs, uvw, dms;
     std::vector<int32_t> dts;
@@ -180,6 +182,7 @@ struct rf_plan {
     int64_t n_blocks = 0, n_gen_images = 0;
     int nbins = 2048;
     int64_t n_images = 0, vis_gridded = 0;
+    int64_t n_col_fft = 0, n_row_fft = 0;      // npix-point transforms one rf_search runs (column pass; row pass = pair transforms)
     int64_t n_entries = 0;
     int last_launches = 0;
     // rf_search_host staging

@@ -115,12 +115,13 @@ template <int N> size_t smem_tree1(int ntiles) {
            (size_t)ntiles * FftCfg<N>::TPF * sizeof(uint32_t);
 }
 template <int N> constexpr int tree2_threads() { return N >= 2048 ? 256 : kThreads2; }
-template <int N, int TB> size_t smem_tree2(int nbins, int cpad, int nthreads = kThreads2) {
+template <int N, int TB> size_t smem_tree2(int nbins, int cpad, int nthreads, bool zm) {
     const size_t g2 = nthreads / FftCfg<N>::TPF;
     const size_t xb = g2 * fft_padded_size(N) * sizeof(float2);
     const size_t fin = (size_t)2 * nbins * sizeof(uint32_t);
-    return std::max(xb, fin) + FftCfg<N>::TW_TOTAL * sizeof(float2) + g2 * cpad * sizeof(float4) +
-           (size_t)(N >= 2048 ? 2 * TB - 1 : TB) * nbins * sizeof(uint32_t) + 80 * 4 + (size_t)2 * kWarps2 * (2 * TB - 1) * 4;
+    const size_t sgp = zm ? row_stage_pitch<N, true>(cpad) : row_stage_pitch<N, false>(cpad);
+    return std::max(xb, fin) + (FftCfg<N>::TW_TOTAL + kTwpSize) * sizeof(float2) + g2 * sgp * sizeof(float4) +
+           (size_t)(N >= 2048 ? 2 * TB - 1 : TB) * nbins * sizeof(uint32_t) + 80 * 4 + (size_t)2 * (nthreads / 32) * (2 * TB - 1) * 4;
 }
 
 // power variant of the row pass (periodicity search): 512 threads, one 32-bit histogram per pair = TB/2 images
@@ -132,17 +133,29 @@ template <int N, int TB> size_t smem_tree2_power(int nbins, int cpad) {
            (size_t)(TB / 2) * nbins * sizeof(uint32_t) + 64 * 4 + (size_t)2 * kWarps2 * TB * 4;
 }
 
+template <int N, int TB, int NT2>
+int launch_row_stats(rf_plan* p, const TreeParams& tp, bool zm, cudaStream_t st) {
+    auto kern = zm ? k_tree_rowfft_stats<N, TB, NT2, true> : k_tree_rowfft_stats<N, TB, NT2, false>;
+    const size_t smem = smem_tree2<N, TB>(tp.nbins, tp.cpad, NT2, zm);
+    int rc = ensure_smem_attr(p, (const void*)kern, smem);
+    if (rc != RF_OK) return rc;
+    kern<<<dim3(tp.n_blk), NT2, smem, st>>>(tp);
+    RF_CUDA_CHECK(cudaGetLastError());
+    return RF_OK;
+}
+
 // event kinds: 0 = grid + column FFT (generic pass 1 / tree column FFT), 1 = row FFT + statistics,
 // 2 = Stokes-I transpose, 3 = tree gather
 template <int N, int TB, int NCOL, int QH>
 int launch_tree(rf_plan* p, const TreeParams& tp, cudaStream_t st) {
     int rc;
     {
-        auto kern = k_tree_gather<TB>;
+        auto kern = tp.part_major ? k_tree_gather<TB, true> : k_tree_gather<TB, false>;
         const size_t smem = (size_t)p->nchan * sizeof(int) + (size_t)kWarpsPerCta * 2 * (2 * TB - 1) * sizeof(float);
         if (tp.n_blk & 1) { set_error("internal: odd block count %d in a tree launch", tp.n_blk); return RF_ERR_STATE; }
         if ((rc = mark(p, st, -1)) != RF_OK) return rc;
-        kern<<<dim3(tp.n_parts, tp.n_blk / 2), kThreads, smem, st>>>(tp);
+        const dim3 grid = tp.part_major ? dim3(tp.n_blk / 2, tp.n_parts) : dim3(tp.n_parts, tp.n_blk / 2);
+        kern<<<grid, kThreads, smem, st>>>(tp);
         RF_CUDA_CHECK(cudaGetLastError());
         if ((rc = mark(p, st, 3)) != RF_OK) return rc;
     }
@@ -164,14 +177,9 @@ int launch_tree(rf_plan* p, const TreeParams& tp, cudaStream_t st) {
         return mark(p, st, 1);
     }
     {
-        constexpr int NT2 = tree2_threads<N>();
         // half planes within 6/16 of the row (always, with the default cell: |u| <= N/3, A13) take the pruned transform
         const bool zm = tp.ncol <= 6 * FftCfg<N>::TPF;
-        auto kern = zm ? k_tree_rowfft_stats<N, TB, NT2, true> : k_tree_rowfft_stats<N, TB, NT2, false>;
-        const size_t smem = smem_tree2<N, TB>(tp.nbins, tp.cpad, NT2);
-        { const int rc_a = ensure_smem_attr(p, (const void*)kern, smem); if (rc_a != RF_OK) return rc_a; }
-        kern<<<dim3(tp.n_blk), NT2, smem, st>>>(tp);
-        RF_CUDA_CHECK(cudaGetLastError());
+        if ((rc = launch_row_stats<N, TB, tree2_threads<N>()>(p, tp, zm, st)) != RF_OK) return rc;
         if ((rc = mark(p, st, 1)) != RF_OK) return rc;
     }
     return RF_OK;
@@ -225,6 +233,8 @@ TreeParams tree_params(rf_plan* p) {
     tp.n_streams = p->d.tree.n_streams;
     tp.n_parts = p->d.tree.n_parts;
     tp.twiddles = p->d.twiddles;
+    tp.twp = p->d.twp;
+    tp.part_major = p->tune_gather_order;
     tp.Ht = p->ws.Ht;
     tp.sumsq = p->ws.sumsq_t;
     tp.counters = p->ws.counters;
@@ -393,6 +403,10 @@ int ensure_workspace(rf_plan* p, bool need_generic) {
         host_twiddles(p->npix, tw);
         RF_CUDA_CHECK(cudaMalloc((void**)&p->d.twiddles, sizeof(tw)));
         RF_CUDA_CHECK(cudaMemcpy(p->d.twiddles, tw, sizeof(tw), cudaMemcpyHostToDevice));
+        float2 twp[kTwpSize];
+        host_twiddle_powers(twp);
+        RF_CUDA_CHECK(cudaMalloc((void**)&p->d.twp, sizeof(twp)));
+        RF_CUDA_CHECK(cudaMemcpy(p->d.twp, twp, sizeof(twp), cudaMemcpyHostToDevice));
     }
     if (!w.counters) {
         RF_CUDA_CHECK(cudaMalloc((void**)&w.counters, 4 * sizeof(int32_t)));

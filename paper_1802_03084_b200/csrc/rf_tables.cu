@@ -474,6 +474,13 @@ int build_image_list(rf_plan* p) {
     }
     p->n_gen_images = (int64_t)imgs.size();
     p->n_blocks = (int64_t)blocks.size();
+    // transforms actually run per search (bench.py: FFT rate under the 5 N log2 N convention): the tree kernels
+    // transform every padded column of every integration of every block and run TB/2 pair transforms per row
+    {
+        const int64_t nb = (int64_t)blocks.size() + (int64_t)blocks2.size();
+        p->n_col_fft = nb * p->tree_tb * p->d.tree.cpad + (int64_t)imgs.size() * p->d.gen.cpad;
+        p->n_row_fft = nb * (p->tree_tb / 2) * p->npix + ((int64_t)imgs.size() + 1) / 2 * p->npix;
+    }
     int rc = upload(p, &p->d.images, imgs.data(), imgs.size());
     if (rc == RF_OK) rc = upload(p, &p->d.blocks, blocks.data(), blocks.size());
     if (rc == RF_OK) rc = upload(p, &p->d.blocks2, blocks2.data(), blocks2.size());

@@ -33,6 +33,7 @@ struct TreeParams {
     const int32_t* group_cell;      // [ngroups + 1]
     const BlockDesc* blocks;        // first block of this batch
     const float2* twiddles;
+    const float2* twp;              // [16][15] stage-2 twiddle powers (rf_fft.cuh), sizes >= 256
     float2* cellsum;                // [n_blk][n_cells][TB] compact grid (unscaled sums)
     float2* Ht;                     // [n_blk][N][TB/2][cpad][2]
     float* sumsq;                   // [n_blk][2*TB-1][n_parts]
@@ -45,6 +46,7 @@ struct TreeParams {
     int32_t dbg_img;                // -1 = off
     int32_t dbg_slot;               // block of the launch the debug outputs refer to
     int32_t tpitch, nchan, ncol, cpad, ngroups, nbins, n_blk, n_cells, n_streams, n_parts;
+    int32_t part_major;             // gather grid (host side): 1 = x runs over block pairs, y over cell ranges, 0 = x over cell ranges
     int32_t dec;                    // 1, or the width dt whose phase-decimated sum array visI points at (B7)
     uint32_t phase_stride;          // dec > 1: elements per phase = (nbl*nchan + 1) * row pitch
     int32_t zero_row;               // >= 0: periodicity mode, every block uses this (all-zero) delay row
@@ -141,7 +143,7 @@ __global__ void __launch_bounds__(256) k_phase_sum(const float2* __restrict__ vi
 // sum_cells w |sum_{q in node} G_q|^2, are taken at the same place (another log2(TB) xor steps over
 // q), so sigma_rms of every image of the block is known before any pixel exists.
 // No tile, no barriers inside the loop, few registers: latency is hidden by occupancy.
-template <int TB>
+template <int TB, bool PART_MAJOR>
 __global__ void __launch_bounds__(kThreads, 4) k_tree_gather(const TreeParams p) {
     constexpr int NIMG = 2 * TB - 1;
     constexpr int LG = 16 / TB, U = kTreeUnroll;
@@ -151,7 +153,10 @@ __global__ void __launch_bounds__(kThreads, 4) k_tree_gather(const TreeParams p)
     float* red = reinterpret_cast<float*>(sdelay + p.nchan);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int part = blockIdx.x, slot = 2 * blockIdx.y;            // the pair (slot, slot + 1)
+    // the pair (slot, slot + 1).  part_major: consecutive CTAs serve the SAME cell range (= the same (baseline, channel)
+    // series) for consecutive block pairs, whose windows overlap almost entirely (neighbouring DM trials, consecutive
+    // times), so a series is fetched from HBM once per launch instead of once per pair
+    const int part = PART_MAJOR ? blockIdx.y : blockIdx.x, slot = 2 * (PART_MAJOR ? blockIdx.x : blockIdx.y);
     const BlockDesc blk = p.blocks[slot];
     const int j = lane / (2 * TB), h = (lane / TB) & 1, q = lane % TB;
     const int s = part * kWarpsPerCta + warp;
@@ -331,8 +336,10 @@ __global__ void __launch_bounds__(NTH) k_tree_colfft(const TreeParams p) {
         const int i = tid % SEG, pr = i / NCOL, c = i % NCOL;
         const float2* ta = tile + (2 * pr * NCOL + c) * PITCH;
         const float2* tb = ta + NCOL * PITCH;
+        const bool col0 = g * NCOL + c == 0;
         for (int y = y0; y < N; y += NTH / SEG) {
-            const float2 a = ta[fft_pad(y)], b = tb[fft_pad(y)];
+            float2 a = ta[fft_pad(y)], b = tb[fft_pad(y)];
+            if (col0) { a.y = 0.f; b.y = 0.f; }       // column 0 is Hermitian along v: its transform is real (B2)
             Hs[((size_t)y * (TB / 2) + q0 / 2 + pr) * p.cpad + g * NCOL + c] = make_float4(a.x, a.y, b.x, b.y);
         }
     }
@@ -390,9 +397,11 @@ __device__ __forceinline__ void tree_row_stats(const float (&x)[16], int img, in
 #pragma unroll
         for (int d = 16; d > 0; d >>= 1) wm = fmaxf(wm, __shfl_xor_sync(0xffffffffu, wm, d));
         int xp = 0x7fffffff;
-        if (m == wm) {
+        if (m == wm) {                   // first element holding the maximum; its position is formed only here
+            int eb = 0;
 #pragma unroll
-            for (int e = 15; e >= 0; e--) if (x[e] == wm) xp = y * N + t + TPF * e;
+            for (int e = 15; e >= 0; e--) if (x[e] == wm) eb = e;
+            xp = y * N + t + TPF * eb;
         }
 #pragma unroll
         for (int d = 16; d > 0; d >>= 1) xp = min(xp, __shfl_xor_sync(0xffffffffu, xp, d));
@@ -433,6 +442,10 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     } while (!done);
 }
 constexpr int kMaxRowGroups = 32;       // transform groups per row-pass CTA (one mbarrier each)
+// entries (16 bytes) of one group's staging buffer in the row pass
+template <int N, bool ZM> __host__ __device__ constexpr int row_stage_pitch(int cpad) {
+    return ZM ? (cpad > 6 * (N / 16) + 4 ? cpad : 6 * (N / 16) + 4) : cpad;
+}
 
 constexpr int kThreads2 = 512;          // tree pass 2: one CTA of 16 warps per SM
 constexpr int kWarps2 = kThreads2 / 32;
@@ -455,8 +468,12 @@ __global__ void __launch_bounds__(NT2, N >= 2048 ? 2 : 1) k_tree_rowfft_stats(co
     // region 0 holds the FFT exchange buffers, later the unpacked histogram + prefix sums
     const int region0 = max(G2 * XB, p.nbins);                               // float2 units
     float2* tw = xbuf + region0;
-    float4* stg = reinterpret_cast<float4*>(tw + C::TW_TOTAL);               // [G2][cpad] staged (row, pair)
-    uint32_t* hist = reinterpret_cast<uint32_t*>(stg + (size_t)G2 * p.cpad); // [NW][nbins]
+    float2* twp = tw + C::TW_TOTAL;                                          // [16][15] stage-2 twiddle powers
+    // staged (row, pair) of each group, [G2][sgp]: ZM reads columns 0 .. 6 TPF unconditionally, so the buffer spans them
+    // and everything past ncol stays zero (the bulk copy writes ncol entries only)
+    const int sgp = row_stage_pitch<N, ZM>(p.cpad);
+    float4* stg = reinterpret_cast<float4*>(twp + kTwpSize);
+    uint32_t* hist = reinterpret_cast<uint32_t*>(stg + (size_t)G2 * sgp);    // [NW][nbins]
     float* sA = reinterpret_cast<float*>(hist + (size_t)NW * p.nbins);       // [16]
     float* sScale = sA + 16;                                                 // [16]
     float* sSig = sScale + 16;                                               // [16] sigma_rms per image
@@ -472,25 +489,32 @@ __global__ void __launch_bounds__(NT2, N >= 2048 ? 2 : 1) k_tree_rowfft_stats(co
     const BlockDesc blk = p.blocks[slot];
     const float2* Hblk = p.Ht + (size_t)slot * N * p.cpad * TB;
     const int grp = tid / C::TPF, t = tid % C::TPF;
-    float4* sg = stg + (size_t)grp * p.cpad;
+    float4* sg = stg + (size_t)grp * sgp;
 
     __shared__ __align__(8) uint64_t mbar[kMaxRowGroups];
-    // stage (row y, pair p2): ncol contiguous 16-byte (H_a, H_b) entries = ONE bulk copy issued by the group's first thread
-    auto stage = [&](int y, int p2) {
-        const float4* src = reinterpret_cast<const float4*>(Hblk + ((size_t)y * (TB / 2) + p2) * p.cpad * 2);
+    // Staging: (row y, pair p2) = ncol contiguous 16-byte (H_a, H_b) entries = ONE bulk copy issued by the group's first
+    // thread.  The group walks rows grp, grp + G2, ... and the TB/2 pairs of each, so the source advances by one
+    // (row, pair) inside a row and by (G2 - 1) TB/2 + 1 of them at the end of a row: a running pointer, no index math.
+    const char* src_next = reinterpret_cast<const char*>(Hblk) + (size_t)grp * (TB / 2) * p.cpad * 16;
+    const uint32_t copy_bytes = (uint32_t)p.ncol * 16u;
+    const size_t step_pair = (size_t)p.cpad * 16, step_row = ((size_t)(G2 - 1) * (TB / 2) + 1) * p.cpad * 16;
+    auto stage_next = [&](bool end_of_row) {
         if (t == 0) {
-            mbar_arrive_expect_tx(&mbar[grp], (uint32_t)p.ncol * 16u);
-            bulk_copy_g2s(sg, src, (uint32_t)p.ncol * 16u, &mbar[grp]);
+            mbar_arrive_expect_tx(&mbar[grp], copy_bytes);
+            bulk_copy_g2s(sg, src_next, copy_bytes, &mbar[grp]);
         }
+        src_next += end_of_row ? step_row : step_pair;
     };
+    for (int i = tid; i < G2 * sgp; i += NT2) stg[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     if (tid < kMaxRowGroups) mbar_init(&mbar[tid], 1);
-    mbar_fence_init();
+    mbar_fence_init();                   // also orders the zero fill (generic proxy) before the first bulk copy
     __syncthreads();
-    stage(grp, 0);
+    stage_next(TB == 2);
     uint32_t phase = 0;
 
     for (int i = tid; i < NW * p.nbins; i += NT2) hist[i] = 0u;
     load_twiddles<N>(tw, p.twiddles, tid, NT2);
+    for (int i = tid; i < kTwpSize; i += NT2) twp[i] = p.twp[i];
     for (int i = tid; i < NWP * NIMG; i += NT2) { sBest[i] = -CUDART_INF_F; sBpos[i] = 0; }
     if (tid < NIMG) {
         int l = 0, off = 0;
@@ -516,29 +540,39 @@ __global__ void __launch_bounds__(NT2, N >= 2048 ? 2 : 1) k_tree_rowfft_stats(co
 
     for (int y = grp; y < N; y += G2) {
         float s2p[16], s4p[16];
-#pragma unroll 1
+#ifndef RF_X_UNROLL
+#define RF_X_UNROLL 1
+#endif
+        constexpr int kUnrollPairs = RF_X_UNROLL;
+#pragma unroll kUnrollPairs
         for (int p2 = 0; p2 < TB / 2; p2++) {
             float2 v[16];
             mbar_wait(&mbar[grp], phase);                        // the (row, pair) has landed
             phase ^= 1u;
+            // Z[c] = H_a[c] + i H_b[c], Z[N - c] = conj(H_a[c]) + i conj(H_b[c]); the column pass stores exact zeros in
+            // the imaginary parts of column 0 (rounding noise of a Hermitian column, B2), so c = 0 needs no special case
 #pragma unroll
             for (int e = 0; e < 16; e++) {
-                if (ZM && e >= 6 && e <= 9) { v[e] = make_float2(0.f, 0.f); continue; }
-                const int c = t + C::TPF * e;
-                const int cc = (e < 8) ? c : N - c;
-                float4 h = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (cc < p.ncol) h = sg[cc];
-                if (cc == 0 || cc == N / 2) v[e] = make_float2(h.x, h.z);
-                else if (e < 8) v[e] = make_float2(h.x - h.w, h.y + h.z);
-                else v[e] = make_float2(h.x + h.w, h.z - h.y);
+                if (ZM) {
+                    if (e >= 6 && e <= 9) { v[e] = make_float2(0.f, 0.f); continue; }
+                    const float4 h = sg[(e < 8) ? t + C::TPF * e : N - C::TPF * e - t];   // past ncol: zeros
+                    v[e] = (e < 8) ? make_float2(h.x - h.w, h.y + h.z) : make_float2(h.x + h.w, h.z - h.y);
+                } else {
+                    const int c = t + C::TPF * e;
+                    const int cc = (e < 8) ? c : N - c;
+                    float4 h = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (cc < p.ncol) h = sg[cc];
+                    if (cc == 0 || cc == N / 2) v[e] = make_float2(h.x, h.z);
+                    else if (e < 8) v[e] = make_float2(h.x - h.w, h.y + h.z);
+                    else v[e] = make_float2(h.x + h.w, h.z - h.y);
+                }
             }
             fft_group_sync<C::TPF>(1 + grp);                     // staging buffer consumed
             {   // prefetch the next (row, pair) of this group while this one is transformed
-                const int np2 = (p2 + 1 == TB / 2) ? 0 : p2 + 1;
-                const int ny = (p2 + 1 == TB / 2) ? y + G2 : y;
-                if (ny < N) stage(ny, np2);
+                const bool last_pair = p2 + 1 == TB / 2;
+                if (!last_pair || y + G2 < N) stage_next(p2 + 2 == TB / 2 || (TB == 2));
             }
-            fft_inverse<N, ZM>(v, xb, tw, t, 1 + grp);
+            fft_inverse<N, ZM, (N >= 2048)>(v, xb, tw, t, 1 + grp, twp);
             float a[16], s2[16];
 #pragma unroll
             for (int e = 0; e < 16; e++) a[e] = v[e].x;

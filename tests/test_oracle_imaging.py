@@ -107,6 +107,51 @@ def test_noiseless_injection_closed_form(width, t0):
     assert np.abs(other).max() < 1e-12
 
 
+def _closed_form_sidelobe_rms2(uvw, f, cell, npix, iu, iv, keep, amp, l, m):
+    """P9: mean(img^2) of a noiseless point source of amplitude A at (l, m) = sum_cells |G_c|^2 / (2 N_w)^2 (Parseval,
+    P6) with G_c = sum over the samples of cell c of A e^{-2 pi i (u l + v m) cell} plus the conjugates of the samples
+    of the mirrored cell: the dirty-beam sidelobes of the source itself, which raise the image sigma."""
+    ul = uvw[:, 0:1] * f[None, :] / O.C_LIGHT
+    vl = uvw[:, 1:2] * f[None, :] / O.C_LIGHT
+    s = amp * np.exp(-2j * np.pi * (ul * l + vl * m) * cell)
+    cells = {}
+    for b, c in zip(*np.nonzero(keep)):
+        a, e = int(iu[b, c]) % npix, int(iv[b, c]) % npix
+        cells[(e, a)] = cells.get((e, a), 0j) + s[b, c]
+        cells[((-e) % npix, (-a) % npix)] = cells.get(((-e) % npix, (-a) % npix), 0j) + s[b, c].conjugate()
+    n_w = int(keep.sum())
+    return sum(abs(g) ** 2 for g in cells.values()) / (2.0 * n_w) ** 2
+
+
+def test_expected_snr_of_the_injected_source_closed_form():
+    """P9 (north_star: "recovered ... with the expected S/N"): at the matched trial the image statistic is NOT the
+    matched-filter S/N A sqrt(N_w N_pol)/s = 107 -- the source's own sidelobes raise sigma:
+        sigma_rms^2 = s^2/(N_w N_pol) + 2 sum_c |g_c|^2/(2 N_w)^2,   S/N_rms = peak_P8 / sigma_rms  (~ 14 for config 1).
+    Noiseless: exact.  With the config's unit noise: the noise term adds in expectation (scatter of a few per cent
+    from the ~190 independent cells and the signal x noise cross term).  The MAD estimator the search uses (A9) is
+    bracketed against the rms one: the sidelobe field is lighter-tailed than a Gaussian of the same rms."""
+    cfg, f, uvw, cell, dms, delays, iu, iv, keep = _setup()
+    src = Transient(2.0, 8, -5, float(dms[3]), 1, 20)             # DM 60 = trial 3: exactly on the grid
+    n_w = int(keep.sum())
+    side2 = _closed_form_sidelobe_rms2(uvw, f, cell, cfg.npix, iu, iv, keep, 2.0, 8, -5)
+    peak_cf = _closed_form_peak(uvw, f, cell, cfg.npix, iu, iv, keep, 2.0, 8, -5)
+    # noiseless: the closed form is exact (complex64 input rounding only)
+    img0 = O.search_image(W.make_segment(cfg, noise=False, sources=[src]), delays, iu, iv, keep, cfg.npix, 3, 1, 20)
+    assert abs((img0 ** 2).mean() - side2) < 1e-6 * side2
+    # matched-filter S/N, for contrast
+    assert abs(2.0 * math.sqrt(n_w * cfg.npol) / 1.0 - 107.3) < 0.5
+    noise2 = 1.0 / (n_w * cfg.npol)
+    snr_expected = peak_cf / math.sqrt(noise2 + side2)
+    assert 12.0 < snr_expected < 16.0                              # SURVEY P9: ~ 14
+    img = O.search_image(W.make_segment(cfg, sources=[src]), delays, iu, iv, keep, cfg.npix, 3, 1, 20)
+    peak, y, x, sigma_mad, snr_mad = O.image_stats(img)
+    assert (y, x) == (59, 8)
+    sig_rms = math.sqrt((img ** 2).mean())
+    assert abs(sig_rms ** 2 - (noise2 + side2)) < 0.12 * (noise2 + side2)
+    assert abs(peak / sig_rms - snr_expected) < 0.10 * snr_expected
+    assert 0.6 * sig_rms < sigma_mad < 1.05 * sig_rms and snr_expected * 0.9 < snr_mad < 30.0
+
+
 def test_tiny_config_recovery():
     """P10: config 1 injects DM 50 between trials 40 and 60: best candidate at trial 40 or
     60, pixel (8,-5), arrival time near t0 = 20, S/N well above threshold."""

@@ -24,3 +24,17 @@ def test_streaming_noise_overlaps_bit_for_bit():
     b = W.make_segment(cfg, 4, inject=False, rows=(0, 2))
     assert overlap == 624 and np.array_equal(a, b)
     assert a.dtype == np.complex64 and a.shape == (2, cfg.nbl, cfg.nchan, cfg.npol)
+
+
+def test_goal_workload_1ms_matches_the_paper_rate():
+    """PAPER.md:94 / Table 1 row "L": 1 ms sampling of the L-band array is 1.4 GB/s; the
+    stream1ms config keeps config 5's 2.0 s stride and overlaps by its own DM 1000 sweep."""
+    import oracle as O
+    cfg = W.get_config("stream1ms")
+    rate = cfg.nbl * cfg.nchan * cfg.npol * 8 / cfg.inttime_s
+    assert abs(rate / 1.4e9 - 1.0) < 0.03
+    delays = O.delay_table(W.channel_freqs_hz(cfg), W.dm_list(cfg), cfg.inttime_s)
+    assert int(delays.max()) == cfg.nint - cfg.stride_int == 3118
+    assert cfg.stride_int * cfg.inttime_s == W.get_config("stream").stride_int * W.get_config("stream").inttime_s == 2.0
+    n_img = sum(O.n_images(cfg.nint, int(delays[d].max()), dt, cfg.stride_int) for d in range(cfg.ndm) for dt in cfg.dt_list)
+    assert n_img == 64 * (2000 + 1000 + 500 + 250)

@@ -95,7 +95,19 @@ _STREAM = Config(
     dm_inj_range=(100.0, 900.0), width_range=(1, 8), offset_mode="central",
     n_segments=32, stride_int=400)
 
-CONFIGS = {c.name: c for c in (_TINY, _LBAND, _SBAND, _HIRES, _STREAM)}
+# The paper's GOAL workload ("1 ms ... 1.4 GB/s"; Table 1 row "L"): the config-5 array,
+# band and trial grid sampled at 1 ms.  Segment stride 2.0 s as in config 5 (2000 integrations), overlap = the
+# DM 1000 sweep at 1 ms = 3118 integrations, 8 consecutive segments.  New data per segment:
+# 2000 x 351 x 256 x 2 x 8 B = 2.875 GB per 2.0 s = 1.44 GB/s.
+_STREAM1MS = Config(
+    name="stream1ms", index=5, layout="Y", nant=27, r_min_m=40.0, r_max_m=1000.0,
+    dec_deg=20.0, ha_hours=-1.0, f_start_ghz=1.0, chan_width_ghz=0.004, nchan=256,
+    npol=2, nint=5118, inttime_s=0.001, dm_max=1000.0, ndm=64, dt_list=(1, 2, 4, 8),
+    npix=512, threshold=7.0, n_transients=2, amp_range=(0.3, 1.0),
+    dm_inj_range=(100.0, 900.0), width_range=(1, 8), offset_mode="central",
+    n_segments=8, stride_int=2000)
+
+CONFIGS = {c.name: c for c in (_TINY, _LBAND, _SBAND, _HIRES, _STREAM, _STREAM1MS)}
 
 
 def get_config(name: str) -> Config:
