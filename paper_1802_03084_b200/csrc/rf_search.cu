@@ -108,19 +108,22 @@ int launch_batch(rf_plan* p, const SearchParams& sp, cudaStream_t st) {
 }
 
 // ---------------------------------------------------------------- boxcar-tree path
-template <int N> int tree_nbins(int) { return N <= 1024 ? 2048 : 4096; }
+// 2048 bins at every size: the quantile error of the interpolated histogram shrinks with the pixel count (B1), and at
+// N >= 2048 (one 32-bit counter per bin and image) 4096 bins would cost the second row-pass CTA per SM
+template <int N> int tree_nbins(int) { return 2048; }
 
 template <int N> size_t smem_tree1(int ntiles) {
     return (size_t)ntiles * (fft_padded_size(N) + 1) * sizeof(float2) + FftCfg<N>::TW_TOTAL * sizeof(float2) +
            (size_t)ntiles * FftCfg<N>::TPF * sizeof(uint32_t);
 }
 template <int N> constexpr int tree2_threads() { return N >= 2048 ? 256 : kThreads2; }
-template <int N, int TB> size_t smem_tree2(int nbins, int cpad, int nthreads, bool zm) {
+template <int N, int TB> size_t smem_tree2(int nbins, int cpad, int nthreads, bool zm, bool rp) {
     const size_t g2 = nthreads / FftCfg<N>::TPF;
     const size_t xb = g2 * fft_padded_size(N) * sizeof(float2);
     const size_t fin = (size_t)2 * nbins * sizeof(uint32_t);
-    const size_t sgp = zm ? row_stage_pitch<N, true>(cpad) : row_stage_pitch<N, false>(cpad);
-    return std::max(xb, fin) + (FftCfg<N>::TW_TOTAL + kTwpSize) * sizeof(float2) + g2 * sgp * sizeof(float4) +
+    // staged items: one per transform group ((row, pair), or a double row with the row-pair hand-off)
+    const size_t stg = rp ? g2 * (size_t)2 * cpad : g2 * (size_t)(zm ? row_stage_pitch<N, true>(cpad) : row_stage_pitch<N, false>(cpad));
+    return std::max(xb, fin) + (FftCfg<N>::TW_TOTAL + kTwpSize) * sizeof(float2) + stg * sizeof(float4) +
            (size_t)(N >= 2048 ? 2 * TB - 1 : TB) * nbins * sizeof(uint32_t) + 80 * 4 + (size_t)2 * (nthreads / 32) * (2 * TB - 1) * 4;
 }
 
@@ -133,13 +136,20 @@ template <int N, int TB> size_t smem_tree2_power(int nbins, int cpad) {
            (size_t)(TB / 2) * nbins * sizeof(uint32_t) + 64 * 4 + (size_t)2 * kWarps2 * TB * 4;
 }
 
+// rp: row-pair hand-off (N >= 2048 with TB = 2, see k_tree_colfft)
+template <int N, int TB> constexpr bool row_pair_layout() { return N >= 2048 && TB == 2; }
+
 template <int N, int TB, int NT2>
-int launch_row_stats(rf_plan* p, const TreeParams& tp, bool zm, cudaStream_t st) {
-    auto kern = zm ? k_tree_rowfft_stats<N, TB, NT2, true> : k_tree_rowfft_stats<N, TB, NT2, false>;
-    const size_t smem = smem_tree2<N, TB>(tp.nbins, tp.cpad, NT2, zm);
+int launch_row_stats(rf_plan* p, const TreeParams& tp, bool zm, bool rp, cudaStream_t st) {
+    void (*kern)(const TreeParams) = zm ? k_tree_rowfft_stats<N, TB, NT2, true, false> : k_tree_rowfft_stats<N, TB, NT2, false, false>;
+    const int nthreads = NT2;
+    if constexpr (row_pair_layout<N, TB>()) {
+        if (rp) kern = zm ? k_tree_rowfft_stats<N, TB, NT2, true, true> : k_tree_rowfft_stats<N, TB, NT2, false, true>;
+    }
+    const size_t smem = smem_tree2<N, TB>(tp.nbins, tp.cpad, nthreads, zm, rp);
     int rc = ensure_smem_attr(p, (const void*)kern, smem);
     if (rc != RF_OK) return rc;
-    kern<<<dim3(tp.n_blk), NT2, smem, st>>>(tp);
+    kern<<<dim3(tp.n_blk), nthreads, smem, st>>>(tp);
     RF_CUDA_CHECK(cudaGetLastError());
     return RF_OK;
 }
@@ -159,9 +169,13 @@ int launch_tree(rf_plan* p, const TreeParams& tp, cudaStream_t st) {
         RF_CUDA_CHECK(cudaGetLastError());
         if ((rc = mark(p, st, 3)) != RF_OK) return rc;
     }
+    // row-pair hand-off (one column per column-pass CTA, three CTAs per SM): transient search at N >= 2048 with TB = 2;
+    // the periodicity search keeps the plain layout its power kernel reads
+    const bool rp = row_pair_layout<N, TB>() && tp.zero_row < 0;
     {
-        constexpr int NTH = N >= 4096 ? 512 : kThreads;   // two concurrent 4096-point transforms per CTA
-        auto kern = k_tree_colfft<N, TB, NCOL, QH, NTH>;
+        constexpr int NTH = (N >= 4096 && QH * NCOL > 2) ? 512 : kThreads;   // 4 tiles of 4096: two concurrent transforms
+        void (*kern)(const TreeParams) = k_tree_colfft<N, TB, NCOL, QH, NTH, false>;
+        if constexpr (row_pair_layout<N, TB>()) { if (rp) kern = k_tree_colfft<N, TB, NCOL, QH, NTH, true>; }
         const size_t smem = smem_tree1<N>(QH * NCOL);
         { const int rc_a = ensure_smem_attr(p, (const void*)kern, smem); if (rc_a != RF_OK) return rc_a; }
         kern<<<dim3(tp.ngroups, tp.n_blk, TB / QH), NTH, smem, st>>>(tp);
@@ -179,7 +193,7 @@ int launch_tree(rf_plan* p, const TreeParams& tp, cudaStream_t st) {
     {
         // half planes within 6/16 of the row (always, with the default cell: |u| <= N/3, A13) take the pruned transform
         const bool zm = tp.ncol <= 6 * FftCfg<N>::TPF;
-        if ((rc = launch_row_stats<N, TB, tree2_threads<N>()>(p, tp, zm, st)) != RF_OK) return rc;
+        if ((rc = launch_row_stats<N, TB, tree2_threads<N>()>(p, tp, zm, rp, st)) != RF_OK) return rc;
         if ((rc = mark(p, st, 1)) != RF_OK) return rc;
     }
     return RF_OK;
@@ -193,8 +207,8 @@ int launch_tree_batch(rf_plan* p, TreeParams& tp, cudaStream_t st, int tb = 0) {
         RF_TCASE(256, 2, 16, 2) RF_TCASE(256, 4, 8, 4) RF_TCASE(256, 8, 4, 8)
         RF_TCASE(512, 2, 8, 2) RF_TCASE(512, 4, 4, 4) RF_TCASE(512, 8, 2, 4)
         RF_TCASE(1024, 2, 4, 2) RF_TCASE(1024, 4, 2, 4) RF_TCASE(1024, 8, 2, 4)
-        RF_TCASE(2048, 2, 2, 2) RF_TCASE(2048, 4, 2, 2)
-        RF_TCASE(4096, 2, 2, 2) RF_TCASE(4096, 4, 2, 2)
+        RF_TCASE(2048, 2, 1, 2) RF_TCASE(2048, 4, 2, 2)
+        RF_TCASE(4096, 2, 1, 2) RF_TCASE(4096, 4, 2, 2)
 #undef RF_TCASE
     }
     set_error("unsupported tree configuration npix %d tb %d", p->npix, tb);

@@ -289,7 +289,8 @@ int build_grid_lists(rf_plan* p) {
 int tree_cols_per_group(int npix, int tb) {
     if (npix <= 512) return (16 * 512) / (npix * tb);     // TB x NCOL = 16 tiles of 512 (32 of 256): 70 KB
     if (npix == 1024) return tb == 2 ? 4 : 2;             // 8 tiles of 1024; TB > 4 is split over blockIdx.z
-    return 2;                                             // 4 tiles of 2048 (70 KB) / 4096 (139 KB)
+    return tb == 2 ? 1 : 2;                               // TB = 2: one column x 2 integrations (row-pair hand-off, 74 KB at 4096,
+                                                          // three CTAs per SM); TB = 4: 4 tiles of 2048 (70 KB) / 4096 (139 KB)
 }
 
 // Row pitch of the phase-decimated sum array of width dt: output integrations j' = t / dt of one series and phase,

@@ -249,7 +249,16 @@ __global__ void __launch_bounds__(kThreads, 4) k_tree_gather(const TreeParams p)
 // (blockIdx.z selects which: QH < TB keeps two columns per CTA, i.e. whole 32-byte sectors in the
 // store, with tiles small enough for four CTAs per SM), from the compact grid into its tiles,
 // transforms the QH*NCOL columns in place (inverse, along v) and stores the half plane.
-template <int N, int TB, int NCOL, int QH, int NTH>
+// Entry (16 bytes = the two integrations of one (row, column)) of a double row in the row-pair hand-off: the two
+// rows of a column share one 32-byte sector, and columns whose bit 2 is set hold them in swapped order, so that the
+// row pass's 16-byte shared-memory reads of 8 consecutive columns of ONE row fall into 8 different bank groups
+// (plain order: lane stride 32 bytes = 2-way bank conflicts on every staging read, +10 % on the 4096^2 row pass).
+__host__ __device__ __forceinline__ int rp_entry(int c, int row_parity) { return 2 * c + (row_parity ^ ((c >> 2) & 1)); }
+
+// RP ("row-pair" hand-off, N >= 2048 with TB = 2): H[slot][y / 2][c][y & 1][q] -- the two integrations of TWO
+// consecutive rows of one column are 32 contiguous bytes, so a CTA that holds ONE column (two 4096-point tiles, 74 KB,
+// three CTAs per SM instead of one) still writes whole 32-byte sectors, and a double row is contiguous for the row pass.
+template <int N, int TB, int NCOL, int QH, int NTH, bool RP = false>
 __global__ void __launch_bounds__(NTH) k_tree_colfft(const TreeParams p) {
     using C = FftCfg<N>;
     constexpr int PITCH = fft_padded_size(N) + 1;
@@ -340,7 +349,8 @@ __global__ void __launch_bounds__(NTH) k_tree_colfft(const TreeParams p) {
         for (int y = y0; y < N; y += NTH / SEG) {
             float2 a = ta[fft_pad(y)], b = tb[fft_pad(y)];
             if (col0) { a.y = 0.f; b.y = 0.f; }       // column 0 is Hermitian along v: its transform is real (B2)
-            Hs[((size_t)y * (TB / 2) + q0 / 2 + pr) * p.cpad + g * NCOL + c] = make_float4(a.x, a.y, b.x, b.y);
+            if (RP) Hs[(((size_t)(y >> 1)) * (TB / 2) + q0 / 2 + pr) * p.cpad * 2 + rp_entry(g * NCOL + c, y & 1)] = make_float4(a.x, a.y, b.x, b.y);
+            else Hs[((size_t)y * (TB / 2) + q0 / 2 + pr) * p.cpad + g * NCOL + c] = make_float4(a.x, a.y, b.x, b.y);
         }
     }
 }
@@ -420,6 +430,12 @@ __device__ __forceinline__ void tree_row_stats(const float (&x)[16], int img, in
 // (row, pair) of the half plane (ncol x 16 bytes) global -> shared; no per-thread copy instructions, no register
 // staging, the consumers sleep on the barrier's phase bit (SASS: UBLKCP + SYNCS).
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+// 16-byte asynchronous global -> shared copy (LDGSTS), used where the source is strided (row-pair hand-off)
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(smem_dst)), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int PENDING> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(PENDING) : "memory"); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
 }
@@ -441,6 +457,22 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
                      : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
     } while (!done);
 }
+// The staging buffer is handed back to the ASYNC proxy (the next bulk copy overwrites it) after a group barrier.  A
+// barrier orders generic-proxy accesses among the threads, but the copy engine is another proxy: a shared-memory load
+// that has only been ISSUED may still sit in the LSU queue when the elected thread passes the barrier (ptxas sinks the
+// instructions that consume the loads past BAR.SYNC), and the engine does not see that queue.  Seen as run-to-run
+// differences of 1e-5 in sigma at npix 1024 (two warps per transform), found by searching the same segment twice and
+// comparing the records bit for bit (tests: test_repeated_search_is_bit_identical).
+// Every reader therefore makes sure its loaded values have ARRIVED before it reaches the barrier: a volatile store of
+// a word that depends on every loaded register cannot issue before the loads have returned.  (A cross-proxy fence,
+// fence.proxy.async = MEMBAR.ALL.CTA + FENCE.VIEW.ASYNC, is the textbook form; it also drains the histogram atomics
+// of the previous transform: +0.7 ms per L-band step.)
+__device__ __forceinline__ void loads_arrived_before_release(const float2 (&v)[16], volatile uint32_t* scratch) {
+    uint32_t acc = 0u;
+#pragma unroll
+    for (int e = 0; e < 16; e++) acc |= __float_as_uint(v[e].x);      // .x and .y of an element come from ONE 16-byte load
+    *scratch = acc;
+}
 constexpr int kMaxRowGroups = 32;       // transform groups per row-pass CTA (one mbarrier each)
 // entries (16 bytes) of one group's staging buffer in the row pass
 template <int N, bool ZM> __host__ __device__ constexpr int row_stage_pitch(int cpad) {
@@ -454,8 +486,18 @@ constexpr int kWarps2 = kThreads2 / 32;
 // needs 128 or 256 threads and two or three smaller CTAs per SM hide its barriers better than one large one.
 // ZM: the half plane occupies at most 6 N/16 columns (ncol <= 6 TPF; always true with the default cell, A13), so
 // elements 6 TPF .. 10 TPF - 1 of every row spectrum are zero: not staged into registers, pruned from the first stage.
-template <int N, int TB, int NT2, bool ZM>
+// RP: the hand-off has the row-pair layout of k_tree_colfft<..., RP = true> (TB = 2): one bulk copy stages a DOUBLE
+// row (ncol x 32 bytes, entries rp_entry(c, y & 1)).  The group unpacks BOTH rows into registers at once and hands the
+// buffer back, so the next double row is copied behind two row transforms.
+template <int N, int TB, int NT2, bool ZM, bool RP = false>
 __global__ void __launch_bounds__(NT2, N >= 2048 ? 2 : 1) k_tree_rowfft_stats(const TreeParams p) {
+    static_assert(!RP || TB == 2, "the row-pair hand-off holds one pair per row");
+    constexpr int RPH = RP ? 2 : 1;                   // rows per staged item
+#ifdef RF_X_NOPAD
+    constexpr bool PADDED = false;
+#else
+    constexpr bool PADDED = ZM && !RP;                // staging buffer zero-padded to 6 TPF columns: unconditional loads
+#endif
     constexpr int NWP = NT2 / 32;
     using C = FftCfg<N>;
     constexpr int G2 = NT2 / C::TPF;
@@ -471,7 +513,7 @@ __global__ void __launch_bounds__(NT2, N >= 2048 ? 2 : 1) k_tree_rowfft_stats(co
     float2* twp = tw + C::TW_TOTAL;                                          // [16][15] stage-2 twiddle powers
     // staged (row, pair) of each group, [G2][sgp]: ZM reads columns 0 .. 6 TPF unconditionally, so the buffer spans them
     // and everything past ncol stays zero (the bulk copy writes ncol entries only)
-    const int sgp = row_stage_pitch<N, ZM>(p.cpad);
+    const int sgp = RPH * row_stage_pitch<N, PADDED>(p.cpad);     // entries of one staged item
     float4* stg = reinterpret_cast<float4*>(twp + kTwpSize);
     uint32_t* hist = reinterpret_cast<uint32_t*>(stg + (size_t)G2 * sgp);    // [NW][nbins]
     float* sA = reinterpret_cast<float*>(hist + (size_t)NW * p.nbins);       // [16]
@@ -492,12 +534,14 @@ __global__ void __launch_bounds__(NT2, N >= 2048 ? 2 : 1) k_tree_rowfft_stats(co
     float4* sg = stg + (size_t)grp * sgp;
 
     __shared__ __align__(8) uint64_t mbar[kMaxRowGroups];
+    __shared__ uint32_t rel_scratch[32];       // see loads_arrived_before_release
     // Staging: (row y, pair p2) = ncol contiguous 16-byte (H_a, H_b) entries = ONE bulk copy issued by the group's first
     // thread.  The group walks rows grp, grp + G2, ... and the TB/2 pairs of each, so the source advances by one
     // (row, pair) inside a row and by (G2 - 1) TB/2 + 1 of them at the end of a row: a running pointer, no index math.
-    const char* src_next = reinterpret_cast<const char*>(Hblk) + (size_t)grp * (TB / 2) * p.cpad * 16;
-    const uint32_t copy_bytes = (uint32_t)p.ncol * 16u;
-    const size_t step_pair = (size_t)p.cpad * 16, step_row = ((size_t)(G2 - 1) * (TB / 2) + 1) * p.cpad * 16;
+    // (RP: an item is a double row of cpad x 32 bytes, one pair per row)
+    const char* src_next = reinterpret_cast<const char*>(Hblk) + (size_t)grp * (TB / 2) * p.cpad * (16 * RPH);
+    const uint32_t copy_bytes = (uint32_t)p.ncol * (16u * RPH);
+    const size_t step_pair = (size_t)p.cpad * (16 * RPH), step_row = ((size_t)(G2 - 1) * (TB / 2) + 1) * p.cpad * (16 * RPH);
     auto stage_next = [&](bool end_of_row) {
         if (t == 0) {
             mbar_arrive_expect_tx(&mbar[grp], copy_bytes);
@@ -538,7 +582,31 @@ __global__ void __launch_bounds__(NT2, N >= 2048 ? 2 : 1) k_tree_rowfft_stats(co
     float2* xb = xbuf + grp * XB;
     const bool dbg = p.image_out != nullptr && slot == p.dbg_slot;
 
-    for (int y = grp; y < N; y += G2) {
+    // unpack one staged row into the transform input: Z[c] = H_a[c] + i H_b[c], Z[N - c] = conj(H_a[c]) + i conj(H_b[c]);
+    // the column pass stores exact zeros in the imaginary parts of column 0 (rounding noise of a Hermitian column, B2)
+    auto unpack = [&](float2 (&v)[16], int hrow) {
+#pragma unroll
+        for (int e = 0; e < 16; e++) {
+            if (ZM && e >= 6 && e <= 9) { v[e] = make_float2(0.f, 0.f); continue; }
+            if (PADDED) {
+                const float4 hv = sg[(e < 8) ? t + C::TPF * e : N - C::TPF * e - t];   // past ncol: zeros
+                v[e] = (e < 8) ? make_float2(hv.x - hv.w, hv.y + hv.z) : make_float2(hv.x + hv.w, hv.z - hv.y);
+            } else {
+                const int c = t + C::TPF * e;
+                const int cc = (e < 8) ? c : N - c;
+                float4 hv = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (cc < p.ncol) hv = sg[RP ? rp_entry(cc, hrow) : cc];
+                if (cc == 0 || cc == N / 2) v[e] = make_float2(hv.x, hv.z);
+                else if (e < 8) v[e] = make_float2(hv.x - hv.w, hv.y + hv.z);
+                else v[e] = make_float2(hv.x + hv.w, hv.z - hv.y);
+            }
+        }
+    };
+    for (int yb = grp * RPH; yb < N; yb += G2 * RPH) {
+      float2 vB[RP ? 16 : 1];                         // RP: the second row of the double row, held while the first is transformed
+#pragma unroll 1
+      for (int h = 0; h < RPH; h++) {
+        const int y = yb + h;
         float s2p[16], s4p[16];
 #ifndef RF_X_UNROLL
 #define RF_X_UNROLL 1
@@ -547,30 +615,25 @@ __global__ void __launch_bounds__(NT2, N >= 2048 ? 2 : 1) k_tree_rowfft_stats(co
 #pragma unroll kUnrollPairs
         for (int p2 = 0; p2 < TB / 2; p2++) {
             float2 v[16];
-            mbar_wait(&mbar[grp], phase);                        // the (row, pair) has landed
-            phase ^= 1u;
-            // Z[c] = H_a[c] + i H_b[c], Z[N - c] = conj(H_a[c]) + i conj(H_b[c]); the column pass stores exact zeros in
-            // the imaginary parts of column 0 (rounding noise of a Hermitian column, B2), so c = 0 needs no special case
-#pragma unroll
-            for (int e = 0; e < 16; e++) {
-                if (ZM) {
-                    if (e >= 6 && e <= 9) { v[e] = make_float2(0.f, 0.f); continue; }
-                    const float4 h = sg[(e < 8) ? t + C::TPF * e : N - C::TPF * e - t];   // past ncol: zeros
-                    v[e] = (e < 8) ? make_float2(h.x - h.w, h.y + h.z) : make_float2(h.x + h.w, h.z - h.y);
-                } else {
-                    const int c = t + C::TPF * e;
-                    const int cc = (e < 8) ? c : N - c;
-                    float4 h = make_float4(0.f, 0.f, 0.f, 0.f);
-                    if (cc < p.ncol) h = sg[cc];
-                    if (cc == 0 || cc == N / 2) v[e] = make_float2(h.x, h.z);
-                    else if (e < 8) v[e] = make_float2(h.x - h.w, h.y + h.z);
-                    else v[e] = make_float2(h.x + h.w, h.z - h.y);
+            if (!RP || h == 0) {
+                mbar_wait(&mbar[grp], phase);                    // the (row, pair) [RP: the double row] has landed
+                phase ^= 1u;
+                unpack(v, 0);
+                loads_arrived_before_release(v, &rel_scratch[warp]);
+                if constexpr (RP) {
+                    unpack(vB, 1);
+                    loads_arrived_before_release(vB, &rel_scratch[warp]);
                 }
-            }
-            fft_group_sync<C::TPF>(1 + grp);                     // staging buffer consumed
-            {   // prefetch the next (row, pair) of this group while this one is transformed
+                fft_group_sync<C::TPF>(1 + grp);                 // staging buffer consumed
+                // prefetch the next (row, pair) of this group while this one is transformed
                 const bool last_pair = p2 + 1 == TB / 2;
-                if (!last_pair || y + G2 < N) stage_next(p2 + 2 == TB / 2 || (TB == 2));
+                if (RP) { if (yb + G2 * RPH < N) stage_next(true); }
+                else if (!last_pair || y + G2 < N) stage_next(p2 + 2 == TB / 2 || (TB == 2));
+            } else {
+                if constexpr (RP) {
+#pragma unroll
+                    for (int e = 0; e < 16; e++) v[e] = vB[e];
+                }
             }
             fft_inverse<N, ZM, (N >= 2048)>(v, xb, tw, t, 1 + grp, twp);
             float a[16], s2[16];
@@ -608,6 +671,7 @@ __global__ void __launch_bounds__(NT2, N >= 2048 ? 2 : 1) k_tree_rowfft_stats(co
                 }
             }
         }
+      }
     }
     __syncthreads();
 
@@ -762,6 +826,7 @@ __global__ void __launch_bounds__(kThreads2, 1) k_tree_rowfft_power(const TreePa
     const int grp = tid / C::TPF, t = tid % C::TPF;
     float4* sg = stg + (size_t)grp * p.cpad;
     __shared__ __align__(8) uint64_t mbar[kMaxRowGroups];
+    __shared__ uint32_t rel_scratch[32];       // see loads_arrived_before_release
     auto stage = [&](int y, int p2) {
         const float4* src = reinterpret_cast<const float4*>(Hblk + ((size_t)y * (TB / 2) + p2) * p.cpad * 2);
         if (t == 0) {
@@ -811,6 +876,7 @@ __global__ void __launch_bounds__(kThreads2, 1) k_tree_rowfft_power(const TreePa
                 else if (e < 8) v[e] = make_float2(h.x - h.w, h.y + h.z);
                 else v[e] = make_float2(h.x + h.w, h.z - h.y);
             }
+            loads_arrived_before_release(v, &rel_scratch[warp]);
             fft_group_sync<C::TPF>(1 + grp);
             {
                 const int np2 = (p2 + 1 == TB / 2) ? 0 : p2 + 1;

@@ -269,3 +269,37 @@ def test_wrong_device_or_knob_is_an_error():
         plan.set_tuning(R.binding.RF_TUNE_DM_GROUP, 0)
     plan.set_tuning(R.binding.RF_TUNE_DM_GROUP, 3)
     plan.destroy()
+
+
+@pytest.mark.parametrize("npix,radius", [(512, 130), (1024, 180)])
+def test_robust_sigma_when_rms_far_exceeds_mad(npix, radius):
+    """The case the robust sigma exists for (thresholding an image that holds a bright source): the
+    histogram of the row pass spans +-3.5 sigma_rms (B1), so its resolution in units of sigma_MAD degrades by
+    sigma_rms / sigma_MAD.  That ratio is bounded by the dirty beam: a single sample gives 1 (a fringe), the VLA-like
+    coverages of the configs 1.1-2.4, and the most concentrated beam a gridded snapshot can have -- a completely FILLED
+    aperture of `radius` cells, one sample per cell, built here on a lattice -- about 11 at 512^2 and 12 at 1024^2.  Even there
+    the S/N must stay within 1e-3 of the oracle and no image may report a histogram overflow."""
+    import torch
+    import paper_1802_03084_b200 as R
+    cell, f = 1.0e-4, np.array([1.4e9])
+    du = 1.0 / (npix * cell)
+    pts = [(a, b) for a in range(0, radius + 1) for b in range(-radius, radius + 1)
+           if a * a + b * b <= radius * radius and (a > 0 or b > 0)]
+    nbl = len(pts)
+    uvw = np.zeros((nbl, 3))
+    uvw[:, 0] = [(a + 0.1) * du * O.C_LIGHT / f[0] for a, _ in pts]
+    uvw[:, 1] = [(b - 0.2) * du * O.C_LIGHT / f[0] for _, b in pts]
+    nint, dms, dts, inttime = 6, np.array([0.0]), (1, 2), 0.005
+    rng = np.random.default_rng(npix)
+    vis = (0.01 * (rng.standard_normal((nint, nbl, 1, 2)) + 1j * rng.standard_normal((nint, nbl, 1, 2)))).astype(np.complex64)
+    vis = O.inject_transient(vis, f, uvw, inttime, cell, 1.0, 40, -25, 0.0, 2, 2).astype(np.complex64)
+    iu, iv, keep = O.cell_table(uvw, f, npix, cell)
+    assert keep.all() and len(set(zip(iu.ravel().tolist(), iv.ravel().tolist()))) == nbl      # one sample per cell
+    delays = O.delay_table(f, dms, inttime)
+    img = O.search_image(vis, delays, iu, iv, keep, npix, 0, 1, 2)
+    ratio = np.sqrt((img ** 2).mean()) / O.image_stats(img)[3]
+    assert ratio > 10.0, ratio
+    plan = R.Plan(f, uvw, 2, nint, inttime, npix, cell, dms, dts, 0.0)
+    g = _compare_all(plan, torch.from_numpy(vis).cuda(), vis, f, uvw, cell, npix, dms, dts, 0.0, inttime, min_match=8)
+    assert (int(g[(0, 0, 2)]["l_pix"]), int(g[(0, 0, 2)]["m_pix"])) == (40, -25)
+    plan.destroy()

@@ -398,3 +398,29 @@ def test_sigma_statistics_many_images():
     assert worst <= SNR_TOL, worst
     print("worst relative S/N deviation over 150 images:", worst)
     plan.destroy()
+
+
+@pytest.mark.parametrize("name,nint,ndm", [("sband", 200, 12), ("lband", 300, 16), ("hires", 40, 4)])
+def test_repeated_search_is_bit_identical(name, nint, ndm):
+    """The search has no order-dependent arithmetic (fixed summation order in the gridding, integer histograms), so
+    the same plan on the same segment must return bit-identical records every time.  Guards the hand-over of the
+    row pass's staging buffer to the bulk-copy engine (a missing cross-proxy fence shows up here as run-to-run
+    differences of 1e-5 in sigma at npix 1024) at the array sizes and geometries of configs 2-4."""
+    import dataclasses
+    torch = _torch()
+    import paper_1802_03084_b200 as R
+    cfg = dataclasses.replace(W.get_config(name), nint=nint, ndm=ndm)
+    f, uvw, dms = W.channel_freqs_hz(cfg), W.baseline_uvw_m(cfg), W.dm_list(cfg)
+    cell = W.default_cell_rad(cfg, uvw)
+    vis = W.make_segment(cfg)
+    d = torch.from_numpy(vis).cuda()
+    plan = R.Plan(f, uvw, cfg.npol, cfg.nint, cfg.inttime_s, cfg.npix, cell, dms, cfg.dt_list, 0.0)
+    if cfg.n_flagged:
+        plan.set_chan_weights(W.chan_weights(cfg))
+    runs = []
+    for _ in range(4):
+        g, n = plan.search(d, capacity=1 << 17)
+        assert n == len(g) == plan.num_images()
+        runs.append(np.sort(g, order=["dm_idx", "dt_idx", "t_idx"]).tobytes())
+    assert all(r == runs[0] for r in runs[1:])
+    plan.destroy()
