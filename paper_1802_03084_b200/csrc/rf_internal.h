@@ -29,9 +29,12 @@ constexpr int kThreads = 32 * kWarpsPerCta;
 constexpr int kDmGroup = 8;         // DM trials interleaved in time by the tree path's block order
 constexpr size_t kSlidingSumBudget = (size_t)24 << 30;   // bytes of sliding-sum arrays (widths off the tree) per plan
 constexpr int kUnitBlocks = 4;      // consecutive time blocks of a DM group kept together in the tree path's block order
+constexpr int kGatherBlocks = 2;    // consecutive time blocks of one DM served by one gather CTA (adjacent in every block list);
+                                    // 4 was measured no faster (L-band gather 5.69 vs 5.68 ms, S-band 209 vs 205 ms) and pads more
+static_assert(kUnitBlocks % kGatherBlocks == 0, "a unit of the block order holds whole gather groups");
 constexpr int kTreeUnroll = 8;      // iterations of the tree gather kept in flight per warp
 constexpr int kStreamIters = 64;    // target length of one warp stream of the tree gather
-constexpr float kHistRange = 3.5f;  // histogram covers +-kHistRange * sigma_rms
+constexpr float kHistRange = 3.5f;  // histogram covers +-kHistRange * sigma_rms (B1)
 
 // One image of the search loop: 16 bytes, device-resident list.
 struct ImgDesc {

@@ -109,7 +109,9 @@ int launch_batch(rf_plan* p, const SearchParams& sp, cudaStream_t st) {
 
 // ---------------------------------------------------------------- boxcar-tree path
 // 2048 bins at every size: the quantile error of the interpolated histogram shrinks with the pixel count (B1), and at
-// N >= 2048 (one 32-bit counter per bin and image) 4096 bins would cost the second row-pass CTA per SM
+// N >= 2048 (one 32-bit counter per bin and image) 4096 bins would cost the second row-pass CTA per SM.  Two
+// bank-partitioned copies of 1024 bins over +-1.75 sigma_rms (same bin width, lanes 0-15 / 16-31 on even / odd banks) were
+// measured SLOWER: row pass 19.6 vs 19.15 ms at 512^2, 728 vs 697 ms at 1024^2, 307 vs 298 ms at 4096^2.
 template <int N> int tree_nbins(int) { return 2048; }
 
 template <int N> size_t smem_tree1(int ntiles) {
@@ -161,10 +163,10 @@ int launch_tree(rf_plan* p, const TreeParams& tp, cudaStream_t st) {
     int rc;
     {
         auto kern = tp.part_major ? k_tree_gather<TB, true> : k_tree_gather<TB, false>;
-        const size_t smem = (size_t)p->nchan * sizeof(int) + (size_t)kWarpsPerCta * 2 * (2 * TB - 1) * sizeof(float);
-        if (tp.n_blk & 1) { set_error("internal: odd block count %d in a tree launch", tp.n_blk); return RF_ERR_STATE; }
+        const size_t smem = (size_t)p->nchan * sizeof(int) + (size_t)kWarpsPerCta * kGatherBlocks * (2 * TB - 1) * sizeof(float);
+        if (tp.n_blk % kGatherBlocks) { set_error("internal: block count %d of a tree launch is not a multiple of %d", tp.n_blk, kGatherBlocks); return RF_ERR_STATE; }
         if ((rc = mark(p, st, -1)) != RF_OK) return rc;
-        const dim3 grid = tp.part_major ? dim3(tp.n_blk / 2, tp.n_parts) : dim3(tp.n_parts, tp.n_blk / 2);
+        const dim3 grid = tp.part_major ? dim3(tp.n_blk / kGatherBlocks, tp.n_parts) : dim3(tp.n_parts, tp.n_blk / kGatherBlocks);
         kern<<<grid, kThreads, smem, st>>>(tp);
         RF_CUDA_CHECK(cudaGetLastError());
         if ((rc = mark(p, st, 3)) != RF_OK) return rc;
@@ -333,7 +335,7 @@ int ensure_tree_workspace(rf_plan* p) {
         blk_batch = (int)std::min<size_t>(4096, std::max<size_t>(1, budget / (h_per_blk * sizeof(float2))));
         if (blk_batch > sms) blk_batch -= blk_batch % sms;
     }
-    blk_batch = std::max(2, blk_batch & ~1);          // launches hold whole block pairs
+    blk_batch = std::max(kGatherBlocks, blk_batch / kGatherBlocks * kGatherBlocks);          // launches hold whole gather groups
     w.blk_batch = blk_batch;
     int rc_grow = grow(&w.Ht, &w.ht_elems, h_per_blk * blk_batch);
     if (rc_grow != RF_OK) return rc_grow;
@@ -350,7 +352,7 @@ int ensure_tree_workspace(rf_plan* p) {
         RF_CUDA_CHECK(cudaMalloc((void**)&w.sumsq_t, (ss_elems + ss_elems / 8) * sizeof(float)));
         w.ss_elems = ss_elems + ss_elems / 8;
     }
-    if (!w.dbg_block) RF_CUDA_CHECK(cudaMalloc((void**)&w.dbg_block, 2 * sizeof(BlockDesc)));
+    if (!w.dbg_block) RF_CUDA_CHECK(cudaMalloc((void**)&w.dbg_block, kGatherBlocks * sizeof(BlockDesc)));
     // phase-decimated sum arrays of the widths off the tree (configure_tree decided which): one after the other
     w.aux_off.assign(p->ndt + 1, 0);
     for (int k = 0; k < p->ndt; k++)
@@ -508,8 +510,8 @@ int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out
             int dev = 0, sms = 148;
             cudaGetDevice(&dev);
             cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-            small = std::min(small, sms) & ~1;
-            if (p->tune_feed_batch > 0) small = std::max(2, std::min(p->ws.blk_batch, p->tune_feed_batch) & ~1);
+            small = std::min(small, sms) / kGatherBlocks * kGatherBlocks;
+            if (p->tune_feed_batch > 0) small = std::max(kGatherBlocks, std::min(p->ws.blk_batch, p->tune_feed_batch) / kGatherBlocks * kGatherBlocks);
         }
         for (int64_t base = 0; base < p->n_blocks;) {
             int n = (int)std::min<int64_t>(p->ws.blk_batch, p->n_blocks - base);
@@ -568,14 +570,15 @@ int launch_debug_image(rf_plan* p, const void* vis, int dm_idx, int dt_idx, int 
         int nsearch = p->nint - p->h_maxdelay[dm_idx];
         if (p->span > 0) nsearch = std::min(nsearch, p->span);
         const int tb = t_idx / per;
-        BlockDesc b[2] = {{dm_idx, tb & ~1, nsearch, 0}, {dm_idx, tb | 1, nsearch, 0}};      // the block and its pair partner
+        BlockDesc b[kGatherBlocks];                       // the block and the others of its gather group
+        for (int h = 0; h < kGatherBlocks; h++) b[h] = {dm_idx, tb / kGatherBlocks * kGatherBlocks + h, nsearch, 0};
         RF_CUDA_CHECK(cudaMemcpyAsync(p->ws.dbg_block, b, sizeof(b), cudaMemcpyHostToDevice, st));
         RF_CUDA_CHECK(cudaStreamSynchronize(st));
         if ((rc = launch_prep(p, vis, st)) != RF_OK) return rc;
         TreeParams tp = tree_params(p);
         tp.blocks = p->ws.dbg_block;
-        tp.n_blk = 2;
-        tp.dbg_slot = tb & 1;
+        tp.n_blk = kGatherBlocks;
+        tp.dbg_slot = tb % kGatherBlocks;
         tp.image_out = image_dev;
         tp.stats_out = stats_dev;
         tp.dbg_img = tree_off(p->tree_tb, l) + t_idx % per;
@@ -587,15 +590,16 @@ int launch_debug_image(rf_plan* p, const void* vis, int dm_idx, int dt_idx, int 
         // node t_idx % TB of block t_idx / TB of this (dm, width)
         const int TB = p->tree_tb, tb = t_idx / TB;
         const int nj = p->h_num_t[(size_t)dm_idx * p->ndt + dt_idx];
-        BlockDesc b[2] = {{dm_idx, tb & ~1, nj, 0}, {dm_idx, tb | 1, nj, 0}};
+        BlockDesc b[kGatherBlocks];
+        for (int h = 0; h < kGatherBlocks; h++) b[h] = {dm_idx, tb / kGatherBlocks * kGatherBlocks + h, nj, 0};
         RF_CUDA_CHECK(cudaMemcpyAsync(p->ws.dbg_block, b, sizeof(b), cudaMemcpyHostToDevice, st));
         RF_CUDA_CHECK(cudaStreamSynchronize(st));
         if ((rc = launch_prep(p, vis, st)) != RF_OK) return rc;
         if ((rc = launch_phase_sum(p, dt_idx, st)) != RF_OK) return rc;
         TreeParams tp = aux_tree_params(p, tree_params(p), dt_idx);
         tp.blocks = p->ws.dbg_block;
-        tp.n_blk = 2;
-        tp.dbg_slot = tb & 1;
+        tp.n_blk = kGatherBlocks;
+        tp.dbg_slot = tb % kGatherBlocks;
         tp.image_out = image_dev;
         tp.stats_out = stats_dev;
         tp.dbg_img = t_idx % TB;
@@ -737,7 +741,7 @@ int launch_search_periodic(rf_plan* p, const void* vis, cudaStream_t st, rf_cand
         for (size_t i = c0; i < c1; i++) {
             const int nt = periodic_nt(p, dms[i]);
             for (int tb = 0; tb < nt / TB; tb++) {
-                if (dbg && (tb | 1) != (((dbg_k - 1) / nimg) | 1)) continue;      // the block and its pair partner
+                if (dbg && tb / kGatherBlocks != ((dbg_k - 1) / nimg) / kGatherBlocks) continue;      // the block's gather group
                 blocks.push_back({dms[i], tb, nt, (int)(i - c0)});
             }
         }
@@ -776,7 +780,7 @@ int launch_search_periodic(rf_plan* p, const void* vis, cudaStream_t st, rf_cand
         tp.image_out = power_dev;
         tp.stats_out = stats_dev;
         tp.dbg_img = (dbg_k - 1) % nimg;
-        tp.dbg_slot = ((dbg_k - 1) / nimg) & 1;
+        tp.dbg_slot = ((dbg_k - 1) / nimg) % kGatherBlocks;
     }
     for (size_t c = 0; c + 1 < chunk_first.size(); c++) {
         const size_t c0 = c * w.n_slabs, c1 = std::min(dms.size(), c0 + w.n_slabs);

@@ -279,7 +279,7 @@ int build_grid_lists(rf_plan* p) {
         return upload(p, &tl.group_cell, group_cell.data(), group_cell.size());
     };
     int rc = emit(p->d.gen, cols_per_group(N));
-    if (rc == RF_OK && p->tree_tb > 0) rc = emit_tree(p->d.tree, tree_cols_per_group(N, p->tree_tb), 16 / p->tree_tb);   // 2 TB lanes per entry
+    if (rc == RF_OK && p->tree_tb > 0) rc = emit_tree(p->d.tree, tree_cols_per_group(N, p->tree_tb), 32 / (kGatherBlocks * p->tree_tb));   // kGatherBlocks TB lanes per entry
     if (rc == RF_OK) RF_CUDA_CHECK(cudaStreamSynchronize(p->tab_stream));
     return rc;
 }
@@ -295,7 +295,7 @@ int tree_cols_per_group(int npix, int tb) {
 
 // Row pitch of the phase-decimated sum array of width dt: output integrations j' = t / dt of one series and phase,
 // plus the read-ahead of the last block pair and of the largest delay.
-int aux_pitch_of(const rf_plan* p, int dt) { return (((p->tpitch + dt - 1) / dt + 2 * p->tree_tb + 8) + 7) & ~7; }
+int aux_pitch_of(const rf_plan* p, int dt) { return (((p->tpitch + dt - 1) / dt + kGatherBlocks * p->tree_tb + 8) + 7) & ~7; }
 
 // Which widths off the tree are searched by the tree kernels on phase-decimated sums (B7): every width > 1 while the
 // sum arrays fit kSlidingSumBudget (each is about the size of the Stokes-I array); the rest takes the per-image path.
@@ -347,8 +347,8 @@ void configure_tree(rf_plan* p) {
         }
         if (p->tree_tb == 1) p->tree_tb = 2;      // the pair transform needs two integrations
     }
-    // read-ahead of the last block PAIR of a DM (the gather reads 2 TB integrations per entry)
-    p->tpitch = p->tree_tb ? ((p->nint + 2 * p->tree_tb + 15) / 16) * 16 : 0;
+    // read-ahead of the last block group of a DM (the gather reads kGatherBlocks TB integrations per entry)
+    p->tpitch = p->tree_tb ? ((p->nint + kGatherBlocks * p->tree_tb + 15) / 16) * 16 : 0;
     // gather entries hold (baseline * nchan + channel) * tpitch in 32 bits
     if (((unsigned long long)p->nbl * p->nchan + 1) * p->tpitch >= (1ull << 32)) {
         p->tree_tb = 0; p->tpitch = 0;
@@ -400,16 +400,16 @@ int build_image_list(rf_plan* p) {
             const int g1 = std::min(p->ndm, g0 + dm_group);
             int max_blk = 0;
             std::vector<int> nblk(g1 - g0, 0);
-            const int TB = p->tree_tb;
+            const int TB = p->tree_tb, GB = kGatherBlocks;
             for (int i = g0; i < g1; i++) {
                 const int nj = p->h_num_t[(size_t)order[i] * p->ndt + k];
-                nblk[i - g0] = nj > 0 ? (((nj + TB - 1) / TB) + 1) & ~1 : 0;    // blocks of TB images, even count (pairs)
+                nblk[i - g0] = nj > 0 ? (((nj + TB - 1) / TB) + GB - 1) / GB * GB : 0;    // blocks of TB images, whole gather groups
                 max_blk = std::max(max_blk, nblk[i - g0]);
             }
-            for (int tb = 0; tb < max_blk; tb += 2)
+            for (int tb = 0; tb < max_blk; tb += GB)
                 for (int i = g0; i < g1; i++)
                     if (tb < nblk[i - g0])
-                        for (int h = 0; h < 2; h++)      // nsearch field = number of valid images of this (dm, width)
+                        for (int h = 0; h < GB; h++)     // nsearch field = number of valid images of this (dm, width)
                             blocks2.push_back({order[i], tb + h, p->h_num_t[(size_t)order[i] * p->ndt + k], 0});
         }
     }
@@ -439,12 +439,13 @@ int build_image_list(rf_plan* p) {
     // launch never needs rows beyond the deadline of its last block (h_block_deadline).
     p->h_block_deadline.clear();
     if (p->tree_tb > 0) {
-        const int TB = p->tree_tb;
-        // blocks per DM, rounded up to an even count: the gather kernel serves PAIRS of consecutive time blocks
-        // (slots 2y, 2y + 1 of a launch); the padding block lies past the searched range and holds no valid image
+        const int TB = p->tree_tb, GB = kGatherBlocks;
+        // blocks per DM, rounded up to whole gather groups: the gather kernel serves GB consecutive time blocks
+        // (slots GB y ... GB y + GB - 1 of a launch); padding blocks lie past the searched range, hold no valid image
+        // and are skipped by the row pass
         std::vector<int> nblk(p->ndm, 0);
         for (int d = 0; d < p->ndm; d++)
-            if (in_tree_dm[d]) nblk[d] = (((nsearch_of[d] + TB - 1) / TB) + 1) & ~1;
+            if (in_tree_dm[d]) nblk[d] = (((nsearch_of[d] + TB - 1) / TB) + GB - 1) / GB * GB;
         struct Unit { int g0, tb, deadline; };
         std::vector<Unit> units;
         for (int g0 = 0; g0 < p->ndm; g0 += dm_group) {
@@ -462,11 +463,11 @@ int build_image_list(rf_plan* p) {
         std::stable_sort(units.begin(), units.end(), [](const Unit& a, const Unit& b) { return a.deadline < b.deadline; });
         for (const Unit& u : units) {
             const int g1 = std::min(p->ndm, u.g0 + dm_group);
-            for (int tb = u.tb; tb < u.tb + kUnitBlocks; tb += 2)
+            for (int tb = u.tb; tb < u.tb + kUnitBlocks; tb += GB)
                 for (int i = u.g0; i < g1; i++) {
                     const int d = order[i];
                     if (tb >= nblk[d]) continue;
-                    for (int h = 0; h < 2; h++) {
+                    for (int h = 0; h < GB; h++) {
                         blocks.push_back({d, tb + h, nsearch_of[d], 0});
                         p->h_block_deadline.push_back(u.deadline);
                     }

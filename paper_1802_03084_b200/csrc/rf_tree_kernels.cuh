@@ -130,35 +130,36 @@ __global__ void __launch_bounds__(256) k_phase_sum(const float2* __restrict__ vi
 }
 
 // ------------------------------------------------------------------------------------------
-// Tree pass 0: gather + grid.  grid = (n_parts, n_blk / 2); block = 256 = 8 warp streams.  Dynamic smem:
-//   sdelay [nchan] int | red [8][2][2*TB-1] float.
-// One CTA serves a PAIR of blocks: slots 2y and 2y + 1 of the launch are consecutive time blocks of the same
-// DM (build_image_list), i.e. 2 TB consecutive integrations.
-// "Time in lanes": lane = (entry j = lane / 2TB, block of the pair h = (lane / TB) & 1, integration q = lane % TB).
-// One iteration reads LG = 16/TB entries; the 2 TB dedispersed samples of an entry are ONE coalesced 16*TB-byte
-// read of visI[bl*nchan + ch][t0 + delay[ch] + 0 .. 2TB-1] (a warp load touches two 128-byte pieces instead of
-// four 64-byte ones: half the L1 wavefronts per byte).  The lane accumulates over the iterations of a cell in a
+// Tree pass 0: gather + grid.  grid = (n_blk / GB, n_parts) [cell-range major] with GB = kGatherBlocks = 2; block = 256
+// = 8 warp streams.  Dynamic smem:  sdelay [nchan] int | red [8][GB][2*TB-1] float.
+// One CTA serves GB consecutive time blocks of one DM: slots GB y ... GB y + GB - 1 of the launch (build_image_list),
+// i.e. GB TB consecutive integrations.
+// "Time in lanes": lane = (entry j = lane / (GB TB), block h = (lane / TB) % GB, integration q = lane % TB).
+// One iteration reads LG = 32 / (GB TB) entries; the GB TB dedispersed samples of an entry are ONE coalesced 8 GB TB-byte
+// read of visI[bl*nchan + ch][t0 + delay[ch] + 0 .. GB TB - 1] (TB = 8, GB = 2: 128 bytes; the delay is arbitrary, so a run
+// straddles one more 128-byte line than it fills).
+// The lane accumulates over the iterations of a cell in a
 // register; the END iteration sums the LG lane groups with xor shuffles and group 0 writes the cell
-// sum (TB contiguous complex values) to the compact grid.  Parseval sums of every boxcar-tree node,
+// sum (TB contiguous complex values per block) to the compact grid.  Parseval sums of every boxcar-tree node,
 // sum_cells w |sum_{q in node} G_q|^2, are taken at the same place (another log2(TB) xor steps over
 // q), so sigma_rms of every image of the block is known before any pixel exists.
 // No tile, no barriers inside the loop, few registers: latency is hidden by occupancy.
 template <int TB, bool PART_MAJOR>
 __global__ void __launch_bounds__(kThreads, 4) k_tree_gather(const TreeParams p) {
     constexpr int NIMG = 2 * TB - 1;
-    constexpr int LG = 16 / TB, U = kTreeUnroll;
+    constexpr int GB = kGatherBlocks, LG = 32 / (GB * TB), U = kTreeUnroll;
     constexpr int LEVELS = (TB == 8) ? 4 : (TB == 4 ? 3 : 2);      // log2(TB) + 1
     extern __shared__ __align__(16) unsigned char smem_raw[];
     int* sdelay = reinterpret_cast<int*>(smem_raw);
     float* red = reinterpret_cast<float*>(sdelay + p.nchan);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    // the pair (slot, slot + 1).  part_major: consecutive CTAs serve the SAME cell range (= the same (baseline, channel)
+    // the blocks slot ... slot + GB - 1.  part_major: consecutive CTAs serve the SAME cell range (= the same (baseline, channel)
     // series) for consecutive block pairs, whose windows overlap almost entirely (neighbouring DM trials, consecutive
     // times), so a series is fetched from HBM once per launch instead of once per pair
-    const int part = PART_MAJOR ? blockIdx.y : blockIdx.x, slot = 2 * (PART_MAJOR ? blockIdx.x : blockIdx.y);
+    const int part = PART_MAJOR ? blockIdx.y : blockIdx.x, slot = GB * (PART_MAJOR ? blockIdx.x : blockIdx.y);
     const BlockDesc blk = p.blocks[slot];
-    const int j = lane / (2 * TB), h = (lane / TB) & 1, q = lane % TB;
+    const int j = lane / (GB * TB), h = (lane / TB) % GB, q = lane % TB;
     const int s = part * kWarpsPerCta + warp;
     const bool has = s < p.n_streams;
     const int it_beg = has ? p.stream_iter[s] : 0;
@@ -207,7 +208,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_tree_gather(const TreeParams p)
             acc.y += __uint_as_float(__float_as_uint(x[u].y) ^ (e[u] & 0x80000000u));     // conjugate: bit 31
             if (e[u] & (1u << 29)) {                                      // warp-uniform: cell complete
 #pragma unroll
-                for (int d = 2 * TB; d < 32; d <<= 1) {
+                for (int d = GB * TB; d < 32; d <<= 1) {
                     acc.x += __shfl_xor_sync(0xffffffffu, acc.x, d);
                     acc.y += __shfl_xor_sync(0xffffffffu, acc.y, d);
                 }
@@ -229,14 +230,14 @@ __global__ void __launch_bounds__(kThreads, 4) k_tree_gather(const TreeParams p)
     if (j == 0) {
 #pragma unroll
         for (int l = 0; l < LEVELS; l++)
-            if ((q & ((1 << l) - 1)) == 0) red[(warp * 2 + h) * NIMG + tree_off(TB, l) + (q >> l)] = ps[l];
+            if ((q & ((1 << l) - 1)) == 0) red[(warp * GB + h) * NIMG + tree_off(TB, l) + (q >> l)] = ps[l];
     }
     __syncthreads();
-    if (tid < 2 * NIMG) {
+    if (tid < GB * NIMG) {
         const int hh = tid / NIMG, node = tid % NIMG;
         float tot = 0.f;
 #pragma unroll
-        for (int w = 0; w < kWarpsPerCta; w++) tot += red[(w * 2 + hh) * NIMG + node];
+        for (int w = 0; w < kWarpsPerCta; w++) tot += red[(w * GB + hh) * NIMG + node];
         p.sumsq[((size_t)(slot + hh) * NIMG + node) * p.n_parts + part] = tot * p.norm * p.norm;
     }
 }
@@ -529,6 +530,7 @@ __global__ void __launch_bounds__(NT2, N >= 2048 ? 2 : 1) k_tree_rowfft_stats(co
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int slot = blockIdx.x;
     const BlockDesc blk = p.blocks[slot];
+    if (blk.tb * TB >= blk.nsearch) return;          // padding block of a gather group: no image (uniform for the CTA)
     const float2* Hblk = p.Ht + (size_t)slot * N * p.cpad * TB;
     const int grp = tid / C::TPF, t = tid % C::TPF;
     float4* sg = stg + (size_t)grp * sgp;
