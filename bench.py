@@ -352,6 +352,7 @@ def measure(args, cfg, ctx):
     plan.set_profiling(False)
     launches = plan.get_counters()["kernel_launches"]
     n_cands = int(count.item())
+    alg = _alg_bytes(cfg, plan)                            # counters of the timed searches (device-counted images)
 
     # ---- end to end through the C-ABI with HOST buffers (pinned input, host candidate array)
     cand_host = np.empty(capacity, dtype=R.CAND_DTYPE)
@@ -387,7 +388,6 @@ def measure(args, cfg, ctx):
         dist.all_reduce(t_all, op=dist.ReduceOp.MAX)
     total_ms, e2e_ms = float(t_all[0]), float(t_all[1])
 
-    alg = _alg_bytes(cfg, plan)
     images = alg["images"]
     if alg["images_device_counted"] != images:
         raise SystemExit(f"the kernels finalised {alg['images_device_counted']} images, the plan lists {images}")

@@ -76,8 +76,8 @@ struct GridLists {
 // Work lists of the boxcar-tree path (built by build_grid_lists, see rf_tables.cu).
 struct TreeLists {
     uint2* entries = nullptr;        // device [n_iters * lg]
-    int32_t* stream_iter = nullptr;  // device [n_streams + 1] first iteration of each warp stream
-    int32_t* stream_cell = nullptr;  // device [n_streams + 1] first cell of each warp stream
+    int32_t* stream_iter = nullptr;  // device [n_streams][2] iteration range of each warp stream, longest streams first
+    int32_t* stream_cell = nullptr;  // device [n_streams] first cell of each warp stream
     uint32_t* cells = nullptr;       // device [n_cells] sorted by (column, row)
     int32_t* group_cell = nullptr;   // device [ngroups + 1] first cell of each column group
     int colgrp = 0, cpad = 0, ngroups = 0, lg = 0;

@@ -263,6 +263,24 @@ int build_grid_lists(rf_plan* p) {
         tl.n_cells = (int)cells.size();
         tl.n_streams = (int)stream_iter.size() - 1;
         tl.n_parts = (tl.n_streams + kWarpsPerCta - 1) / kWarpsPerCta;
+        // A cell cannot be split, so streams differ in length (a 848-sample cell alone is 424 iterations at S-band) and a
+        // gather CTA waits at its final barrier for its longest stream.  Streams are therefore handed out sorted by
+        // length: the 8 streams of a CTA are about equally long, and the long CTAs come first in the grid.
+        {
+            std::vector<int> order(tl.n_streams);
+            for (int i = 0; i < tl.n_streams; i++) order[i] = i;
+            std::stable_sort(order.begin(), order.end(), [&](int a, int b) {
+                return stream_iter[a + 1] - stream_iter[a] > stream_iter[b + 1] - stream_iter[b];
+            });
+            std::vector<int32_t> it2(2 * (size_t)tl.n_streams), c2(tl.n_streams);
+            for (int i = 0; i < tl.n_streams; i++) {
+                it2[2 * i] = stream_iter[order[i]];
+                it2[2 * i + 1] = stream_iter[order[i] + 1];
+                c2[i] = stream_cell[order[i]];
+            }
+            stream_iter.swap(it2);
+            stream_cell.swap(c2);
+        }
         int rc;
         // widths searched on phase-decimated sums: the same entries with that array's row pitch
         if ((int)p->d.aux_entries.size() != p->ndt) p->d.aux_entries.assign(p->ndt, nullptr);

@@ -27,8 +27,8 @@ struct TreeParams {
     const float2* visI;             // [nbl*nchan][tpitch]
     const int32_t* delay;           // [ndm][nchan]
     const uint2* entries;           // gather entries, [n_iters][LG]
-    const int32_t* stream_iter;     // [n_streams + 1]
-    const int32_t* stream_cell;     // [n_streams + 1]
+    const int32_t* stream_iter;     // [n_streams][2] first and past-the-last iteration of each warp stream (sorted by length)
+    const int32_t* stream_cell;     // [n_streams] first cell of each warp stream
     const uint32_t* cells;          // [n_cells]
     const int32_t* group_cell;      // [ngroups + 1]
     const BlockDesc* blocks;        // first block of this batch
@@ -162,8 +162,8 @@ __global__ void __launch_bounds__(kThreads, 4) k_tree_gather(const TreeParams p)
     const int j = lane / (GB * TB), h = (lane / TB) % GB, q = lane % TB;
     const int s = part * kWarpsPerCta + warp;
     const bool has = s < p.n_streams;
-    const int it_beg = has ? p.stream_iter[s] : 0;
-    const int it_end = has ? p.stream_iter[s + 1] : 0;
+    const int it_beg = has ? p.stream_iter[2 * s] : 0;
+    const int it_end = has ? p.stream_iter[2 * s + 1] : 0;
     int cell = has ? p.stream_cell[s] : 0;
     const int32_t* drow = p.delay + (size_t)(p.zero_row >= 0 ? p.zero_row : blk.dm_idx) * p.nchan;
     uint2 en[U];                           // entries of the next batch of iterations (prefetched)
