@@ -283,12 +283,7 @@ __device__ __forceinline__ void fft_inverse(float2 (&v)[16], float2* __restrict_
     fft_stage<N, C::R1, 1, false, ZMID>(v, sm, tw, tid);
     fft_group_sync<C::TPF>(bar_id);
     fft_reload<N>(v, sm, tid);
-#ifndef RF_X_NOSHFL
-#define RF_X_SHFL512 true
-#else
-#define RF_X_SHFL512 false
-#endif
-    if constexpr (N == 512 && RF_X_SHFL512) {
+    if constexpr (N == 512) {
         // second stage in registers (one butterfly per lane, k = lane & 15), third stage by shuffles
         apply_twiddle_powers<16>(v, tw[tid & 15]);
         bfly<16>(v);

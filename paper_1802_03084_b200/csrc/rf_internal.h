@@ -33,7 +33,9 @@ constexpr int kGatherBlocks = 2;    // consecutive time blocks of one DM served 
                                     // 4 was measured no faster (L-band gather 5.69 vs 5.68 ms, S-band 209 vs 205 ms) and pads more
 static_assert(kUnitBlocks % kGatherBlocks == 0, "a unit of the block order holds whole gather groups");
 constexpr int kTreeUnroll = 8;      // iterations of the tree gather kept in flight per warp
-constexpr int kStreamIters = 64;    // target length of one warp stream of the tree gather
+constexpr int kStreamIters = 256;   // target length of one warp stream of the tree gather.  Measured (gather per step, L-band /
+                                    // S-band, streams sorted by length): 32: 5.86 ms / 189 ms, 64: 5.19 / 164, 128: 4.77 / 150,
+                                    // 256: 4.63 / 143, 512: 4.77 / 139 -- a CTA's set-up and pipeline fill amortise over its streams
 constexpr float kHistRange = 3.5f;  // histogram covers +-kHistRange * sigma_rms (B1)
 
 // One image of the search loop: 16 bytes, device-resident list.

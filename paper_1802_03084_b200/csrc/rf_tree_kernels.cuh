@@ -494,11 +494,7 @@ template <int N, int TB, int NT2, bool ZM, bool RP = false>
 __global__ void __launch_bounds__(NT2, N >= 2048 ? 2 : 1) k_tree_rowfft_stats(const TreeParams p) {
     static_assert(!RP || TB == 2, "the row-pair hand-off holds one pair per row");
     constexpr int RPH = RP ? 2 : 1;                   // rows per staged item
-#ifdef RF_X_NOPAD
-    constexpr bool PADDED = false;
-#else
     constexpr bool PADDED = ZM && !RP;                // staging buffer zero-padded to 6 TPF columns: unconditional loads
-#endif
     constexpr int NWP = NT2 / 32;
     using C = FftCfg<N>;
     constexpr int G2 = NT2 / C::TPF;
@@ -610,11 +606,7 @@ __global__ void __launch_bounds__(NT2, N >= 2048 ? 2 : 1) k_tree_rowfft_stats(co
       for (int h = 0; h < RPH; h++) {
         const int y = yb + h;
         float s2p[16], s4p[16];
-#ifndef RF_X_UNROLL
-#define RF_X_UNROLL 1
-#endif
-        constexpr int kUnrollPairs = RF_X_UNROLL;
-#pragma unroll kUnrollPairs
+#pragma unroll 1
         for (int p2 = 0; p2 < TB / 2; p2++) {
             float2 v[16];
             if (!RP || h == 0) {
