@@ -151,7 +151,7 @@ int rf_plan_set_batch(rf_plan* plan, int images_per_batch);
  *   RF_TUNE_AUX_WIDTHS  0: widths off the boxcar tree take the per-image path instead of the tree
  *                          kernels on phase-decimated sums (B7); default 1
  *   RF_TUNE_DM_GROUP    DM trials interleaved in time by the block order (L2 locality); default 8
- *   RF_TUNE_FEED_BATCH  blocks per launch while rf_search_host's upload is in flight; 0 (default) = one wave
+ *   RF_TUNE_FEED_BATCH  blocks per launch while rf_search_host's upload is in flight; 0 (default) = two waves
  *   RF_TUNE_TREE_MAXPIX largest npix searched by the boxcar-tree kernels; default 4096            */
 #define RF_TUNE_AUX_WIDTHS  1
 #define RF_TUNE_DM_GROUP    2

@@ -160,7 +160,7 @@ struct rf_plan {
     // tuning knobs (rf_plan_set_tuning): none of them changes a result
     bool tune_aux = true;            // widths off the tree ride the tree kernels on phase-decimated sums (B7)
     int tune_dm_group = rf::kDmGroup;   // DM trials interleaved in time by the block order
-    int tune_feed_batch = 0;         // blocks per launch behind an upload (0 = one wave of row-pass CTAs)
+    int tune_feed_batch = 0;         // blocks per launch behind an upload (0 = two waves of row-pass CTAs)
     int tune_tree_maxpix = 4096;     // largest npix searched by the boxcar-tree kernels
     int tune_gather_order = 1;       // 1 = gather grid runs over block pairs fastest (cell-range major), 0 = cell ranges fastest
     std::map<const void*, size_t> smem_attr;   // dynamic shared memory opted in per kernel, on this plan's device

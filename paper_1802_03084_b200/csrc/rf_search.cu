@@ -499,18 +499,18 @@ int launch_search(rf_plan* p, const void* vis, cudaStream_t st, rf_cand_out* out
         tp.cand_items = out->items;
         tp.cand_count = out->count;
         tp.cand_capacity = out->capacity;
-        // behind an upload the launches start small (one wave of row-pass CTAs), so that the first ones wait for
-        // few integrations; once a launch needs the whole segment anyway the batches are full-sized
-        // behind an upload the launches start small (one wave of row-pass CTAs), so that the first ones wait for
+        // behind an upload the launches start small (two waves of row-pass CTAs), so that the first ones wait for
         // few integrations; once a launch needs the whole segment anyway the batches are full-sized.  Measured at L-band
-        // (end to end per segment): launches of 74 blocks 61.2 ms, 148 (one wave, the default) 44.8, 296 44.6, 592 46.0,
-        // the blocks that become searchable with each uploaded chunk 45.6.  rf_plan_set_tuning(RF_TUNE_FEED_BATCH, n).
+        // (end to end per segment, two runs): launches of 74 blocks 61.2 / 60.0 ms, 148 (one wave) 44.8 / 43.7, 296 44.6 / 43.1,
+        // 592 46.0 / 44.4, the blocks that become searchable with each uploaded chunk 45.6.  The floor of searching behind
+        // the upload is about 40 ms: half-way through the 28 ms upload only 27 % of the work is searchable (a DM trial
+        // needs its whole sweep), so the GPU idles early and finishes late.  rf_plan_set_tuning(RF_TUNE_FEED_BATCH, n).
         int small = p->ws.blk_batch;
         if (feed) {
             int dev = 0, sms = 148;
             cudaGetDevice(&dev);
             cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-            small = std::min(small, sms) / kGatherBlocks * kGatherBlocks;
+            small = std::min(small, 2 * sms) / kGatherBlocks * kGatherBlocks;
             if (p->tune_feed_batch > 0) small = std::max(kGatherBlocks, std::min(p->ws.blk_batch, p->tune_feed_batch) / kGatherBlocks * kGatherBlocks);
         }
         for (int64_t base = 0; base < p->n_blocks;) {
