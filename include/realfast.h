@@ -198,6 +198,24 @@ int rf_plan_set_mode(rf_plan* plan, int use_tree);
 int rf_plan_set_meansub(rf_plan* plan, int enable);
 int rf_prep_meansub(rf_plan* plan, void* vis_dev, void* cuda_stream);
 
+/* The same operation for callers that may not allocate (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): no plan, and no cudaMalloc / cudaFree / allocating library routine on any
+ * call.  Subtracts, IN PLACE in the caller's DEVICE buffer vis_dev (complex64 [nint][nbl][nchan][npol], 16-byte
+ * aligned, memory of the CURRENT CUDA device), the arithmetic mean over the nint integrations of every (baseline,
+ * channel, polarisation); bit-identical to rf_prep_meansub (same kernels, same order of the float64 sums).
+ * Enqueues three kernels on cuda_stream (0 = the default stream), never synchronises.
+ *   Scratch: the partial sums and the means live in one static device array inside the library, 136 bytes x
+ *   RF_STATIC_MAX_ELEMS = 25.5 MiB, which every GPU that loads the library holds until the process exits.
+ *   nbl*nchan*npol > RF_STATIC_MAX_ELEMS (e.g. the 1024-channel S-band segment) -> RF_ERR_ARG, nothing enqueued:
+ *   use rf_prep_meansub.  1 <= nint <= 2^21; npol in {1, 2, 4}.
+ *   Every call on a device shares that array: calls that OVERLAP on the GPU (two streams, two threads) race and
+ *   give wrong means; calls on one stream, or otherwise ordered, are fine.  The array keeps the last call's
+ *   contents; nothing in it needs clearing, because each call writes every word before reading it.
+ *   The first call on each device looks the array's address up (cudaGetSymbolAddress, which may load the module):
+ *   make one call before starting a stream capture.  vis_dev on another device or on the host -> RF_ERR_STATE. */
+#define RF_STATIC_MAX_ELEMS 196608   /* 3 * 2^16 >= 351 baselines x 256 channels x 2 polarisations */
+int rf_meansub_static(void* vis_dev, int nint, int nbl, int nchan, int npol, void* cuda_stream);
+
 /* Candidate cut-out, spectrum half ("candidate visualizations"; "image and
  * spectrum"; the image half is rf_debug_image).  Writes to DEVICE memory the float32
  * dynamic spectrum [2*half_window + 1][nchan] of the array phased towards pixel (l_pix, m_pix) (signed

@@ -6,4 +6,5 @@ from .binding import (  # noqa: F401
     RealfastError,
     lib_path,
     load_library,
+    meansub_static,
 )

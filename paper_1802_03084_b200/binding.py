@@ -23,8 +23,9 @@ EXPORTS = [
     "rf_search_host", "rf_plan_set_profiling", "rf_plan_get_kernel_times", "rf_plan_set_mode",
     "rf_plan_set_meansub", "rf_prep_meansub", "rf_cand_spectrum", "rf_inject",
     "rf_search_periodic", "rf_plan_periodic_nt", "rf_debug_periodic_image", "rf_plan_set_tuning",
-    "rf_plan_fft_work",
+    "rf_plan_fft_work", "rf_meansub_static",
 ]
+RF_STATIC_MAX_ELEMS = 196608     # include/realfast.h
 RF_TUNE_AUX_WIDTHS, RF_TUNE_DM_GROUP, RF_TUNE_FEED_BATCH, RF_TUNE_TREE_MAXPIX = 1, 2, 3, 4
 RF_TUNE_GATHER_ORDER = 5
 
@@ -85,6 +86,7 @@ def load_library() -> C.CDLL:
     lib.rf_plan_get_kernel_times.argtypes = [vp, C.POINTER(C.c_float), ip]
     lib.rf_plan_set_meansub.argtypes = [vp, C.c_int]
     lib.rf_prep_meansub.argtypes = [vp, vp, vp]
+    lib.rf_meansub_static.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, vp]
     lib.rf_inject.argtypes = [vp, vp, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int, C.c_int, vp]
     lib.rf_cand_spectrum.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, vp, vp]
     lib.rf_search_periodic.argtypes = [vp, vp, vp, C.POINTER(_CandOut)]
@@ -100,6 +102,18 @@ def load_library() -> C.CDLL:
 def _check(rc: int) -> None:
     if rc != RF_OK:
         raise RealfastError(f"realfast error {rc}: {load_library().rf_last_error().decode()}")
+
+
+def meansub_static(vis, stream=None) -> None:
+    """rf_meansub_static: rf_prep_meansub without a plan and without any allocation (scratch in a static device
+    array of the library; nbl*nchan*npol <= RF_STATIC_MAX_ELEMS; overlapping calls race).  vis: torch complex64
+    CUDA tensor [nint][nbl][nchan][npol], modified in place."""
+    import torch
+    assert vis.is_cuda and vis.dtype == torch.complex64 and vis.is_contiguous() and vis.dim() == 4
+    nint, nbl, nchan, npol = (int(n) for n in vis.shape)
+    st = torch.cuda.current_stream(vis.device) if stream is None else stream
+    with torch.cuda.device(vis.device):
+        _check(load_library().rf_meansub_static(vis.data_ptr(), nint, nbl, nchan, npol, st.cuda_stream))
 
 
 def _dptr(a: np.ndarray):

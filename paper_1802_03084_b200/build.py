@@ -17,7 +17,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "librealfast_b200.so")
 STAMP = LIB + ".srchash"
-SOURCES = ["rf_api.cu", "rf_tables.cu", "rf_search.cu", "rf_prep.cu", "rf_cutout.cu"]
+SOURCES = ["rf_api.cu", "rf_tables.cu", "rf_search.cu", "rf_prep.cu", "rf_cutout.cu", "rf_static.cu"]
 HEADERS = ["rf_internal.h", "rf_fft.cuh", "rf_kernels.cuh", "rf_tree_kernels.cuh",
            os.path.join("..", "..", "include", "realfast.h")]
 NVCC_FLAGS = [
