@@ -115,7 +115,9 @@ def _fft_rate(cfg, plan, k_ms, sm_mhz):
     return {"convention": "5 N log2 N per N-point complex transform actually run", "column_transforms": n_col,
             "row_pair_transforms": n_row, "flop_per_step": (n_col + n_row) * per, "column_pass_tflops": col,
             "row_pass_tflops": row, "both_passes_tflops": tot, "fp32_peak_tflops": peak, "frac_of_fp32_peak": tot / peak,
-            "note": "the row-pass kernel also holds the statistics, the column-pass kernel the scatter and the hand-off store"}
+            "note": "the row-pass kernel also holds the statistics, the column-pass kernel the scatter and the hand-off store; "
+                    "at npix >= 2048 the column pass is a pruned DFT over the occupied cells of each uv column "
+                    "(k_tree_coldft), so its rate is the rate of the FFTs it replaces, not of operations executed"}
 
 
 def _cpu_model():

@@ -27,7 +27,7 @@ EXPORTS = [
 ]
 RF_STATIC_MAX_ELEMS = 196608     # include/realfast.h
 RF_TUNE_AUX_WIDTHS, RF_TUNE_DM_GROUP, RF_TUNE_FEED_BATCH, RF_TUNE_TREE_MAXPIX = 1, 2, 3, 4
-RF_TUNE_GATHER_ORDER = 5
+RF_TUNE_GATHER_ORDER, RF_TUNE_COL_DFT = 5, 6
 
 # numpy view of rf_cand (32 bytes)
 CAND_DTYPE = np.dtype([("dm_idx", "<i4"), ("dt_idx", "<i4"), ("t_idx", "<i4"), ("l_pix", "<i4"),

@@ -46,7 +46,7 @@ int check_device(const rf_plan* p) {
 void free_tables(rf_plan* p) {
     rf::DeviceTables& d = p->d;
     cudaFree(d.delay); cudaFree(d.cell); cudaFree(d.keep); cudaFree(d.gen.entries); cudaFree(d.gen.warp_chunk);
-    cudaFree(d.tree.entries); cudaFree(d.tree.cells); cudaFree(d.tree.stream_iter); cudaFree(d.tree.stream_cell); cudaFree(d.tree.group_cell); cudaFree(d.blocks); cudaFree(d.blocks2);
+    cudaFree(d.tree.entries); cudaFree(d.tree.cells); cudaFree(d.tree.stream_iter); cudaFree(d.tree.stream_cell); cudaFree(d.tree.group_cell); cudaFree(d.tree.dft_blk); cudaFree(d.tree.dft_off); cudaFree(d.blocks); cudaFree(d.blocks2);
     for (uint2* e : d.aux_entries) cudaFree(e); cudaFree(d.images); cudaFree(d.freqs); cudaFree(d.uvw); cudaFree(d.dms); cudaFree(d.weights); cudaFree(d.twiddles); cudaFree(d.twp);
     p->dev_cap.clear();
     d = rf::DeviceTables{};
@@ -269,6 +269,10 @@ int rf_plan_set_tuning(rf_plan* p, int knob, int value) {
             break;
         case RF_TUNE_GATHER_ORDER:
             p->tune_gather_order = value != 0;
+            return RF_OK;
+        case RF_TUNE_COL_DFT:
+            if (value < 0 || value > rf::kDftMaxSpc) { set_error("blocks per column-pass CTA must be in 0..%d", rf::kDftMaxSpc); return RF_ERR_ARG; }
+            p->tune_col_dft = value;
             return RF_OK;
         default: set_error("unknown tuning knob %d", knob); return RF_ERR_ARG;
     }

@@ -80,10 +80,14 @@ struct TreeLists {
     uint2* entries = nullptr;        // device [n_iters * lg]
     int32_t* stream_iter = nullptr;  // device [n_streams][2] iteration range of each warp stream, longest streams first
     int32_t* stream_cell = nullptr;  // device [n_streams] first cell of each warp stream
-    uint32_t* cells = nullptr;       // device [n_cells] sorted by (column, row)
+    uint32_t* cells = nullptr;       // device [n_cells] sorted by (column, row mod 16, row)
     int32_t* group_cell = nullptr;   // device [ngroups + 1] first cell of each column group
     int colgrp = 0, cpad = 0, ngroups = 0, lg = 0;
     int n_cells = 0, n_streams = 0, n_parts = 0;   // n_parts = gather CTAs per block
+    int max_group_cells = 0;         // most cells in one column group
+    int32_t* dft_blk = nullptr;      // device, npix >= 2048: list blocks of k_tree_coldft, one per column group
+    int32_t* dft_off = nullptr;      // device [ngroups + 1] first int of each block
+    int dft_max_blk = 0;             // ints in the longest block
     int64_t n_iters = 0;
 };
 
@@ -162,6 +166,8 @@ struct rf_plan {
     int tune_dm_group = rf::kDmGroup;   // DM trials interleaved in time by the block order
     int tune_feed_batch = 0;         // blocks per launch behind an upload (0 = two waves of row-pass CTAs)
     int tune_tree_maxpix = 4096;     // largest npix searched by the boxcar-tree kernels
+    int tune_col_dft = 6;            // npix >= 2048: column pass as a pruned DFT over the occupied cells (k_tree_coldft), a CTA
+                                     // keeps one column group for this many blocks of a launch; 0 = column FFTs
     int tune_gather_order = 1;       // 1 = gather grid runs over block pairs fastest (cell-range major), 0 = cell ranges fastest
     std::map<const void*, size_t> smem_attr;   // dynamic shared memory opted in per kernel, on this plan's device
     std::vector<double> freqs, uvw, dms;
@@ -216,6 +222,7 @@ int build_grid_lists(rf_plan* p);             // host binning of the cell table 
 int aux_pitch_of(const rf_plan* p, int dt);   // row pitch of the phase-decimated sum array of a width
 int build_image_list(rf_plan* p);             // (dm, dt, j) loop -> d.images (generic) + d.blocks (tree)
 size_t phase_sum_smem(int dt, int* jc_out);   // dynamic shared memory (and JC) of k_phase_sum for a width
+constexpr int kDftMaxSpc = 64;        // k_tree_coldft: most blocks of a launch one CTA walks (RF_TUNE_COL_DFT)
 constexpr size_t kMaxDynSmem = 227 * 1024;    // opt-in limit per CTA on sm_100a
 // cudaFuncSetAttribute(MaxDynamicSharedMemorySize) once per (plan = device, kernel); kernels are per-device objects
 int ensure_smem_attr(rf_plan* p, const void* kern, size_t smem);

@@ -174,7 +174,27 @@ int launch_tree(rf_plan* p, const TreeParams& tp, cudaStream_t st) {
     // row-pair hand-off (one column per column-pass CTA, three CTAs per SM): transient search at N >= 2048 with TB = 2;
     // the periodicity search keeps the plain layout its power kernel reads
     const bool rp = row_pair_layout<N, TB>() && tp.zero_row < 0;
-    {
+    bool dft = false;
+    if constexpr (N >= 2048) {
+        // pruned DFT over the occupied cells of every uv column (k_tree_coldft); units of N/16 threads = (column, pair),
+        // a CTA keeps one column group for tune_col_dft blocks of the launch
+        constexpr int M1 = N / 16, PAIRS = TB / 2;
+        constexpr int NP = (256 / (M1 * NCOL) >= PAIRS) ? PAIRS : (256 / (M1 * NCOL) >= 1 ? 256 / (M1 * NCOL) : 1);
+        static_assert(PAIRS % NP == 0, "the pairs of a block split evenly over blockIdx.z");
+        const size_t smem = (size_t)kDftStages * (tp.ncmax + 1) * TB * sizeof(float2) + (size_t)tp.dft_max_blk * sizeof(int);
+        // a geometry with a very full column group (the buffers of its cells must leave room for two CTAs per SM) keeps the FFTs
+        dft = p->tune_col_dft > 0 && tp.dft_blk != nullptr && smem <= (size_t)100 * 1024;
+        if (dft) {
+            void (*kern)(const TreeParams, int) = k_tree_coldft<N, TB, NCOL, NP, false>;
+            if constexpr (row_pair_layout<N, TB>()) { if (rp) kern = k_tree_coldft<N, TB, NCOL, NP, true>; }
+            const int spc = p->tune_col_dft;
+            { const int rc_a = ensure_smem_attr(p, (const void*)kern, smem); if (rc_a != RF_OK) return rc_a; }
+            kern<<<dim3(tp.ngroups, (tp.n_blk + spc - 1) / spc, PAIRS / NP), M1 * NCOL * NP, smem, st>>>(tp, spc);
+            RF_CUDA_CHECK(cudaGetLastError());
+            if ((rc = mark(p, st, 0)) != RF_OK) return rc;
+        }
+    }
+    if (!dft) {
         constexpr int NTH = (N >= 4096 && QH * NCOL > 2) ? 512 : kThreads;   // 4 tiles of 4096: two concurrent transforms
         void (*kern)(const TreeParams) = k_tree_colfft<N, TB, NCOL, QH, NTH, false>;
         if constexpr (row_pair_layout<N, TB>()) { if (rp) kern = k_tree_colfft<N, TB, NCOL, QH, NTH, true>; }
@@ -250,6 +270,10 @@ TreeParams tree_params(rf_plan* p) {
     tp.n_parts = p->d.tree.n_parts;
     tp.twiddles = p->d.twiddles;
     tp.twp = p->d.twp;
+    tp.ncmax = p->d.tree.max_group_cells;
+    tp.dft_max_blk = p->d.tree.dft_max_blk;
+    tp.dft_blk = p->d.tree.dft_blk;
+    tp.dft_off = p->d.tree.dft_off;
     tp.part_major = p->tune_gather_order;
     tp.Ht = p->ws.Ht;
     tp.sumsq = p->ws.sumsq_t;

@@ -261,6 +261,8 @@ int build_grid_lists(rf_plan* p) {
         stream_cell.push_back((int32_t)cells.size());
         tl.n_iters = iters;
         tl.n_cells = (int)cells.size();
+        tl.max_group_cells = 0;
+        for (int g = 0; g < tl.ngroups; g++) tl.max_group_cells = std::max(tl.max_group_cells, group_cell[g + 1] - group_cell[g]);
         tl.n_streams = (int)stream_iter.size() - 1;
         tl.n_parts = (tl.n_streams + kWarpsPerCta - 1) / kWarpsPerCta;
         // A cell cannot be split, so streams differ in length (a 848-sample cell alone is 424 iterations at S-band) and a
@@ -290,6 +292,39 @@ int build_grid_lists(rf_plan* p) {
             for (uint2& e : e2) e.x = (e.x / (uint32_t)p->tpitch) * (uint32_t)p->aux_pitch[k];
             if ((rc = upload(p, &p->d.aux_entries[k], e2.data(), e2.size())) != RF_OK) return rc;
         }
+        // List blocks of the pruned column transform (k_tree_coldft, npix >= 2048), one per column group:
+        //   [first entry of (column, class) k = 0 .. 16 colgrp | pad to 4 ints][entries | 4 entries of read-ahead | pad to 4]
+        // entry = (row / 16) | (cell of the group + 1) << 8, sorted by (column, class = row mod 16) like the cells themselves;
+        // every class is padded to an even number of entries with 0 (= the zero cell in front of the staged values).
+        tl.dft_max_blk = 0;
+        if (N >= 2048) {
+            const int NK = kColsPerGroup * 16, hdr = (NK + 1 + 3) & ~3;
+            std::vector<int32_t> blk, off(tl.ngroups + 1, 0);
+            std::vector<int> cnt(NK), start(NK + 1);
+            for (int g = 0; g < tl.ngroups; g++) {
+                off[g] = (int32_t)blk.size();
+                const int cb = group_cell[g], nc = group_cell[g + 1] - cb;
+                std::fill(cnt.begin(), cnt.end(), 0);
+                auto key_of = [](uint32_t m) { return (int)((m >> 12) & 0xfu) * 16 + (int)(m & 0xfu); };
+                for (int i = 0; i < nc; i++) cnt[key_of(cells[cb + i])]++;
+                start[0] = 0;
+                for (int k = 0; k < NK; k++) start[k + 1] = start[k] + cnt[k] + (cnt[k] & 1);
+                const int total = start[NK];
+                const size_t base = blk.size();
+                blk.resize(base + hdr + (((size_t)total + 4 + 3) & ~(size_t)3), 0);
+                for (int k = 0; k <= NK; k++) blk[base + k] = start[k];
+                std::fill(cnt.begin(), cnt.end(), 0);
+                for (int i = 0; i < nc; i++) {
+                    const uint32_t m = cells[cb + i];
+                    const int k = key_of(m);
+                    blk[base + hdr + start[k] + cnt[k]++] = (int32_t)(((m & 0xfffu) >> 4) | ((uint32_t)(i + 1) << 8));
+                }
+                tl.dft_max_blk = std::max(tl.dft_max_blk, (int)(blk.size() - base));
+            }
+            off[tl.ngroups] = (int32_t)blk.size();
+            if ((rc = upload(p, &tl.dft_blk, blk.data(), blk.size())) != RF_OK) return rc;
+            if ((rc = upload(p, &tl.dft_off, off.data(), off.size())) != RF_OK) return rc;
+        }
         if ((rc = upload(p, &tl.entries, entries.data(), entries.size())) != RF_OK) return rc;
         if ((rc = upload(p, &tl.cells, cells.data(), cells.size())) != RF_OK) return rc;
         if ((rc = upload(p, &tl.stream_iter, stream_iter.data(), stream_iter.size())) != RF_OK) return rc;
@@ -297,6 +332,16 @@ int build_grid_lists(rf_plan* p) {
         return upload(p, &tl.group_cell, group_cell.data(), group_cell.size());
     };
     int rc = emit(p->d.gen, cols_per_group(N));
+    if (rc == RF_OK && p->tree_tb > 0) {
+        // the pruned column transform (k_tree_coldft) walks the cells of a column class by class (row mod 16)
+        std::sort(raw.begin(), raw.end(), [](const Raw& a, const Raw& b) {
+            if (a.col != b.col) return a.col < b.col;
+            if ((a.row & 15u) != (b.row & 15u)) return (a.row & 15u) < (b.row & 15u);
+            if (a.row != b.row) return a.row < b.row;
+            if (a.elem != b.elem) return a.elem < b.elem;
+            return a.conj < b.conj;
+        });
+    }
     if (rc == RF_OK && p->tree_tb > 0) rc = emit_tree(p->d.tree, tree_cols_per_group(N, p->tree_tb), 32 / (kGatherBlocks * p->tree_tb));   // kGatherBlocks TB lanes per entry
     if (rc == RF_OK) RF_CUDA_CHECK(cudaStreamSynchronize(p->tab_stream));
     return rc;

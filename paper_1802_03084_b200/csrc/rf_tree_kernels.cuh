@@ -46,6 +46,10 @@ struct TreeParams {
     int32_t dbg_img;                // -1 = off
     int32_t dbg_slot;               // block of the launch the debug outputs refer to
     int32_t tpitch, nchan, ncol, cpad, ngroups, nbins, n_blk, n_cells, n_streams, n_parts;
+    int32_t ncmax;                  // most cells in one column group (k_tree_coldft's value buffers)
+    int32_t dft_max_blk;            // ints in the longest list block
+    const int32_t* dft_blk;         // k_tree_coldft: list blocks of all column groups (rf_tables.cu)
+    const int32_t* dft_off;         // [ngroups + 1] first int of each block (multiples of 4)
     int32_t part_major;             // gather grid (host side): 1 = x runs over block pairs, y over cell ranges, 0 = x over cell ranges
     int32_t dec;                    // 1, or the width dt whose phase-decimated sum array visI points at (B7)
     uint32_t phase_stride;          // dec > 1: elements per phase = (nbl*nchan + 1) * row pitch
@@ -447,6 +451,9 @@ __device__ __forceinline__ void mbar_fence_init() {       // make the initialise
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
 __device__ __forceinline__ void bulk_copy_g2s(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(smem_u32(smem_dst)), "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)) : "memory");
@@ -478,6 +485,166 @@ constexpr int kMaxRowGroups = 32;       // transform groups per row-pass CTA (on
 // entries (16 bytes) of one group's staging buffer in the row pass
 template <int N, bool ZM> __host__ __device__ constexpr int row_stage_pitch(int cpad) {
     return ZM ? (cpad > 6 * (N / 16) + 4 ? cpad : 6 * (N / 16) + 4) : cpad;
+}
+
+// ------------------------------------------------------------------------------------------
+// Tree pass 1, sparse form (N >= 2048): the column transform as a PRUNED DFT.  A uv column of the 4096^2 half plane
+// holds 32 occupied cells on average out of 4096 (one (baseline, channel) track crosses a column once), so most of a
+// column FFT moves and adds zeros.  Split the row index v = 16 m + r (class r = v mod 16) and the output index
+// y = k1 + M1 k2 with M1 = N/16:
+//     e^{2 pi i v y / N} = e^{2 pi i m k1 / M1} * e^{2 pi i r k1 / N} * e^{2 pi i r k2 / 16},
+//     Y_r[k1]       = sum over the cells of class r of  x * e^{2 pi i m k1 / M1}          (direct, occupied cells only)
+//     X[k1 + M1 k2] = sum_r (Y_r[k1] W_N^{r k1}) e^{2 pi i r k2 / 16}                      (one radix-16 butterfly)
+// One thread owns one k1 of one (column, integration pair): 2 x 16 complex accumulators in registers, the cells
+// broadcast from shared memory, the twiddle e^{2 pi i (m k1 mod M1)/M1} from the special-function unit (exact angle).
+// No exchange through shared memory, no tile, no scatter; the 16 outputs of a thread are rows k1 + M1 k2 of the
+// hand-off, stored straight from registers.
+// A CTA keeps ONE column group and walks `spc` consecutive blocks of the launch (consecutive CTAs take the next groups
+// for the same blocks, so the 32-byte pieces of a hand-off line are written close together in time while the CTAs stay
+// roughly in step; more than ~6 blocks and they drift apart, the lines reach DRAM in pieces and the pass slows down).
+// The group's LIST BLOCK, built once per plan by rf_tables.cu, is copied once: the first entry of every (column, class)
+// and the entries (m | (cell + 1) << 8) sorted by class, every class padded to an even length with entry 0 = the zero
+// cell in front of the values, so the loop takes two cells per turn without a remainder.  The cell values of a block
+// (contiguous in the compact grid) arrive by one bulk copy, two turns ahead of the arithmetic.  The warps of a CTA
+// never meet at a barrier inside the loop: a buffer is `full` when its copy has landed and `empty` again when all warps
+// have arrived after their last read of it (two mbarriers per buffer).
+// grid = (ngroups, ceil(n_blk / spc), (TB/2) / NP); block = M1 * NCOL * NP: unit u = tid / M1 = (column u % NCOL, pair u / NCOL).
+// Dynamic smem: values [kDftStages][ncmax + 1][TB] float2 (cell 0 of each stays zero) | list block [dft_max_blk] int.
+constexpr int kDftStages = 3;         // buffers of k_tree_coldft: the copies run two turns ahead of the arithmetic
+__host__ __device__ constexpr int dft_list_header(int ncol) { return (ncol * 16 + 1 + 3) & ~3; }     // ints before the entries
+
+template <int N, int TB, int NCOL, int NP, bool RP>
+__global__ void __launch_bounds__((N / 16) * NCOL * NP) k_tree_coldft(const TreeParams p, const int spc) {
+    constexpr int M1 = N / 16, NTH = M1 * NCOL * NP, HDR = dft_list_header(NCOL);
+    static_assert(M1 == 256 || M1 == 128, "the low byte of m k1 is the twiddle index");
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const size_t xbytes = (size_t)(p.ncmax + 1) * TB * sizeof(float2);
+    const int* lblk = reinterpret_cast<const int*>(smem_raw + kDftStages * xbytes);      // the group's list block
+    __shared__ __align__(8) uint64_t full[kDftStages], empty[kDftStages], lfull;
+
+    const int tid = threadIdx.x;
+    const int g = blockIdx.x, pr0 = blockIdx.z * NP;
+    const int s0 = blockIdx.y * spc, ns = min(p.n_blk, s0 + spc) - s0;
+    const int c_beg = p.group_cell[g], nc = p.group_cell[g + 1] - c_beg;
+    const uint32_t vbytes = (uint32_t)nc * (TB * 8u);
+    if (tid < kDftStages) { mbar_init(&full[tid], 1); mbar_init(&empty[tid], NTH / 32); }
+    if (tid == kDftStages) mbar_init(&lfull, 1);
+    if (tid < kDftStages * (TB / 2))
+        reinterpret_cast<float4*>(smem_raw + (size_t)(tid / (TB / 2)) * xbytes)[tid % (TB / 2)] = make_float4(0.f, 0.f, 0.f, 0.f);
+    mbar_fence_init();
+    __syncthreads();
+    // turn n = block s0 + n uses buffer n % kDftStages
+    auto fill = [&](int n) {
+        const int b = n % kDftStages;
+        mbar_arrive_expect_tx(&full[b], vbytes);
+        bulk_copy_g2s(smem_raw + (size_t)b * xbytes + TB * 8, p.cellsum + ((size_t)(s0 + n) * p.n_cells + c_beg) * TB, vbytes, &full[b]);
+    };
+    if (tid == 0) {
+        const int off = p.dft_off[g];
+        const uint32_t lb = (uint32_t)(p.dft_off[g + 1] - off) * 4u;
+        mbar_arrive_expect_tx(&lfull, lb);
+        bulk_copy_g2s(smem_raw + kDftStages * xbytes, p.dft_blk + off, lb, &lfull);
+        if (nc > 0)
+            for (int n = 0; n < kDftStages - 1 && n < ns; n++) fill(n);
+    }
+
+    const int u = tid / M1, k1 = tid % M1;
+    const int c = u % NCOL, pp = u / NCOL, pr = pr0 + pp;
+    const float2 w1 = __ldg(p.twiddles + 16 + k1);         // exp(2 pi i k1 / N), k1 < 256
+    const float sc = p.norm;
+    const int col = g * NCOL + c;
+    const bool col0 = col == 0;
+    mbar_wait(&lfull, 0);
+    const int* ucls = lblk + c * 16;
+    const int* lst = lblk + HDR;
+    for (int n = 0; n < ns; n++) {
+        const int buf = n % kDftStages;
+        float4* Hs = reinterpret_cast<float4*>(p.Ht + (size_t)(s0 + n) * N * p.cpad * TB);
+        if (nc > 0 && tid == 0 && n + kDftStages - 1 < ns) {
+            // the buffer of turn n + kDftStages - 1 is the one turn n - 1 read: every warp has arrived on `empty` after its
+            // last read (a fresh barrier passes the wait for parity 1, so the first fill of a buffer does not block)
+            const int k = n + kDftStages - 1;
+            mbar_wait(&empty[k % kDftStages], ((k / kDftStages) & 1) ^ 1);
+            fill(k);
+        }
+        if (nc > 0) mbar_wait(&full[buf], (n / kDftStages) & 1);
+        const float4* ux = reinterpret_cast<const float4*>(smem_raw + (size_t)buf * xbytes) + pr;   // cell 0 = zeros, cell i + 1 = cell i of the group
+        auto x_of = [&](int e) { return ux[(e >> 8) * (TB / 2)]; };
+        // e^{2 pi i (m k1 mod M1) / M1}: the angle is an exact multiple of 2 pi / M1 below 2 pi, so the two special-function
+        // evaluations are good to ~5e-7 absolute (an M1-entry table in shared memory costs 3.5 wavefronts per read: the
+        // stride m k1 of a warp's 32 consecutive k1 conflicts for every m that is not odd)
+        auto tw_of = [&](int e) {
+            // j as a float without the conversion unit (it shares the special-function pipe): 2^23 + j is exact
+            const uint32_t prod = (uint32_t)(e * k1) & (M1 == 256 ? 0xffffffffu : 0xffffff7fu);
+            const float fj = __uint_as_float(__byte_perm(prod, 0x4B000000u, 0x7650));      // low byte of prod under 0x4B0000..
+            constexpr float kStep = 6.283185307179586f / (float)M1;
+            const float a = fmaf(fj, kStep, -8388608.f * kStep);
+            float2 w;
+            __sincosf(a, &w.y, &w.x);
+            return w;
+        };
+        float2 ya[16], yb[16];
+#pragma unroll
+        for (int r = 0; r < 16; r++) { ya[r] = make_float2(0.f, 0.f); yb[r] = make_float2(0.f, 0.f); }
+        {
+            int i = ucls[0];
+            int e0 = lst[i], e1 = lst[i + 1];
+            float4 x0 = x_of(e0), x1 = x_of(e1);
+            float2 w0 = tw_of(e0), w1c = tw_of(e1);
+#pragma unroll
+            for (int r = 0; r < 16; r++) {
+                const int end = ucls[r + 1];
+#pragma unroll 1
+                while (i < end) {                 // two cells per turn; the list is padded, the classes are even
+                    e0 = lst[i + 2];
+                    e1 = lst[i + 3];
+                    ya[r].x = fmaf(x0.x, w0.x, ya[r].x); ya[r].x = fmaf(-x0.y, w0.y, ya[r].x);
+                    ya[r].y = fmaf(x0.x, w0.y, ya[r].y); ya[r].y = fmaf(x0.y, w0.x, ya[r].y);
+                    yb[r].x = fmaf(x0.z, w0.x, yb[r].x); yb[r].x = fmaf(-x0.w, w0.y, yb[r].x);
+                    yb[r].y = fmaf(x0.z, w0.y, yb[r].y); yb[r].y = fmaf(x0.w, w0.x, yb[r].y);
+                    ya[r].x = fmaf(x1.x, w1c.x, ya[r].x); ya[r].x = fmaf(-x1.y, w1c.y, ya[r].x);
+                    ya[r].y = fmaf(x1.x, w1c.y, ya[r].y); ya[r].y = fmaf(x1.y, w1c.x, ya[r].y);
+                    yb[r].x = fmaf(x1.z, w1c.x, yb[r].x); yb[r].x = fmaf(-x1.w, w1c.y, yb[r].x);
+                    yb[r].y = fmaf(x1.z, w1c.y, yb[r].y); yb[r].y = fmaf(x1.w, w1c.x, yb[r].y);
+                    x0 = x_of(e0); w0 = tw_of(e0);
+                    x1 = x_of(e1); w1c = tw_of(e1);
+                    i += 2;
+                }
+            }
+        }
+        // the values of this turn are consumed: hand the buffer back (the loads fed the multiply-adds above, so they have
+        // arrived; the read-ahead past the list points at the zero cell, which no copy writes)
+        __syncwarp();
+        if (nc > 0 && (tid & 31) == 0) mbar_arrive(&empty[buf]);
+        // ---- twiddles W_N^{r k1} (with the normalisation folded in), radix-16 butterfly over the classes
+        {
+            float2 w[16];
+            w[1] = w1;
+#pragma unroll
+            for (int t = 2; t < 16; t++) w[t] = (t & 1) ? cmul(w[t - 1], w1) : cmul(w[t / 2], w[t / 2]);
+            ya[0] = make_float2(ya[0].x * sc, ya[0].y * sc);
+            yb[0] = make_float2(yb[0].x * sc, yb[0].y * sc);
+#pragma unroll
+            for (int t = 1; t < 16; t++) {
+                const float2 ws = make_float2(w[t].x * sc, w[t].y * sc);
+                ya[t] = cmul(ya[t], ws);
+                yb[t] = cmul(yb[t], ws);
+            }
+        }
+        bfly<16>(ya);
+        bfly<16>(yb);
+        // ---- store rows k1 + M1 k2 of H (layouts of k_tree_colfft); streaming: the row pass reads them a whole launch later
+        {
+#pragma unroll
+            for (int k2 = 0; k2 < 16; k2++) {
+                const int y = k1 + M1 * k2;
+                float4 o = make_float4(ya[k2].x, ya[k2].y, yb[k2].x, yb[k2].y);
+                if (col0) { o.y = 0.f; o.w = 0.f; }       // column 0 is Hermitian along v: its transform is real (B2)
+                if (RP) __stcs(&Hs[(((size_t)(y >> 1)) * (TB / 2) + pr) * p.cpad * 2 + rp_entry(col, y & 1)], o);
+                else __stcs(&Hs[((size_t)y * (TB / 2) + pr) * p.cpad + col], o);
+            }
+        }
+    }
 }
 
 constexpr int kThreads2 = 512;          // tree pass 2: one CTA of 16 warps per SM

@@ -258,6 +258,44 @@ def test_npix_2048_width_8_rides_the_phase_sums():
     plan.destroy()
 
 
+@pytest.mark.parametrize("dts", [(1, 2), (1, 2, 4)])
+def test_npix_2048_column_pass_forms_agree(dts):
+    """npix >= 2048 runs the column pass as a pruned DFT over the occupied cells of each uv column (k_tree_coldft);
+    RF_TUNE_COL_DFT = 0 keeps the column FFTs.  Both forms, with TB = 2 (row-pair hand-off) and TB = 4, against the
+    oracle on every image, and against each other record by record; several blocks per CTA and a ragged tail."""
+    import torch
+    import paper_1802_03084_b200 as R
+    npix, nint = 2048, 23
+    cfg, f, uvw, cell = _tiny_setup(npix)
+    dms = np.array([0.0, 45.0])
+    vis = _rand_vis((nint, cfg.nbl, cfg.nchan, 2), 2050 + len(dts))
+    vis = O.inject_transient(vis, f, uvw, cfg.inttime_s, cell, 1.0, -411, 640, 45.0, 2, 6).astype(np.complex64)
+    d = torch.from_numpy(vis).cuda()
+    lists = {}
+    for form in (4, 0, 1):
+        plan = R.Plan(f, uvw, 2, nint, cfg.inttime_s, npix, cell, dms, dts, 0.0)
+        plan.set_tuning(R.binding.RF_TUNE_COL_DFT, form)
+        g = _compare_all(plan, d, vis, f, uvw, cell, npix, dms, dts, 0.0, cfg.inttime_s, min_match=10)
+        assert len(g) == plan.num_images()
+        lists[form] = g
+        if form == 4:
+            delays = O.delay_table(f, dms, cfg.inttime_s)
+            iu, iv, keep = O.cell_table(uvw, f, npix, cell)
+            ref = O.search_image(vis, delays, iu, iv, keep, npix, 1, dts[-1], 1)
+            img, _ = plan.debug_image(d, 1, len(dts) - 1, 1)
+            assert np.abs(img - ref).max() <= PIX_TOL * np.sqrt((ref ** 2).mean())
+        plan.destroy()
+    for form in (0, 1):
+        assert set(lists[form]) == set(lists[4])
+        for key, c in lists[4].items():
+            o = lists[form][key]
+            assert abs(float(c["snr"]) - float(o["snr"])) <= 2e-4 * float(o["snr"]), (form, key)
+    plan2 = R.Plan(f, uvw, 2, nint, cfg.inttime_s, 2048, cell, dms, (1,), 6.0)
+    with pytest.raises(R.RealfastError):
+        plan2.set_tuning(R.binding.RF_TUNE_COL_DFT, 65)
+    plan2.destroy()
+
+
 def test_wrong_device_or_knob_is_an_error():
     import torch
     import paper_1802_03084_b200 as R
