@@ -296,6 +296,36 @@ def test_npix_2048_column_pass_forms_agree(dts):
     plan2.destroy()
 
 
+@pytest.mark.parametrize("cell_mult,u_scale,dts", [(70, 1e-3, (1, 2, 4)), (70, 1e-3, (1, 2)), (40, 0.03, (1, 2))])
+def test_npix_2048_dense_columns(cell_mult, u_scale, dts):
+    """Nearly north-south baselines and a wide field: the samples fall into a few uv columns that hold hundreds of cells
+    (column 0, with its Hermitian mirror, more than a thousand).  First case (TB = 4, two columns per group): three value
+    buffers of the pruned column DFT would exceed 100 KB, so the plan keeps the column FFTs for this geometry; second
+    case (TB = 2): the DFT runs on a column of > 1000 cells; third: on ~18 columns of 100-200 cells, many per row class.
+    Every image against the oracle."""
+    import torch
+    import paper_1802_03084_b200 as R
+    npix, nint = 2048, 11
+    cfg, f, uvw, cell = _tiny_setup(npix)
+    cell *= cell_mult
+    uvw = uvw.copy()
+    uvw[:, 0] *= u_scale
+    dms = np.array([0.0, 45.0])
+    vis = _rand_vis((nint, cfg.nbl, cfg.nchan, 2), 2060)
+    vis = O.inject_transient(vis, f, uvw, cfg.inttime_s, cell, 1.0, 5, 640, 45.0, 2, 3).astype(np.complex64)
+    d = torch.from_numpy(vis).cuda()
+    plan = R.Plan(f, uvw, 2, nint, cfg.inttime_s, npix, cell, dms, dts, 0.0)
+    g = _compare_all(plan, d, vis, f, uvw, cell, npix, dms, dts, 0.0, cfg.inttime_s, min_match=10)
+    assert len(g) == plan.num_images()
+    delays = O.delay_table(f, dms, cfg.inttime_s)
+    iu, iv, keep = O.cell_table(uvw, f, npix, cell)
+    assert keep.sum() > 1000 and np.abs(iu[keep]).max() <= (1 if u_scale < 0.01 else 40)
+    ref = O.search_image(vis, delays, iu, iv, keep, npix, 0, 1, 2)
+    img, _ = plan.debug_image(d, 0, 0, 2)
+    assert np.abs(img - ref).max() <= PIX_TOL * np.sqrt((ref ** 2).mean())
+    plan.destroy()
+
+
 def test_wrong_device_or_knob_is_an_error():
     import torch
     import paper_1802_03084_b200 as R
