@@ -151,7 +151,7 @@ int rf_search_host(rf_plan* p, const void* vis_host, rf_cand* cand_host, int32_t
     if (p->tree_tb > 0 && p->n_blocks > 0 && !p->meansub && p->n_kept > 0) {
         // The boxcar-tree search consumes the segment front to back: upload it in chunks on a copy stream and
         // let the search run behind the upload (each launch waits only for the integrations it reads).
-        const int rows = 64;
+        const int rows = 64;       // chunks of 32 integrations measured the same end to end (43.3 vs 43.3 ms at L-band), 128: 45.0 ms
         const int n_chunks = (p->nint + rows - 1) / rows;
         if (!p->copy_stream) RF_CUDA_CHECK(cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking));
         while ((int)p->chunk_done.size() < n_chunks) {
