@@ -158,9 +158,10 @@ int rf_plan_set_batch(rf_plan* plan, int images_per_batch);
 #define RF_TUNE_FEED_BATCH  3
 #define RF_TUNE_TREE_MAXPIX 4
 #define RF_TUNE_GATHER_ORDER 5  /* gather grid order: 1 (default) block pairs fastest, 0 cell ranges fastest      */
-#define RF_TUNE_COL_DFT     6  /* column pass of the tree kernels at npix >= 2048: n in 1..64 (default 6) pruned DFT
-                                   over the occupied cells of a uv column, a CTA keeps one column group for n
-                                   blocks of a launch; 0 column FFTs (same hand-off, same results within rounding) */
+#define RF_TUNE_COL_DFT     6  /* column pass of the transient search at npix >= 2048 with widths <= 2 on the tree: n in
+                                   1..64 (default 6) pruned DFT over the occupied cells of a uv column, a CTA keeps
+                                   one column group for n blocks of a launch; 0 column FFTs (same hand-off, same
+                                   results within rounding)                                                      */
 int rf_plan_set_tuning(rf_plan* plan, int knob, int value);
 
 /* End-to-end convenience entry with HOST buffers: copies the segment host->device into a

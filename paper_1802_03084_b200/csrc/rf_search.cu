@@ -175,18 +175,19 @@ int launch_tree(rf_plan* p, const TreeParams& tp, cudaStream_t st) {
     // the periodicity search keeps the plain layout its power kernel reads
     const bool rp = row_pair_layout<N, TB>() && tp.zero_row < 0;
     bool dft = false;
-    if constexpr (N >= 2048) {
+    if constexpr (row_pair_layout<N, TB>()) {
         // pruned DFT over the occupied cells of every uv column (k_tree_coldft); units of N/16 threads = (column, pair),
-        // a CTA keeps one column group for tune_col_dft blocks of the launch
+        // a CTA keeps one column group for tune_col_dft blocks of the launch.  Only with the row-pair hand-off, where two
+        // lanes fill a 32-byte sector: with the plain layout (TB = 4, or the periodicity search) every lane writes a lone
+        // 16-byte piece and the kernel measured 18.7 ms against 6.75 ms for the FFTs (npix 2048, TB = 4).
         constexpr int M1 = N / 16, PAIRS = TB / 2;
         constexpr int NP = (256 / (M1 * NCOL) >= PAIRS) ? PAIRS : (256 / (M1 * NCOL) >= 1 ? 256 / (M1 * NCOL) : 1);
         static_assert(PAIRS % NP == 0, "the pairs of a block split evenly over blockIdx.z");
         const size_t smem = (size_t)kDftStages * (tp.ncmax + 1) * TB * sizeof(float2) + (size_t)tp.dft_max_blk * sizeof(int);
         // a geometry with a very full column group (the buffers of its cells must leave room for two CTAs per SM) keeps the FFTs
-        dft = p->tune_col_dft > 0 && tp.dft_blk != nullptr && smem <= (size_t)100 * 1024;
+        dft = rp && p->tune_col_dft > 0 && tp.dft_blk != nullptr && smem <= (size_t)100 * 1024;
         if (dft) {
-            void (*kern)(const TreeParams, int) = k_tree_coldft<N, TB, NCOL, NP, false>;
-            if constexpr (row_pair_layout<N, TB>()) { if (rp) kern = k_tree_coldft<N, TB, NCOL, NP, true>; }
+            void (*kern)(const TreeParams, int) = k_tree_coldft<N, TB, NCOL, NP>;
             const int spc = p->tune_col_dft;
             { const int rc_a = ensure_smem_attr(p, (const void*)kern, smem); if (rc_a != RF_OK) return rc_a; }
             kern<<<dim3(tp.ngroups, (tp.n_blk + spc - 1) / spc, PAIRS / NP), M1 * NCOL * NP, smem, st>>>(tp, spc);

@@ -292,12 +292,12 @@ int build_grid_lists(rf_plan* p) {
             for (uint2& e : e2) e.x = (e.x / (uint32_t)p->tpitch) * (uint32_t)p->aux_pitch[k];
             if ((rc = upload(p, &p->d.aux_entries[k], e2.data(), e2.size())) != RF_OK) return rc;
         }
-        // List blocks of the pruned column transform (k_tree_coldft, npix >= 2048), one per column group:
+        // List blocks of the pruned column transform (k_tree_coldft, npix >= 2048 with TB = 2), one per column group:
         //   [first entry of (column, class) k = 0 .. 16 colgrp | pad to 4 ints][entries | 4 entries of read-ahead | pad to 4]
         // entry = (row / 16) | (cell of the group + 1) << 8, sorted by (column, class = row mod 16) like the cells themselves;
         // every class is padded to an even number of entries with 0 (= the zero cell in front of the staged values).
         tl.dft_max_blk = 0;
-        if (N >= 2048) {
+        if (N >= 2048 && p->tree_tb == 2) {
             const int NK = kColsPerGroup * 16, hdr = (NK + 1 + 3) & ~3;
             std::vector<int32_t> blk, off(tl.ngroups + 1, 0);
             std::vector<int> cnt(NK), start(NK + 1);

@@ -488,7 +488,7 @@ template <int N, bool ZM> __host__ __device__ constexpr int row_stage_pitch(int 
 }
 
 // ------------------------------------------------------------------------------------------
-// Tree pass 1, sparse form (N >= 2048): the column transform as a PRUNED DFT.  A uv column of the 4096^2 half plane
+// Tree pass 1, sparse form (N >= 2048 with TB = 2, the row-pair hand-off): the column transform as a PRUNED DFT.  A uv column of the 4096^2 half plane
 // holds 32 occupied cells on average out of 4096 (one (baseline, channel) track crosses a column once), so most of a
 // column FFT moves and adds zeros.  Split the row index v = 16 m + r (class r = v mod 16) and the output index
 // y = k1 + M1 k2 with M1 = N/16:
@@ -513,9 +513,10 @@ template <int N, bool ZM> __host__ __device__ constexpr int row_stage_pitch(int 
 constexpr int kDftStages = 3;         // buffers of k_tree_coldft: the copies run two turns ahead of the arithmetic
 __host__ __device__ constexpr int dft_list_header(int ncol) { return (ncol * 16 + 1 + 3) & ~3; }     // ints before the entries
 
-template <int N, int TB, int NCOL, int NP, bool RP>
+template <int N, int TB, int NCOL, int NP>
 __global__ void __launch_bounds__((N / 16) * NCOL * NP) k_tree_coldft(const TreeParams p, const int spc) {
     constexpr int M1 = N / 16, NTH = M1 * NCOL * NP, HDR = dft_list_header(NCOL);
+    static_assert(TB == 2, "writes the row-pair hand-off (two lanes fill one 32-byte sector); with the plain layout it loses to the FFTs");
     static_assert(M1 == 256 || M1 == 128, "the low byte of m k1 is the twiddle index");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const size_t xbytes = (size_t)(p.ncmax + 1) * TB * sizeof(float2);
@@ -633,15 +634,14 @@ __global__ void __launch_bounds__((N / 16) * NCOL * NP) k_tree_coldft(const Tree
         }
         bfly<16>(ya);
         bfly<16>(yb);
-        // ---- store rows k1 + M1 k2 of H (layouts of k_tree_colfft); streaming: the row pass reads them a whole launch later
+        // ---- store rows k1 + M1 k2 of H (row-pair layout of k_tree_colfft<..., RP>); streaming: the row pass reads them a whole launch later
         {
 #pragma unroll
             for (int k2 = 0; k2 < 16; k2++) {
                 const int y = k1 + M1 * k2;
                 float4 o = make_float4(ya[k2].x, ya[k2].y, yb[k2].x, yb[k2].y);
                 if (col0) { o.y = 0.f; o.w = 0.f; }       // column 0 is Hermitian along v: its transform is real (B2)
-                if (RP) __stcs(&Hs[(((size_t)(y >> 1)) * (TB / 2) + pr) * p.cpad * 2 + rp_entry(col, y & 1)], o);
-                else __stcs(&Hs[((size_t)y * (TB / 2) + pr) * p.cpad + col], o);
+                __stcs(&Hs[(((size_t)(y >> 1)) * (TB / 2) + pr) * p.cpad * 2 + rp_entry(col, y & 1)], o);
             }
         }
     }

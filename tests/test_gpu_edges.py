@@ -260,9 +260,10 @@ def test_npix_2048_width_8_rides_the_phase_sums():
 
 @pytest.mark.parametrize("dts", [(1, 2), (1, 2, 4)])
 def test_npix_2048_column_pass_forms_agree(dts):
-    """npix >= 2048 runs the column pass as a pruned DFT over the occupied cells of each uv column (k_tree_coldft);
-    RF_TUNE_COL_DFT = 0 keeps the column FFTs.  Both forms, with TB = 2 (row-pair hand-off) and TB = 4, against the
-    oracle on every image, and against each other record by record; several blocks per CTA and a ragged tail."""
+    """npix >= 2048 with TB = 2 (row-pair hand-off) runs the column pass as a pruned DFT over the occupied cells of each uv
+    column (k_tree_coldft); RF_TUNE_COL_DFT = 0 keeps the column FFTs, and so does TB = 4 whatever the knob says.  Every
+    setting against the oracle on every image, and against each other record by record; several blocks per CTA and a
+    ragged tail."""
     import torch
     import paper_1802_03084_b200 as R
     npix, nint = 2048, 23
@@ -299,9 +300,9 @@ def test_npix_2048_column_pass_forms_agree(dts):
 @pytest.mark.parametrize("cell_mult,u_scale,dts", [(70, 1e-3, (1, 2, 4)), (70, 1e-3, (1, 2)), (40, 0.03, (1, 2))])
 def test_npix_2048_dense_columns(cell_mult, u_scale, dts):
     """Nearly north-south baselines and a wide field: the samples fall into a few uv columns that hold hundreds of cells
-    (column 0, with its Hermitian mirror, more than a thousand).  First case (TB = 4, two columns per group): three value
-    buffers of the pruned column DFT would exceed 100 KB, so the plan keeps the column FFTs for this geometry; second
-    case (TB = 2): the DFT runs on a column of > 1000 cells; third: on ~18 columns of 100-200 cells, many per row class.
+    (column 0, with its Hermitian mirror, more than a thousand).  First case (TB = 4): column FFTs on these columns;
+    second (TB = 2): the pruned column DFT runs on a column of > 1000 cells; third: on ~18 columns of 100-200 cells, many
+    per row class.
     Every image against the oracle."""
     import torch
     import paper_1802_03084_b200 as R
@@ -323,6 +324,33 @@ def test_npix_2048_dense_columns(cell_mult, u_scale, dts):
     ref = O.search_image(vis, delays, iu, iv, keep, npix, 0, 1, 2)
     img, _ = plan.debug_image(d, 0, 0, 2)
     assert np.abs(img - ref).max() <= PIX_TOL * np.sqrt((ref ** 2).mean())
+    plan.destroy()
+
+
+@pytest.mark.parametrize("array", ["tiny", "lband"])
+def test_npix_4096_north_south_array(array):
+    """All baselines north-south at npix 4096: every sample lands in uv column 0, which with its Hermitian mirror then
+    holds ~1,800 cells for the 45-baseline array (the pruned column DFT runs on it: the largest list the kernel sees
+    in any test) and ~3,000 for the 351-baseline one (three value buffers would need > 100 KB, so the plan keeps the
+    column FFTs for that geometry).  Every image against the oracle."""
+    import torch
+    import paper_1802_03084_b200 as R
+    npix, nint, dts = 4096, 9, (1, 2)
+    cfg = W.get_config("tiny")
+    f = W.channel_freqs_hz(cfg)
+    uvw = W.baseline_uvw_m(W.get_config(array)).copy()
+    uvw[:, 0] *= 1e-5
+    cell = 1900.0 / (np.abs(uvw[:, 1]).max() * f.max() / 299792458.0 * npix)       # |iv| <= 1900 < npix / 2
+    dms = np.array([0.0, 45.0])
+    vis = _rand_vis((nint, uvw.shape[0], f.size, 2), 4097)
+    vis = O.inject_transient(vis, f, uvw, cfg.inttime_s, cell, 1.0, 3, -1500, 45.0, 1, 2).astype(np.complex64)
+    iu, iv, keep = O.cell_table(uvw, f, npix, cell)
+    rows = set((iv[keep] % npix).tolist()) | set((-iv[keep] % npix).tolist())
+    assert np.abs(iu[keep]).max() == 0 and (1500 < len(rows) < 1950 if array == "tiny" else len(rows) > 2200)
+    d = torch.from_numpy(vis).cuda()
+    plan = R.Plan(f, uvw, 2, nint, cfg.inttime_s, npix, cell, dms, dts, 0.0)
+    g = _compare_all(plan, d, vis, f, uvw, cell, npix, dms, dts, 0.0, cfg.inttime_s, min_match=8)
+    assert len(g) == plan.num_images()
     plan.destroy()
 
 
